@@ -1,0 +1,161 @@
+/*
+ * risp.h -- C ABI of the B200-native TDA-risp sigma-build library (librisp.so).
+ *
+ * Method: arxiv/paper_2603_29257 ("GPU Accelerated Minimal Auxiliary Basis Approach TDDFT
+ * for Large Organic Molecules").  Citations are PAPER.md:<line> of /root/reference/PAPER.md.
+ *
+ * The library computes, entirely in CUDA kernels for sm_100a and in FP64,
+ *
+ *     sigma_m = A X_m ,   A[ia,jb] = d_ij d_ab (e_a - e_i) + 2 (ia|jb) - (ij|J^|ab)        (Eq. 9-10)
+ *
+ * with (ia|jb) by RI in the Coulomb metric over an s+p auxiliary basis, evaluated AO-direct with the
+ * three-centre integrals regenerated on the fly (Eq. 11-17), and (ij|J^|ab) by RI over the
+ * K auxiliary subset with stored T_ij^P, T_ab^P tensors restricted to the energy window
+ * (Eq. 18-26); J^ = (alpha + beta erf(omega r12))/r12 (Eq. 25).  risp_tda_solve runs a
+ * Davidson loop whose subspace lives in pinned host memory.
+ *
+ * Conventions
+ *   - every call returns RISP_OK (0) or a negative RISP_E* code; nothing throws across the ABI;
+ *     risp_last_error() gives a text for the last failure on that context.
+ *   - units: bohr and Hartree; only `cutoff_ev` is in eV (1 Ha = 27.211386245988 eV).
+ *   - AO order inside a shell: s; p = (x, y, z); d = (xy, yz, z2, xz, x2-y2); unit-normalised real solid
+ *     harmonics; a contracted shell is sum_k c_k N(a_k,l) r^l exp(-a_k r^2) Y_lm, rescaled by the library to
+ *     unit norm (so `prim_coef` multiplies *unit-normalised primitives* and its overall scale is irrelevant).
+ *   - auxiliary functions (Eq. 4): unit-normalised primitive Cartesian Gaussians, l = 0 (one
+ *     function) or l = 1 (x, y, z).  Function index = running index over `aux_*` shells in the given order.
+ *     The caller supplies the exponents theta/R_A^2 and omits hydrogens.
+ *   - pointers in risp_system are HOST pointers, read during risp_setup only and never retained.
+ *   - one context per host thread at a time; no global state.
+ */
+#ifndef RISP_H
+#define RISP_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RISP_OK 0
+#define RISP_EINVAL (-1)   /* bad argument (NULL, negative size, l out of range, overlapping X/sigma, ...) */
+#define RISP_ENOMEM (-2)   /* device or pinned-host allocation failed */
+#define RISP_ECUDA (-3)    /* a CUDA call or kernel failed; see risp_last_error */
+#define RISP_ENOTPD (-4)   /* an auxiliary metric (P|Q) is not positive definite */
+#define RISP_ENOTCONV (-5) /* risp_tda_solve hit max_iter; outputs are still filled with the last Ritz pairs */
+
+typedef struct risp_ctx risp_ctx; /* opaque; owns every device and pinned allocation it makes */
+
+/* The problem, as the paper states it: a converged closed-shell SCF (geometry, AO basis, MO coefficients,
+ * orbital energies) plus the method parameters (aux exponents, Eq. 4; the K operator, Eq. 25;
+ * the exchange-space cutoff). */
+typedef struct {
+    int32_t natm;
+    const double *xyz_bohr;     /* [natm][3] */
+    const int32_t *Z;           /* [natm] nuclear charges (reporting only) */
+    int32_t nshl;               /* AO shells */
+    const int32_t *shl_atom;    /* [nshl] */
+    const int32_t *shl_l;       /* [nshl] 0, 1 or 2 */
+    const int32_t *shl_nprim;   /* [nshl] >= 1 */
+    const int32_t *shl_poff;    /* [nshl] offset of the shell's first primitive in prim_exp / prim_coef */
+    const double *prim_exp;
+    const double *prim_coef;
+    int32_t naux;               /* auxiliary shells (all of them enter J) */
+    const int32_t *aux_atom;    /* [naux] */
+    const int32_t *aux_l;       /* [naux] 0 or 1 */
+    const double *aux_exp;      /* [naux] */
+    const uint8_t *aux_in_K;    /* [naux] 1: shell also belongs to the K auxiliary set (paper: the s shells) */
+    int32_t nao, nocc, nvir;    /* nao = sum (2l+1); nocc + nvir <= nao */
+    const double *C;            /* [nao][nocc+nvir] row-major, occupied columns first */
+    const double *eps;          /* [nocc+nvir] Hartree, ascending within occ and within vir */
+    double alpha, beta, omega;  /* K operator (alpha + beta erf(omega r))/r; global hybrid: alpha = a_x, beta = 0 */
+    double cutoff_ev;           /* keep occ with eps > -cutoff and vir with eps < +cutoff;
+                                   <= 0 or +inf: no truncation */
+} risp_system;
+
+typedef struct {
+    double screen_tol;          /* shell-pair screening threshold tau (0 -> default 1e-13; < 0 -> keep every pair) */
+    size_t hbm_budget_bytes;    /* 0 -> 85 % of the free device memory at setup */
+    size_t host_budget_bytes;   /* pinned-host budget of the Davidson subspace; 0 -> 8 GiB */
+    int32_t device;             /* CUDA device ordinal */
+    int32_t flags;              /* reserved, 0 */
+} risp_options;
+
+typedef struct {
+    double tol;                 /* residual 2-norm threshold (0 -> 1e-5) */
+    int32_t max_iter;           /* 0 -> 100 */
+    int32_t n_guess;            /* initial unit vectors on the smallest e_a - e_i (0 -> 2*nroots) */
+    int32_t max_sub;            /* restart when the subspace would exceed this (0 -> 20*nroots) */
+    int32_t flags;              /* reserved, 0 */
+} risp_solve_options;
+
+#define RISP_MAX_ROOTS 64
+typedef struct {
+    int32_t iterations, restarts, n_sigma, converged;
+    double resid[RISP_MAX_ROOTS];        /* final residual norms */
+    double sec_total, sec_matvec, sec_subspace; /* wall seconds */
+    double bytes_h2d, bytes_d2h;         /* subspace traffic over the host link */
+    int32_t subspace_max;                /* largest subspace held */
+} risp_solve_info;
+
+typedef struct {
+    int32_t nao, nocc, nvir, nauxJ, nauxK; /* function counts */
+    int32_t noccK, nvirK, occK_first, virK_first; /* window: occupied [occK_first, occK_first+noccK), virtual likewise
+                                                     (indices within occ / within vir) */
+    int64_t n_shell_pairs, n_shell_pairs_kept, n_ao_pairs_kept;
+    int64_t bytes_Tij, bytes_Tab, bytes_device_total;
+    int32_t aux_chunk;                   /* K auxiliary functions per chunk in the matvec */
+} risp_dims;
+
+/* per-phase device seconds of the last risp_matvec (CUDA events; valid after the stream was synchronised) */
+typedef struct {
+    double total, j_transform_in, j_pass1, j_solve, j_pass2, j_transform_out, k_gather, k_gemm1, k_gemm2, assemble;
+    int32_t kernel_launches;
+} risp_timings;
+
+/* Build everything that does not depend on X: screened shell-pair list, metrics (P|Q)_J, (P|J^|Q)_K and their
+ * Cholesky factors, the window, and the tensors T_ij^P (Eq. 20), T_ab^P (Eq. 21).  Synchronous. */
+int risp_setup(const risp_system *sys, const risp_options *opt, risp_ctx **out);
+
+/* sigma = A X for a batch of m trial vectors.  X_dev, sigma_dev: DEVICE pointers, [m][nocc][nvir] row-major,
+ * sigma overwritten, X not modified, the two must not overlap.  Asynchronous on `cuda_stream` (a cudaStream_t;
+ * NULL = default stream). */
+int risp_matvec(risp_ctx *ctx, int32_t m, const double *X_dev, double *sigma_dev, void *cuda_stream);
+
+/* Same with HOST buffers: copies X in, runs risp_matvec, copies sigma out, synchronises. */
+int risp_matvec_host(risp_ctx *ctx, int32_t m, const double *X_host, double *sigma_host);
+
+/* Lowest `nroots` eigenpairs of A by a Davidson iteration whose subspace (V, W = A V) lives in pinned host
+ * memory and is streamed through the device on a side stream.  omega_hartree: HOST [nroots]
+ * ascending.  X_out: DEVICE [nroots][nocc][nvir] or NULL.  info may be NULL. */
+int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_options *opt, double *omega_hartree, double *X_out,
+                   risp_solve_info *info);
+
+void risp_destroy(risp_ctx *ctx);
+const char *risp_last_error(const risp_ctx *ctx); /* static text if ctx == NULL */
+
+/* ---- debug / parity getters (not timed) ---- */
+int risp_get_dims(const risp_ctx *ctx, risp_dims *out);
+int risp_get_timings(const risp_ctx *ctx, risp_timings *out);
+
+/* (shell_i shell_j | aux shell k) block, out_host[(2li+1)][(2lj+1)][nk] (nk = 1 or 3), computed by the same device
+ * integral code as the hot path.  op = 0: Coulomb 1/r (J); op = 1: the K operator of risp_system. */
+int risp_eri3c_shell(risp_ctx *ctx, int32_t shl_i, int32_t shl_j, int32_t aux_k, int32_t op, double *out_host);
+
+/* Intermediate of the LAST risp_matvec / setup, copied to out_host (HOST).  `which`: */
+#define RISP_STAGE_R 1       /* R_mQ (Eq. 14):  out[nauxJ][m]                                   sel ignored */
+#define RISP_STAGE_RTILDE 2  /* R~_mP (Eq. 15): out[nauxJ][m]                                                */
+#define RISP_STAGE_J 3       /* J_mia (Eq. 17): out[m][nocc][nvir]                                           */
+#define RISP_STAGE_K 4       /* K_mia (Eq. 23) scattered to the full space: out[m][nocc][nvir]               */
+#define RISP_STAGE_TIJ 5     /* T_ij^P for the K-aux functions P in sel: out[nsel][noccK][noccK]             */
+#define RISP_STAGE_TAB 6     /* T_ab^P:                                  out[nsel][nvirK][nvirK]             */
+#define RISP_STAGE_PAIRS 7   /* kept shell pairs as (shl_i, shl_j) int64 pairs: out = int64[n_kept][2]       */
+#define RISP_STAGE_METRIC_J 8 /* (P|Q)_J: out[nauxJ][nauxJ] */
+#define RISP_STAGE_METRIC_K 9 /* (P|J^|Q)_K: out[nauxK][nauxK] */
+#define RISP_STAGE_U 10      /* U^m (Eq. 16), dense AO matrix of vector sel[0]: out[nao][nao] */
+int risp_get_stage(risp_ctx *ctx, int32_t which, const int64_t *sel, int64_t nsel, void *out_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RISP_H */

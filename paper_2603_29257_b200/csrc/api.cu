@@ -1,0 +1,182 @@
+// api.cu -- the remaining C-ABI entry points of include/risp.h: teardown, error text, parity getters.
+#include "ctx.h"
+
+using namespace risp_eri;
+
+extern "C" void risp_destroy(risp_ctx *ctx)
+{
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+    double **bufs[] = {&ctx->d_C, &ctx->d_eps, &ctx->d_boys, &ctx->d_MJ, &ctx->d_LinvJ, &ctx->d_MK, &ctx->d_MKinv, &ctx->d_Tij, &ctx->d_Tab,
+                       &ctx->w_Y, &ctx->w_D, &ctx->w_dbar, &ctx->w_Rpart, &ctx->w_R, &ctx->w_Rt, &ctx->w_Rtmp, &ctx->w_J, &ctx->w_Xk, &ctx->w_Kk,
+                       &ctx->w_M, &ctx->w_Xin, &ctx->w_Sout};
+    for (auto b : bufs) if (*b) cudaFree(*b);
+    for (int c = 0; c < 6; ++c) if (ctx->cls[c].d_pairs) cudaFree(ctx->cls[c].d_pairs);
+    if (ctx->d_prims) cudaFree(ctx->d_prims);
+    if (ctx->d_cenJ) cudaFree(ctx->d_cenJ);
+    if (ctx->d_cenK) cudaFree(ctx->d_cenK);
+    if (ctx->ev_ok) for (int i = 0; i < 12; ++i) cudaEventDestroy(ctx->ev[i]);
+    if (ctx->side) cudaStreamDestroy(ctx->side);
+    delete ctx;
+}
+
+extern "C" const char *risp_last_error(const risp_ctx *ctx)
+{
+    if (!ctx) return "risp: no context (risp_setup was given a NULL argument or could not allocate)";
+    return ctx->err.c_str();
+}
+
+extern "C" int risp_get_dims(const risp_ctx *ctx, risp_dims *out)
+{
+    if (!ctx || !out) return RISP_EINVAL;
+    std::memset(out, 0, sizeof(*out));
+    out->nao = ctx->nao; out->nocc = ctx->nocc; out->nvir = ctx->nvir; out->nauxJ = ctx->nauxJ; out->nauxK = ctx->nauxK;
+    out->noccK = ctx->noccK; out->nvirK = ctx->nvirK; out->occK_first = ctx->occK0; out->virK_first = ctx->virK0;
+    out->n_shell_pairs = ctx->n_shell_pairs; out->n_shell_pairs_kept = ctx->n_shell_pairs_kept; out->n_ao_pairs_kept = ctx->n_ao_pairs_kept;
+    out->bytes_Tij = ctx->has_K ? (int64_t)ctx->nauxK * ctx->noccK * ctx->noccK * 8 : 0;
+    out->bytes_Tab = ctx->has_K ? (int64_t)ctx->nauxK * ctx->nvirK * ctx->nvirK * 8 : 0;
+    out->bytes_device_total = (int64_t)(ctx->setup_bytes + ctx->w_bytes);
+    out->aux_chunk = ctx->aux_chunk;
+    return RISP_OK;
+}
+
+extern "C" int risp_get_timings(const risp_ctx *cctx, risp_timings *out)
+{
+    risp_ctx *ctx = const_cast<risp_ctx *>(cctx);
+    if (!ctx || !out) return RISP_EINVAL;
+    std::memset(out, 0, sizeof(*out));
+    if (!ctx->last_m) return RISP_OK;
+    RISP_CUDA_TRY(cudaEventSynchronize(ctx->ev[8]));
+    auto el = [&](int a, int b) { float ms = 0; cudaEventElapsedTime(&ms, ctx->ev[a], ctx->ev[b]); return (double)ms * 1e-3; };
+    out->total = el(0, 8);
+    out->j_transform_in = el(0, 1); out->j_pass1 = el(1, 2); out->j_solve = el(2, 3); out->j_pass2 = el(3, 4); out->j_transform_out = el(4, 5);
+    out->k_gather = el(5, 6); out->k_gemm1 = el(6, 7); out->k_gemm2 = 0.0; out->assemble = el(7, 8);
+    out->kernel_launches = ctx->tim.kernel_launches;
+    return RISP_OK;
+}
+
+extern "C" int risp_eri3c_shell(risp_ctx *ctx, int32_t shl_i, int32_t shl_j, int32_t aux_k, int32_t op, double *out_host)
+{
+    if (!ctx) return RISP_EINVAL;
+    if (shl_i < 0 || shl_i >= ctx->nshl || shl_j < 0 || shl_j >= ctx->nshl || aux_k < 0 || aux_k >= (int)ctx->h_aux_l.size() || !out_host ||
+        (op != 0 && op != 1)) {
+        risp_set_error(ctx, "risp_eri3c_shell: index out of range");
+        return RISP_EINVAL;
+    }
+    RISP_CUDA_TRY(cudaSetDevice(ctx->device));
+    int A = shl_i, B = shl_j;
+    bool swapped = ctx->h_shl_l[A] < ctx->h_shl_l[B];
+    if (swapped) std::swap(A, B);
+    ShellPair sp;
+    std::vector<PrimPair> pp;
+    risp_build_pair(ctx, A, B, sp, pp, -1.0);
+    sp.aoA = 0; sp.aoB = 0;
+    const int la = ctx->h_shl_l[A], lb = ctx->h_shl_l[B], nfa = 2 * la + 1, nfb = 2 * lb + 1;
+    const int lk = ctx->h_aux_l[aux_k], nk = 2 * lk + 1;
+    AuxCentre c;
+    int at = ctx->h_aux_atom[aux_k];
+    c.x = ctx->h_xyz[3 * at]; c.y = ctx->h_xyz[3 * at + 1]; c.z = ctx->h_xyz[3 * at + 2];
+    c.g = ctx->h_aux_exp[aux_k];
+    c.ns = std::pow(2.0 * c.g / 3.14159265358979323846, 0.75);
+    c.np = c.ns * 2.0 * std::sqrt(c.g);
+    c.qs = lk == 0 ? 0 : -1; c.qp = lk == 1 ? 0 : -1;
+    ShellPair *d_sp = nullptr; PrimPair *d_pp = nullptr; AuxCentre *d_c = nullptr; double *d_out = nullptr;
+    RISP_CUDA_TRY(cudaMalloc((void **)&d_sp, sizeof(sp)));
+    RISP_CUDA_TRY(cudaMalloc((void **)&d_pp, pp.size() * sizeof(PrimPair)));
+    RISP_CUDA_TRY(cudaMalloc((void **)&d_c, sizeof(c)));
+    RISP_CUDA_TRY(cudaMalloc((void **)&d_out, (size_t)nk * nfa * nfb * sizeof(double)));
+    RISP_CUDA_TRY(cudaMemcpy(d_sp, &sp, sizeof(sp), cudaMemcpyHostToDevice));
+    RISP_CUDA_TRY(cudaMemcpy(d_pp, pp.data(), pp.size() * sizeof(PrimPair), cudaMemcpyHostToDevice));
+    RISP_CUDA_TRY(cudaMemcpy(d_c, &c, sizeof(c), cudaMemcpyHostToDevice));
+    OpParams o{1.0, 0.0, 0.0};
+    if (op == 1) o = OpParams{ctx->alpha, ctx->beta, ctx->omega * ctx->omega};
+    RISP_CUDA_TRY(risp_eri_fill(la, lb, lk == 1, op == 1, d_sp, 1, d_pp, d_c, 1, o, ctx->d_boys, d_out, (long long)nfa * nfb, nfb, 0, 0));
+    std::vector<double> h((size_t)nk * nfa * nfb);
+    RISP_CUDA_TRY(cudaMemcpy(h.data(), d_out, h.size() * sizeof(double), cudaMemcpyDeviceToHost));
+    cudaFree(d_sp); cudaFree(d_pp); cudaFree(d_c); cudaFree(d_out);
+    // h[k][a][b] -> out[i][j][k]
+    const int nfi = swapped ? nfb : nfa, nfj = swapped ? nfa : nfb;
+    for (int i = 0; i < nfi; ++i)
+        for (int j = 0; j < nfj; ++j)
+            for (int k = 0; k < nk; ++k) {
+                int a = swapped ? j : i, b = swapped ? i : j;
+                out_host[((size_t)i * nfj + j) * nk + k] = h[((size_t)k * nfa + a) * nfb + b];
+            }
+    return RISP_OK;
+}
+
+extern "C" int risp_get_stage(risp_ctx *ctx, int32_t which, const int64_t *sel, int64_t nsel, void *out_host)
+{
+    if (!ctx || !out_host) return RISP_EINVAL;
+    RISP_CUDA_TRY(cudaSetDevice(ctx->device));
+    RISP_CUDA_TRY(cudaDeviceSynchronize());
+    const int m = ctx->last_m;
+    double *out = (double *)out_host;
+    auto need_mv = [&]() { if (!m) { risp_set_error(ctx, "risp_get_stage: no risp_matvec has run"); return true; } return false; };
+    switch (which) {
+    case RISP_STAGE_R:
+    case RISP_STAGE_RTILDE: {
+        if (need_mv()) return RISP_EINVAL;
+        RISP_CUDA_TRY(cudaMemcpy2D(out, (size_t)m * 8, which == RISP_STAGE_R ? ctx->w_R : ctx->w_Rt, (size_t)RISP_MS * 8, (size_t)m * 8, ctx->nauxJ,
+                                   cudaMemcpyDeviceToHost));
+        return RISP_OK;
+    }
+    case RISP_STAGE_J:
+        if (need_mv()) return RISP_EINVAL;
+        RISP_CUDA_TRY(cudaMemcpy(out, ctx->w_J, (size_t)m * ctx->nocc * ctx->nvir * 8, cudaMemcpyDeviceToHost));
+        return RISP_OK;
+    case RISP_STAGE_K: {
+        if (need_mv()) return RISP_EINVAL;
+        size_t n = (size_t)m * ctx->nocc * ctx->nvir;
+        if (!ctx->has_K) { std::memset(out, 0, n * 8); return RISP_OK; }
+        double *tmp = nullptr;
+        RISP_CUDA_TRY(cudaMalloc((void **)&tmp, n * 8));
+        RISP_CUDA_TRY(risp_scatter_window(ctx->w_Kk, tmp, m, ctx->nocc, ctx->nvir, ctx->occK0, ctx->noccK, ctx->virK0, ctx->nvirK, 0));
+        RISP_CUDA_TRY(cudaMemcpy(out, tmp, n * 8, cudaMemcpyDeviceToHost));
+        cudaFree(tmp);
+        return RISP_OK;
+    }
+    case RISP_STAGE_TIJ:
+    case RISP_STAGE_TAB: {
+        if (!ctx->has_K || !sel) { risp_set_error(ctx, "risp_get_stage: no K tensors / no selection"); return RISP_EINVAL; }
+        const size_t no = ctx->noccK, nv = ctx->nvirK, nK = ctx->nauxK;
+        for (int64_t s = 0; s < nsel; ++s) {
+            if (sel[s] < 0 || sel[s] >= (int64_t)nK) { risp_set_error(ctx, "risp_get_stage: aux index out of range"); return RISP_EINVAL; }
+            if (which == RISP_STAGE_TIJ)
+                RISP_CUDA_TRY(cudaMemcpy2D(out + s * no * no, no * 8, ctx->d_Tij + sel[s] * no, nK * no * 8, no * 8, no, cudaMemcpyDeviceToHost));
+            else
+                RISP_CUDA_TRY(cudaMemcpy(out + s * nv * nv, ctx->d_Tab + sel[s] * nv * nv, nv * nv * 8, cudaMemcpyDeviceToHost));
+        }
+        return RISP_OK;
+    }
+    case RISP_STAGE_PAIRS:
+        std::memcpy(out_host, ctx->h_kept_pairs.data(), ctx->h_kept_pairs.size() * sizeof(long long));
+        return RISP_OK;
+    case RISP_STAGE_METRIC_J:
+        RISP_CUDA_TRY(cudaMemcpy(out, ctx->d_MJ, (size_t)ctx->nauxJ * ctx->nauxJ * 8, cudaMemcpyDeviceToHost));
+        return RISP_OK;
+    case RISP_STAGE_METRIC_K:
+        if (!ctx->has_K) { risp_set_error(ctx, "risp_get_stage: no K metric"); return RISP_EINVAL; }
+        RISP_CUDA_TRY(cudaMemcpy(out, ctx->d_MK, (size_t)ctx->nauxK * ctx->nauxK * 8, cudaMemcpyDeviceToHost));
+        return RISP_OK;
+    case RISP_STAGE_U: {
+        if (need_mv() || !sel || sel[0] < 0 || sel[0] >= m) return RISP_EINVAL;
+        RISP_CUDA_TRY(cudaMemcpy(out, ctx->w_D + sel[0] * (size_t)ctx->nao * ctx->nao, (size_t)ctx->nao * ctx->nao * 8, cudaMemcpyDeviceToHost));
+        return RISP_OK;
+    }
+    default:
+        risp_set_error(ctx, "risp_get_stage: unknown stage");
+        return RISP_EINVAL;
+    }
+}
+
+// Debug export (not part of the method): the DMMA GEMM on caller-provided DEVICE buffers, used by the GEMM unit test and
+// the FP64 tensor-rate measurement of bench.py.  C = alpha op(A) op(B) + beta C, see GemmDesc in common.cuh.
+extern "C" int risp_debug_dgemm(int M, int N, int K, const double *A, long long lda, int a_kc, const double *B, long long ldb, int b_kc, double *C,
+                                long long ldc, double alpha, double beta, int nbatch, long long sA, long long sB, long long sC, void *stream)
+{
+    GemmDesc d = gemm_desc(M, N, K, A, lda, a_kc != 0, B, ldb, b_kc != 0, C, ldc, alpha, beta);
+    d.nb1 = nbatch; d.sA1 = sA; d.sB1 = sB; d.sC1 = sC;
+    return risp_dgemm(d, (cudaStream_t)stream) == cudaSuccess ? RISP_OK : RISP_ECUDA;
+}

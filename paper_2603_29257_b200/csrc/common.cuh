@@ -1,0 +1,50 @@
+// common.cuh -- shared declarations of the librisp CUDA sources (sm_100a, FP64).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+#include "../../include/risp.h"
+
+#define RISP_CUDA_TRY(expr)                                                                         \
+    do {                                                                                            \
+        cudaError_t e_ = (expr);                                                                    \
+        if (e_ != cudaSuccess) {                                                                    \
+            risp_set_error(ctx, std::string(#expr) + ": " + cudaGetErrorString(e_) + " at " +       \
+                                    __FILE__ + ":" + std::to_string(__LINE__));                     \
+            return e_ == cudaErrorMemoryAllocation ? RISP_ENOMEM : RISP_ECUDA;                      \
+        }                                                                                           \
+    } while (0)
+
+struct risp_ctx;
+void risp_set_error(risp_ctx *ctx, const std::string &msg);
+
+// ---------------------------------------------------------------------------------------------------
+// FP64 tensor-core GEMM (DMMA m8n8k4), gemm.cu
+//   C[b](m,n) = alpha * sum_k A[b](m,k) B[b](k,n) + beta * C[b](m,n),  C row-major with leading dimension ldc.
+//   a_kc: A(m,k) = A[m*lda + k] (K contiguous) else A[k*lda + m];  b_kc: B(k,n) = B[n*ldb + k] else B[k*ldb + n].
+//   Two-level batch: batch index z = z1*nb2 + z2, operand offsets z1*s?1 + z2*s?2 (elements).
+struct GemmDesc {
+    int M, N, K;
+    const double *A; long long lda;
+    const double *B; long long ldb;
+    double *C; long long ldc;
+    double alpha, beta;
+    int nb1, nb2;
+    long long sA1, sA2, sB1, sB2, sC1, sC2;
+    bool a_kc, b_kc;
+    // optional split of the C rows: row r lives at (r / c_rpg) * c_gstride + (r % c_rpg) * ldc  (c_rpg = 0: plain r * ldc)
+    int c_rpg; long long c_gstride;
+};
+cudaError_t risp_dgemm(const GemmDesc &d, cudaStream_t st);
+inline GemmDesc gemm_desc(int M, int N, int K, const double *A, long long lda, bool a_kc, const double *B, long long ldb, bool b_kc,
+                          double *C, long long ldc, double alpha = 1.0, double beta = 0.0)
+{
+    GemmDesc d;
+    d.M = M; d.N = N; d.K = K; d.A = A; d.lda = lda; d.B = B; d.ldb = ldb; d.C = C; d.ldc = ldc;
+    d.alpha = alpha; d.beta = beta; d.nb1 = 1; d.nb2 = 1;
+    d.sA1 = d.sA2 = d.sB1 = d.sB2 = d.sC1 = d.sC2 = 0; d.a_kc = a_kc; d.b_kc = b_kc; d.c_rpg = 0; d.c_gstride = 0;
+    return d;
+}

@@ -1,0 +1,352 @@
+// eri_kernels.cu -- kernels built on the integral engine of eri.cuh.
+//
+//   eri_fill      (mu nu|P) blocks written to a dense [P][mu][nu] buffer: K-tensor build (Eq. 20-21),
+//                 the two-centre metrics (P|Q) (Eq. 3, 26) and the parity getter risp_eri3c_shell.
+//   dens_to_e0    Eq. 14 prologue: symmetrised AO density block -> e0 space (adjoint HRR + spherical transform).
+//   j_pass1       R_mQ = sum_z (Q|z) D_z^m        (Eq. 14), integrals generated on the fly.
+//   j_pass2       U_z^m = sum_P (z|P) R~_mP       (Eq. 16), integrals regenerated.
+//   e0_to_U       Eq. 16 epilogue: e0 space -> symmetric AO matrix U^m.
+//
+// Mapping (J passes): a warp generates the integrals of 32 (pair, aux-centre) tasks at once, one task per lane,
+// and parks them in shared memory; then the lanes switch roles to the m trial vectors and contract the parked
+// integrals with D (pass 1) or R~ (pass 2) -- each integral is generated once and used for all m vectors.
+#include "ctx.h"
+
+using namespace risp_eri;
+
+namespace {
+
+constexpr int MS = RISP_MS;  // padded trial-vector stride of the e0-space / aux-space arrays
+
+// ------------------------------------------------------------------------------------------------- eri_fill
+template <int LA, int LB, bool HASP, bool ERF>
+__global__ void __launch_bounds__(128) eri_fill_kernel(const ShellPair *__restrict__ pairs, int npairs, const PrimPair *__restrict__ prims,
+                                                       const AuxCentre *__restrict__ cen, int ncen, OpParams op,
+                                                       const double *__restrict__ boys_tab, double *__restrict__ out,
+                                                       long long stride_q, long long ld, int mirror)
+{
+    constexpr int NE = ne_of(LA, LB), NC = HASP ? 4 : 1;
+    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    int pi = (int)(t / ncen), ci = (int)(t % ncen);
+    if (pi >= npairs) return;
+    const ShellPair sp = pairs[pi];
+    const AuxCentre ax = cen[ci];
+    double e0[NC][NE];
+#pragma unroll
+    for (int c = 0; c < NC; ++c)
+#pragma unroll
+        for (int e = 0; e < NE; ++e) e0[c][e] = 0.0;
+    for (int k = 0; k < sp.npp; ++k) {
+        const PrimPair pp = prims[sp.ppoff + k];
+        eri_e0_prim<LA, LB, HASP, ERF>(pp, sp.Ax, sp.Ay, sp.Az, ax, op, boys_tab, [&](int e, int c, double v) { e0[c][e] += v; });
+    }
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+        int q = c == 0 ? ax.qs : (ax.qp < 0 ? -1 : ax.qp + c - 1);
+        if (q < 0) continue;
+        double blk[2 * LA + 1][2 * LB + 1];
+        e0_to_sph<LA, LB>(e0[c], sp.ABx, sp.ABy, sp.ABz, blk);
+        double *o = out + (long long)q * stride_q;
+#pragma unroll
+        for (int i = 0; i < 2 * LA + 1; ++i)
+#pragma unroll
+            for (int j = 0; j < 2 * LB + 1; ++j) {
+                o[(long long)(sp.aoA + i) * ld + sp.aoB + j] = blk[i][j];
+                if (mirror && sp.shA != sp.shB) o[(long long)(sp.aoB + j) * ld + sp.aoA + i] = blk[i][j];
+            }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------- density -> e0
+template <int LA, int LB>
+__global__ void __launch_bounds__(128) dens_to_e0_kernel(const ShellPair *__restrict__ pairs, int npairs, long long e_off, int m, int nao,
+                                                         const double *__restrict__ D, double *__restrict__ dbar)
+{
+    constexpr int NE = ne_of(LA, LB);
+    int mi = threadIdx.x;
+    int pi = blockIdx.x * blockDim.y + threadIdx.y;
+    if (pi >= npairs) return;
+    const ShellPair sp = pairs[pi];
+    double out[NE];
+    if (mi < m) {
+        const double *Dm = D + (long long)mi * nao * nao;
+        double d[2 * LA + 1][2 * LB + 1];
+#pragma unroll
+        for (int i = 0; i < 2 * LA + 1; ++i)
+#pragma unroll
+            for (int j = 0; j < 2 * LB + 1; ++j) {
+                double v = Dm[(long long)(sp.aoA + i) * nao + sp.aoB + j];
+                if (sp.shA != sp.shB) v += Dm[(long long)(sp.aoB + j) * nao + sp.aoA + i];   // sym(D) on a lower-triangular pair (reading G13)
+                d[i][j] = v;
+            }
+        sph_to_e0_adjoint<LA, LB>(d, sp.ABx, sp.ABy, sp.ABz, out);
+    } else {
+#pragma unroll
+        for (int e = 0; e < NE; ++e) out[e] = 0.0;
+    }
+#pragma unroll
+    for (int e = 0; e < NE; ++e) dbar[(e_off + (long long)pi * NE + e) * MS + mi] = out[e];
+}
+
+template <int LA, int LB>
+__global__ void __launch_bounds__(128) e0_to_U_kernel(const ShellPair *__restrict__ pairs, int npairs, long long e_off, int m, int nao,
+                                                      const double *__restrict__ ubar, double *__restrict__ U)
+{
+    constexpr int NE = ne_of(LA, LB);
+    int mi = threadIdx.x;
+    int pi = blockIdx.x * blockDim.y + threadIdx.y;
+    if (pi >= npairs || mi >= m) return;
+    const ShellPair sp = pairs[pi];
+    double e0[NE];
+#pragma unroll
+    for (int e = 0; e < NE; ++e) e0[e] = ubar[(e_off + (long long)pi * NE + e) * MS + mi];
+    double blk[2 * LA + 1][2 * LB + 1];
+    e0_to_sph<LA, LB>(e0, sp.ABx, sp.ABy, sp.ABz, blk);
+    double *Um = U + (long long)mi * nao * nao;
+#pragma unroll
+    for (int i = 0; i < 2 * LA + 1; ++i)
+#pragma unroll
+        for (int j = 0; j < 2 * LB + 1; ++j) {
+            Um[(long long)(sp.aoA + i) * nao + sp.aoB + j] = blk[i][j];
+            if (sp.shA != sp.shB) Um[(long long)(sp.aoB + j) * nao + sp.aoA + i] = blk[i][j];
+        }
+}
+
+// ------------------------------------------------------------------------------------------------- J passes
+constexpr int JW = 4;   // warps per CTA
+
+template <int LA, int LB>
+__device__ __forceinline__ void park_integrals(double *__restrict__ g, int lane, bool valid, const ShellPair &sp,
+                                               const PrimPair *__restrict__ prims, const AuxCentre &ax, const double *__restrict__ boys_tab)
+{
+    constexpr int NE = ne_of(LA, LB);
+#pragma unroll
+    for (int k = 0; k < NE * 4; ++k) g[k * 32 + lane] = 0.0;
+    if (valid) {
+        OpParams op{1.0, 0.0, 0.0};
+        for (int k = 0; k < sp.npp; ++k) {
+            const PrimPair pp = prims[sp.ppoff + k];
+            eri_e0_prim<LA, LB, true, false>(pp, sp.Ax, sp.Ay, sp.Az, ax, op, boys_tab,
+                                             [&](int e, int c, double v) { g[(e * 4 + c) * 32 + lane] += v; });
+        }
+    }
+}
+
+// pass 2: one pair per warp, 32 aux centres per step.  ubar[(e_off + pair*NE + e)*MS + mi]
+template <int LA, int LB>
+__global__ void __launch_bounds__(32 * JW) j_pass2_kernel(const ShellPair *__restrict__ pairs, int npairs, const PrimPair *__restrict__ prims,
+                                                          const AuxCentre *__restrict__ cen, int ncen, const double *__restrict__ boys_tab,
+                                                          const double *__restrict__ Rt, long long e_off, double *__restrict__ ubar)
+{
+    constexpr int NE = ne_of(LA, LB);
+    extern __shared__ double smem[];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    double *g = smem + (size_t)w * NE * 4 * 32;
+    const int pi = blockIdx.x * JW + w;
+    if (pi >= npairs) return;
+    const ShellPair sp = pairs[pi];
+    double acc[NE];
+#pragma unroll
+    for (int e = 0; e < NE; ++e) acc[e] = 0.0;
+    for (int c0 = 0; c0 < ncen; c0 += 32) {
+        const int ci = c0 + lane;
+        const bool valid = ci < ncen;
+        const AuxCentre ax = cen[valid ? ci : 0];
+        park_integrals<LA, LB>(g, lane, valid, sp, prims, ax, boys_tab);
+        __syncwarp();
+        const int nc = min(32, ncen - c0);
+        for (int s = 0; s < nc; s += 2) {
+            double rt[2][4];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const bool ok = s + h < nc;
+                const int qs = ok ? __ldg(&cen[c0 + s + h].qs) : -1, qp = ok ? __ldg(&cen[c0 + s + h].qp) : -1;
+                rt[h][0] = qs >= 0 ? Rt[(long long)qs * MS + lane] : 0.0;
+#pragma unroll
+                for (int d = 0; d < 3; ++d) rt[h][1 + d] = qp >= 0 ? Rt[(long long)(qp + d) * MS + lane] : 0.0;
+            }
+#pragma unroll
+            for (int e = 0; e < NE; ++e)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const double2 gg = *reinterpret_cast<const double2 *>(&g[(e * 4 + c) * 32 + s]);
+                    acc[e] = fma(gg.x, rt[0][c], fma(gg.y, rt[1][c], acc[e]));
+                }
+        }
+        __syncwarp();
+    }
+#pragma unroll
+    for (int e = 0; e < NE; ++e) ubar[(e_off + (long long)pi * NE + e) * MS + lane] = acc[e];
+}
+
+// pass 1: CTA = (pair chunk, 8 aux centres); warp step = 4 pairs x 8 centres.
+// Rpart[((chunk_global * ncen_pad + centre) * 4 + comp) * MS + mi]
+template <int LA, int LB>
+__global__ void __launch_bounds__(32 * JW) j_pass1_kernel(const ShellPair *__restrict__ pairs, int npairs, int chunk, int chunk_base,
+                                                          const PrimPair *__restrict__ prims, const AuxCentre *__restrict__ cen, int ncen,
+                                                          int ncen_pad, const double *__restrict__ boys_tab, const double *__restrict__ dbar,
+                                                          long long e_off, double *__restrict__ Rpart)
+{
+    constexpr int NE = ne_of(LA, LB);
+    extern __shared__ double smem[];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    double *g = smem + (size_t)w * NE * 4 * 32;
+    const int p_begin = blockIdx.x * chunk, p_end = min(npairs, p_begin + chunk);
+    const int ci = blockIdx.y * 8 + (lane & 7), slot = lane >> 3;
+    const bool cvalid = ci < ncen;
+    const AuxCentre ax = cen[cvalid ? ci : 0];
+    double acc[32];
+#pragma unroll
+    for (int k = 0; k < 32; ++k) acc[k] = 0.0;
+    for (int pg = p_begin + w * 4; pg < p_end; pg += JW * 4) {
+        const int pi = pg + slot;
+        const bool valid = cvalid && pi < p_end;
+        const ShellPair sp = pairs[pi < p_end ? pi : p_begin];
+        park_integrals<LA, LB>(g, lane, valid, sp, prims, ax, boys_tab);
+        __syncwarp();
+        const int ns = min(4, p_end - pg);
+        for (int s = 0; s < ns; ++s) {
+            const double *db = dbar + (e_off + (long long)(pg + s) * NE) * MS + lane;
+#pragma unroll
+            for (int e = 0; e < NE; ++e) {
+                const double d = db[(long long)e * MS];
+#pragma unroll
+                for (int c = 0; c < 4; ++c)
+#pragma unroll
+                    for (int a = 0; a < 8; a += 2) {
+                        const double2 gg = *reinterpret_cast<const double2 *>(&g[(e * 4 + c) * 32 + s * 8 + a]);
+                        acc[a * 4 + c] = fma(gg.x, d, acc[a * 4 + c]);
+                        acc[(a + 1) * 4 + c] = fma(gg.y, d, acc[(a + 1) * 4 + c]);
+                    }
+            }
+        }
+        __syncwarp();
+    }
+    // cross-warp reduction (fixed order -> deterministic), reuse the parking area
+    __syncthreads();
+    double *red = smem;   // [JW][32][32], NE*4*32 >= 32*32 only if NE >= 8, so use a dedicated region after the parking area
+    red = smem + (size_t)JW * NE * 4 * 32;
+#pragma unroll
+    for (int k = 0; k < 32; ++k) red[(w * 32 + k) * 32 + lane] = acc[k];
+    __syncthreads();
+    for (int k = w; k < 32; k += JW) {
+        double s = 0.0;
+#pragma unroll
+        for (int ww = 0; ww < JW; ++ww) s += red[(ww * 32 + k) * 32 + lane];
+        const int a = k >> 2, c = k & 3;
+        const int cc = blockIdx.y * 8 + a;
+        if (cc < ncen) Rpart[(((long long)(chunk_base + blockIdx.x) * ncen_pad + cc) * 4 + c) * MS + lane] = s;
+    }
+}
+
+__global__ void j_reduce_R_kernel(const double *__restrict__ Rpart, int nchunks, const AuxCentre *__restrict__ cen, int ncen, int ncen_pad,
+                                  double *__restrict__ R)
+{
+    const int lane = threadIdx.x, k = blockIdx.x;          // k = centre*4 + comp
+    const int ci = k >> 2, c = k & 3;
+    if (ci >= ncen) return;
+    const int q = c == 0 ? cen[ci].qs : (cen[ci].qp < 0 ? -1 : cen[ci].qp + c - 1);
+    if (q < 0) return;
+    double s = 0.0;
+    for (int ch = 0; ch < nchunks; ++ch) s += Rpart[(((long long)ch * ncen_pad + ci) * 4 + c) * MS + lane];
+    R[(long long)q * MS + lane] = s;
+}
+
+template <class F>
+inline void dispatch_class(int la, int lb, F &&f)
+{
+    if (la == 0) f(std::integral_constant<int, 0>{}, std::integral_constant<int, 0>{});
+    else if (la == 1 && lb == 0) f(std::integral_constant<int, 1>{}, std::integral_constant<int, 0>{});
+    else if (la == 1) f(std::integral_constant<int, 1>{}, std::integral_constant<int, 1>{});
+    else if (lb == 0) f(std::integral_constant<int, 2>{}, std::integral_constant<int, 0>{});
+    else if (lb == 1) f(std::integral_constant<int, 2>{}, std::integral_constant<int, 1>{});
+    else f(std::integral_constant<int, 2>{}, std::integral_constant<int, 2>{});
+}
+
+template <class K>
+cudaError_t ensure_smem(K kernel, size_t bytes)
+{
+    if (bytes <= 48 * 1024) return cudaSuccess;
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+}  // namespace
+
+// ===================================================================================================== host wrappers
+cudaError_t risp_eri_fill(int la, int lb, bool hasp, bool erf_op, const ShellPair *pairs, int npairs, const PrimPair *prims,
+                          const AuxCentre *cen, int ncen, OpParams op, const double *boys_tab, double *out, long long stride_q,
+                          long long ld, int mirror, cudaStream_t st)
+{
+    if (npairs <= 0 || ncen <= 0) return cudaSuccess;
+    long long total = (long long)npairs * ncen;
+    unsigned grid = (unsigned)((total + 127) / 128);
+    dispatch_class(la, lb, [&](auto LA, auto LB) {
+        constexpr int A = decltype(LA)::value, B = decltype(LB)::value;
+        if (hasp) {
+            if (erf_op) eri_fill_kernel<A, B, true, true><<<grid, 128, 0, st>>>(pairs, npairs, prims, cen, ncen, op, boys_tab, out, stride_q, ld, mirror);
+            else eri_fill_kernel<A, B, true, false><<<grid, 128, 0, st>>>(pairs, npairs, prims, cen, ncen, op, boys_tab, out, stride_q, ld, mirror);
+        } else {
+            if (erf_op) eri_fill_kernel<A, B, false, true><<<grid, 128, 0, st>>>(pairs, npairs, prims, cen, ncen, op, boys_tab, out, stride_q, ld, mirror);
+            else eri_fill_kernel<A, B, false, false><<<grid, 128, 0, st>>>(pairs, npairs, prims, cen, ncen, op, boys_tab, out, stride_q, ld, mirror);
+        }
+    });
+    return cudaGetLastError();
+}
+
+cudaError_t risp_dens_to_e0(const PairClass &pc, int m, int nao, const double *D, double *dbar, cudaStream_t st)
+{
+    if (pc.npairs <= 0) return cudaSuccess;
+    dim3 block(32, 4), grid((pc.npairs + 3) / 4);
+    dispatch_class(pc.la, pc.lb, [&](auto LA, auto LB) {
+        dens_to_e0_kernel<decltype(LA)::value, decltype(LB)::value><<<grid, block, 0, st>>>(pc.d_pairs, pc.npairs, pc.e_off, m, nao, D, dbar);
+    });
+    return cudaGetLastError();
+}
+
+cudaError_t risp_e0_to_U(const PairClass &pc, int m, int nao, const double *ubar, double *U, cudaStream_t st)
+{
+    if (pc.npairs <= 0) return cudaSuccess;
+    dim3 block(32, 4), grid((pc.npairs + 3) / 4);
+    dispatch_class(pc.la, pc.lb, [&](auto LA, auto LB) {
+        e0_to_U_kernel<decltype(LA)::value, decltype(LB)::value><<<grid, block, 0, st>>>(pc.d_pairs, pc.npairs, pc.e_off, m, nao, ubar, U);
+    });
+    return cudaGetLastError();
+}
+
+cudaError_t risp_j_pass1(const PairClass &pc, const PrimPair *prims, const AuxCentre *cen, int ncen, int ncen_pad, const double *boys_tab,
+                         const double *dbar, double *Rpart, cudaStream_t st)
+{
+    if (pc.npairs <= 0) return cudaSuccess;
+    cudaError_t err = cudaSuccess;
+    dispatch_class(pc.la, pc.lb, [&](auto LA, auto LB) {
+        constexpr int A = decltype(LA)::value, B = decltype(LB)::value;
+        size_t smem = ((size_t)JW * ne_of(A, B) * 4 * 32 + (size_t)JW * 32 * 32) * sizeof(double);
+        err = ensure_smem(j_pass1_kernel<A, B>, smem);
+        if (err != cudaSuccess) return;
+        dim3 grid(pc.nchunks, (ncen + 7) / 8);
+        j_pass1_kernel<A, B><<<grid, 32 * JW, smem, st>>>(pc.d_pairs, pc.npairs, pc.chunk, pc.chunk_base, prims, cen, ncen, ncen_pad, boys_tab,
+                                                          dbar, pc.e_off, Rpart);
+    });
+    return err != cudaSuccess ? err : cudaGetLastError();
+}
+
+cudaError_t risp_j_reduce_R(const double *Rpart, int nchunks, const AuxCentre *cen, int ncen, int ncen_pad, double *R, cudaStream_t st)
+{
+    j_reduce_R_kernel<<<ncen * 4, 32, 0, st>>>(Rpart, nchunks, cen, ncen, ncen_pad, R);
+    return cudaGetLastError();
+}
+
+cudaError_t risp_j_pass2(const PairClass &pc, const PrimPair *prims, const AuxCentre *cen, int ncen, const double *boys_tab, const double *Rt,
+                         double *ubar, cudaStream_t st)
+{
+    if (pc.npairs <= 0) return cudaSuccess;
+    cudaError_t err = cudaSuccess;
+    dispatch_class(pc.la, pc.lb, [&](auto LA, auto LB) {
+        constexpr int A = decltype(LA)::value, B = decltype(LB)::value;
+        size_t smem = (size_t)JW * ne_of(A, B) * 4 * 32 * sizeof(double);
+        err = ensure_smem(j_pass2_kernel<A, B>, smem);
+        if (err != cudaSuccess) return;
+        j_pass2_kernel<A, B><<<(pc.npairs + JW - 1) / JW, 32 * JW, smem, st>>>(pc.d_pairs, pc.npairs, prims, cen, ncen, boys_tab, Rt, pc.e_off, ubar);
+    });
+    return err != cudaSuccess ? err : cudaGetLastError();
+}

@@ -1,0 +1,523 @@
+// solve.cu -- risp_tda_solve: host-memory-assisted Davidson for the lowest roots of A X = X Omega (Eq. 9).
+//
+// Placement follows PAPER.md:189-201 (Fig. 2): the expansion vectors V and their images W = A V live in PINNED HOST
+// memory; only the newest block, the Ritz vectors and two streaming chunk buffers are device resident.  Every pass
+// over the subspace (projection V^T W_new, Ritz reconstruction X = V y / A X = W y, orthogonalisation of the
+// corrections) streams V / W through the device in chunks on a side stream, double buffered against the compute
+// stream.  When the subspace would outgrow its budget the solver restarts from the current Ritz vectors
+// (reading G17: W <- W y by linearity, no extra sigma-build).
+// The Davidson recipe itself (guess, preconditioner, Gram-Schmidt) is the "standard" one of DESIGN.md reading G16.
+#include "ctx.h"
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+
+namespace {
+
+// ------------------------------------------------------------------------------------------------ device kernels
+__global__ void unit_guess_kernel(double *V, long long dim, const long long *idx, int n)
+{
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j < n) V[(long long)j * dim + idx[j]] = 1.0;
+}
+
+// res[j] = AX[j] - theta[j] X[j]; partial squared norms per block -> part[j][blockIdx.x]
+__global__ void residual_kernel(const double *__restrict__ X, const double *__restrict__ AX, const double *__restrict__ theta,
+                                double *__restrict__ res, long long dim, double *__restrict__ part)
+{
+    const int j = blockIdx.y;
+    const double th = theta[j];
+    double s = 0.0;
+    for (long long x = (long long)blockIdx.x * blockDim.x + threadIdx.x; x < dim; x += (long long)gridDim.x * blockDim.x) {
+        double r = AX[j * dim + x] - th * X[j * dim + x];
+        res[j * dim + x] = r;
+        s += r * r;
+    }
+    __shared__ double sh[256];
+    sh[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) part[j * gridDim.x + blockIdx.x] = sh[0];
+}
+
+// t[j] = res[src[j]] / (theta[src[j]] - (eps_a - eps_i)), |denominator| floored at 1e-8 (sign kept)
+__global__ void precondition_kernel(const double *__restrict__ res, const double *__restrict__ theta, const int *__restrict__ src,
+                                    const double *__restrict__ eps, int nocc, int nvir, double *__restrict__ t, long long dim)
+{
+    const int j = blockIdx.y, sj = src[j];
+    const double th = theta[sj];
+    for (long long x = (long long)blockIdx.x * blockDim.x + threadIdx.x; x < dim; x += (long long)gridDim.x * blockDim.x) {
+        int a = (int)(x % nvir), i = (int)(x / nvir);
+        double den = th - (eps[nocc + a] - eps[i]);
+        if (fabs(den) < 1e-8) den = den < 0 ? -1e-8 : 1e-8;
+        t[j * dim + x] = res[sj * dim + x] / den;
+    }
+}
+
+__global__ void reduce_partials_kernel(const double *__restrict__ part, int nz, int n, double *__restrict__ out)
+{
+    int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    double s = 0.0;
+    for (int z = 0; z < nz; ++z) s += part[(long long)z * n + e];
+    out[e] = s;
+}
+
+// ------------------------------------------------------------------------------------------------ host eigen solver
+// Symmetric eigenproblem of the projected matrix (k <= a few hundred): Householder tridiagonalisation followed by the
+// implicit-shift QL iteration, eigenvectors accumulated.  a: n x n row-major (destroyed); w ascending; z[i*n + j] = i-th
+// component of eigenvector j.
+void sym_eig(std::vector<double> &a, int n, std::vector<double> &w, std::vector<double> &z)
+{
+    z.assign((size_t)n * n, 0.0);
+    for (int i = 0; i < n; ++i) z[(size_t)i * n + i] = 1.0;
+    std::vector<double> v(n), p(n), d(n), e(n, 0.0);
+    for (int k = 0; k + 2 < n; ++k) {
+        int len = n - k - 1;
+        double nrm = 0.0;
+        for (int i = 0; i < len; ++i) { v[i] = a[(size_t)(k + 1 + i) * n + k]; nrm += v[i] * v[i]; }
+        nrm = std::sqrt(nrm);
+        double tail = 0.0;
+        for (int i = 1; i < len; ++i) tail += v[i] * v[i];
+        if (tail == 0.0) continue;                        // already tridiagonal in this column
+        double alpha = v[0] > 0 ? -nrm : nrm;
+        v[0] -= alpha;
+        double vv = 0.0;
+        for (int i = 0; i < len; ++i) vv += v[i] * v[i];
+        double beta = 2.0 / vv;
+        for (int i = 0; i < len; ++i) {                   // p = beta A22 v
+            double s = 0.0;
+            for (int j = 0; j < len; ++j) s += a[(size_t)(k + 1 + i) * n + k + 1 + j] * v[j];
+            p[i] = beta * s;
+        }
+        double K = 0.0;
+        for (int i = 0; i < len; ++i) K += v[i] * p[i];
+        K *= 0.5 * beta;
+        for (int i = 0; i < len; ++i) p[i] -= K * v[i];   // w
+        for (int i = 0; i < len; ++i)
+            for (int j = 0; j < len; ++j) a[(size_t)(k + 1 + i) * n + k + 1 + j] -= v[i] * p[j] + p[i] * v[j];
+        a[(size_t)(k + 1) * n + k] = a[(size_t)k * n + k + 1] = alpha;
+        for (int i = 1; i < len; ++i) a[(size_t)(k + 1 + i) * n + k] = a[(size_t)k * n + k + 1 + i] = 0.0;
+        for (int r = 0; r < n; ++r) {                     // Q <- Q H
+            double s = 0.0;
+            for (int j = 0; j < len; ++j) s += z[(size_t)r * n + k + 1 + j] * v[j];
+            s *= beta;
+            for (int j = 0; j < len; ++j) z[(size_t)r * n + k + 1 + j] -= s * v[j];
+        }
+    }
+    for (int i = 0; i < n; ++i) d[i] = a[(size_t)i * n + i];
+    for (int i = 0; i + 1 < n; ++i) e[i] = a[(size_t)(i + 1) * n + i];
+    // implicit QL with Wilkinson-type shift
+    for (int l = 0; l < n; ++l) {
+        int iter = 0, m;
+        do {
+            for (m = l; m < n - 1; ++m) {
+                double dd = std::fabs(d[m]) + std::fabs(d[m + 1]);
+                if (std::fabs(e[m]) <= 2.3e-16 * dd) break;
+            }
+            if (m != l) {
+                if (++iter > 200) break;
+                double g = (d[l + 1] - d[l]) / (2.0 * e[l]);
+                double r = std::hypot(g, 1.0);
+                g = d[m] - d[l] + e[l] / (g + (g >= 0 ? std::fabs(r) : -std::fabs(r)));
+                double s = 1.0, c = 1.0, pp = 0.0;
+                int i;
+                for (i = m - 1; i >= l; --i) {
+                    double f = s * e[i], b = c * e[i];
+                    e[i + 1] = r = std::hypot(f, g);
+                    if (r == 0.0) { d[i + 1] -= pp; e[m] = 0.0; break; }
+                    s = f / r; c = g / r;
+                    g = d[i + 1] - pp;
+                    r = (d[i] - g) * s + 2.0 * c * b;
+                    pp = s * r;
+                    d[i + 1] = g + pp;
+                    g = c * r - b;
+                    for (int k = 0; k < n; ++k) {
+                        double f2 = z[(size_t)k * n + i + 1];
+                        z[(size_t)k * n + i + 1] = s * z[(size_t)k * n + i] + c * f2;
+                        z[(size_t)k * n + i] = c * z[(size_t)k * n + i] - s * f2;
+                    }
+                }
+                if (r == 0.0 && i >= l) continue;
+                d[l] -= pp; e[l] = g; e[m] = 0.0;
+            }
+        } while (m != l);
+    }
+    // sort ascending
+    std::vector<int> ord(n);
+    for (int i = 0; i < n; ++i) ord[i] = i;
+    std::sort(ord.begin(), ord.end(), [&](int x, int y) { return d[x] < d[y]; });
+    w.resize(n);
+    std::vector<double> zs((size_t)n * n);
+    for (int j = 0; j < n; ++j) {
+        w[j] = d[ord[j]];
+        for (int i = 0; i < n; ++i) zs[(size_t)i * n + j] = z[(size_t)i * n + ord[j]];
+    }
+    z.swap(zs);
+}
+
+struct Solver {
+    risp_ctx *ctx;
+    long long dim;
+    int cap = 0, k = 0, CH = 16;
+    double *hV = nullptr, *hW = nullptr;           // pinned host [cap][dim]
+    double *dB = nullptr, *dWB = nullptr;          // newest block and its image [32][dim]
+    double *dX = nullptr, *dAX = nullptr, *dRes = nullptr, *dT = nullptr;   // [nroots][dim]
+    double *dChunk[2] = {nullptr, nullptr};        // streaming buffers [CH][dim]
+    double *dCoef = nullptr, *dPart = nullptr, *dSmall = nullptr, *dTheta = nullptr;
+    int *dSrc = nullptr;
+    cudaEvent_t evUp[2], evFree[2], evD2H;
+    double bytes_h2d = 0, bytes_d2h = 0;
+    cudaStream_t st = 0;                           // compute stream (default)
+};
+
+int gram(Solver &S, const double *A, int na, const double *B, int nb, std::vector<double> &out)
+{
+    // out[na][nb] = sum_x A[i][x] B[j][x]: split-K batched DMMA GEMM + fixed-order reduction
+    risp_ctx *ctx = S.ctx;
+    const long long slice = 16384;
+    int nfull = (int)(S.dim / slice);
+    long long tail = S.dim - (long long)nfull * slice;
+    int nz = nfull + (tail ? 1 : 0);
+    if (nfull) {
+        GemmDesc d = gemm_desc(na, nb, (int)slice, A, S.dim, true, B, S.dim, true, S.dPart, nb);
+        d.nb1 = nfull; d.sA1 = slice; d.sB1 = slice; d.sC1 = (long long)na * nb;
+        RISP_CUDA_TRY(risp_dgemm(d, S.st));
+    }
+    if (tail) {
+        GemmDesc d = gemm_desc(na, nb, (int)tail, A + (long long)nfull * slice, S.dim, true, B + (long long)nfull * slice, S.dim, true,
+                               S.dPart + (long long)nfull * na * nb, nb);
+        RISP_CUDA_TRY(risp_dgemm(d, S.st));
+    }
+    reduce_partials_kernel<<<(na * nb + 127) / 128, 128, 0, S.st>>>(S.dPart, nz, na * nb, S.dSmall);
+    out.resize((size_t)na * nb);
+    RISP_CUDA_TRY(cudaMemcpyAsync(out.data(), S.dSmall, (size_t)na * nb * 8, cudaMemcpyDeviceToHost, S.st));
+    RISP_CUDA_TRY(cudaStreamSynchronize(S.st));
+    return RISP_OK;
+}
+
+// C[nc][dim] = alpha * coef[nc][na] * A[na][dim] + beta * C
+int lincomb(Solver &S, const std::vector<double> &coef, int nc, int na, const double *A, double *C, double alpha, double beta)
+{
+    risp_ctx *ctx = S.ctx;
+    RISP_CUDA_TRY(cudaMemcpyAsync(S.dCoef, coef.data(), (size_t)nc * na * 8, cudaMemcpyHostToDevice, S.st));
+    GemmDesc d = gemm_desc(nc, (int)std::min<long long>(S.dim, 1 << 30), na, S.dCoef, na, true, A, S.dim, false, C, S.dim, alpha, beta);
+    RISP_CUDA_TRY(risp_dgemm(d, S.st));
+    RISP_CUDA_TRY(cudaStreamSynchronize(S.st));   // coef is a host temporary
+    return RISP_OK;
+}
+
+// stream host vectors [0, n) of `h` through the device in chunks; fn(dev_ptr, first, count) runs on the compute stream
+template <class F>
+int stream_pass(Solver &S, const double *h, int n, F &&fn)
+{
+    risp_ctx *ctx = S.ctx;
+    int nchunk = (n + S.CH - 1) / S.CH;
+    auto upload = [&](int c) -> int {
+        int b = c & 1, first = c * S.CH, cnt = std::min(S.CH, n - first);
+        RISP_CUDA_TRY(cudaStreamWaitEvent(ctx->side, S.evFree[b], 0));
+        RISP_CUDA_TRY(cudaMemcpyAsync(S.dChunk[b], h + (long long)first * S.dim, (size_t)cnt * S.dim * 8, cudaMemcpyHostToDevice, ctx->side));
+        RISP_CUDA_TRY(cudaEventRecord(S.evUp[b], ctx->side));
+        S.bytes_h2d += (double)cnt * S.dim * 8;
+        return RISP_OK;
+    };
+    int rc;
+    if (nchunk > 0 && (rc = upload(0))) return rc;
+    for (int c = 0; c < nchunk; ++c) {
+        if (c + 1 < nchunk && (rc = upload(c + 1))) return rc;
+        int b = c & 1, first = c * S.CH, cnt = std::min(S.CH, n - first);
+        RISP_CUDA_TRY(cudaStreamWaitEvent(S.st, S.evUp[b], 0));
+        if ((rc = fn(S.dChunk[b], first, cnt))) return rc;
+        RISP_CUDA_TRY(cudaEventRecord(S.evFree[b], S.st));
+    }
+    return RISP_OK;
+}
+
+}  // namespace
+
+extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_options *opt_in, double *omega_out, double *X_out,
+                              risp_solve_info *info)
+{
+    if (!ctx) return RISP_EINVAL;
+    const long long dim = (long long)ctx->nocc * ctx->nvir;
+    if (nroots <= 0 || nroots > RISP_MAX_ROOTS || nroots > dim || !omega_out) { risp_set_error(ctx, "risp_tda_solve: bad nroots or NULL output"); return RISP_EINVAL; }
+    RISP_CUDA_TRY(cudaSetDevice(ctx->device));
+    risp_solve_options opt;
+    std::memset(&opt, 0, sizeof(opt));
+    if (opt_in) opt = *opt_in;
+    const double tol = opt.tol > 0 ? opt.tol : 1e-5;
+    const int max_iter = opt.max_iter > 0 ? opt.max_iter : 100;
+    int n_guess = opt.n_guess > 0 ? opt.n_guess : 2 * nroots;
+    n_guess = (int)std::min<long long>(std::max(n_guess, nroots), dim);
+    int max_sub = opt.max_sub > 0 ? opt.max_sub : 20 * nroots;
+    auto t_start = std::chrono::steady_clock::now();
+    double sec_mv = 0.0;
+
+    Solver S;
+    S.ctx = ctx; S.dim = dim;
+    // subspace capacity: user limit, and the pinned-host budget (V and W)
+    long long by_budget = (long long)(ctx->host_budget / (2.0 * dim * 8.0));
+    S.cap = (int)std::min<long long>(max_sub, by_budget);
+    S.cap = std::max(S.cap, std::max(n_guess, 2 * nroots));
+    const int slots = S.cap + nroots;              // room to append one more block before the restart decision
+    RISP_CUDA_TRY(cudaHostAlloc((void **)&S.hV, (size_t)slots * dim * 8, cudaHostAllocDefault));
+    RISP_CUDA_TRY(cudaHostAlloc((void **)&S.hW, (size_t)slots * dim * 8, cudaHostAllocDefault));
+    const int nbmax = std::max(n_guess, nroots);
+    auto DA = [&](double *&p, size_t n) -> int { RISP_CUDA_TRY(cudaMalloc((void **)&p, n * 8)); return RISP_OK; };
+    int rc;
+    if ((rc = DA(S.dB, (size_t)nbmax * dim)) || (rc = DA(S.dWB, (size_t)nbmax * dim)) || (rc = DA(S.dX, (size_t)nroots * dim)) ||
+        (rc = DA(S.dAX, (size_t)nroots * dim)) || (rc = DA(S.dRes, (size_t)nroots * dim)) || (rc = DA(S.dT, (size_t)nroots * dim)) ||
+        (rc = DA(S.dChunk[0], (size_t)S.CH * dim)) || (rc = DA(S.dChunk[1], (size_t)S.CH * dim)))
+        return rc;
+    const int small = std::max(slots, 64);
+    const int nzmax = (int)(dim / 16384) + 2;
+    if ((rc = DA(S.dCoef, (size_t)small * small)) || (rc = DA(S.dPart, std::max((size_t)nzmax * 64 * 64, (size_t)RISP_MAX_ROOTS * 256))) || (rc = DA(S.dSmall, (size_t)64 * 64 + 4096)) ||
+        (rc = DA(S.dTheta, (size_t)RISP_MAX_ROOTS)))
+        return rc;
+    RISP_CUDA_TRY(cudaMalloc((void **)&S.dSrc, RISP_MAX_ROOTS * sizeof(int)));
+    for (int b = 0; b < 2; ++b) { RISP_CUDA_TRY(cudaEventCreateWithFlags(&S.evUp[b], cudaEventDisableTiming)); RISP_CUDA_TRY(cudaEventCreateWithFlags(&S.evFree[b], cudaEventDisableTiming)); }
+    RISP_CUDA_TRY(cudaEventCreateWithFlags(&S.evD2H, cudaEventDisableTiming));
+
+    auto cleanup = [&]() {
+        cudaDeviceSynchronize();
+        cudaFreeHost(S.hV); cudaFreeHost(S.hW);
+        double *bufs[] = {S.dB, S.dWB, S.dX, S.dAX, S.dRes, S.dT, S.dChunk[0], S.dChunk[1], S.dCoef, S.dPart, S.dSmall, S.dTheta};
+        for (double *b : bufs) if (b) cudaFree(b);
+        if (S.dSrc) cudaFree(S.dSrc);
+        for (int b = 0; b < 2; ++b) { cudaEventDestroy(S.evUp[b]); cudaEventDestroy(S.evFree[b]); }
+        cudaEventDestroy(S.evD2H);
+    };
+#define SOLVE_TRY(x) do { int rc_ = (x); if (rc_) { cleanup(); return rc_; } } while (0)
+
+    // ---------------- initial guess: unit vectors on the smallest eps_a - eps_i
+    int nb = n_guess;
+    {
+        std::vector<std::pair<double, long long>> dl;
+        // the n_guess smallest differences: occupied from the top, virtual from the bottom
+        int no_top = (int)std::min<long long>(ctx->nocc, n_guess), nv_bot = (int)std::min<long long>(ctx->nvir, n_guess);
+        for (int i = ctx->nocc - no_top; i < ctx->nocc; ++i)
+            for (int a = 0; a < nv_bot; ++a) dl.push_back({ctx->h_eps[ctx->nocc + a] - ctx->h_eps[i], (long long)i * ctx->nvir + a});
+        std::stable_sort(dl.begin(), dl.end(), [](auto &x, auto &y) { return x.first < y.first || (x.first == y.first && x.second < y.second); });
+        std::vector<long long> idx(nb);
+        for (int j = 0; j < nb; ++j) idx[j] = dl[j].second;
+        long long *d_idx = nullptr;
+        RISP_CUDA_TRY(cudaMalloc((void **)&d_idx, nb * sizeof(long long)));
+        RISP_CUDA_TRY(cudaMemcpy(d_idx, idx.data(), nb * sizeof(long long), cudaMemcpyHostToDevice));
+        RISP_CUDA_TRY(cudaMemsetAsync(S.dB, 0, (size_t)nb * dim * 8, S.st));
+        unit_guess_kernel<<<(nb + 63) / 64, 64, 0, S.st>>>(S.dB, dim, d_idx, nb);
+        RISP_CUDA_TRY(cudaStreamSynchronize(S.st));
+        cudaFree(d_idx);
+    }
+
+    std::vector<double> G;          // projected matrix, k x k, row-major with leading dimension ldg
+    const int ldg = slots;
+    G.assign((size_t)ldg * ldg, 0.0);
+    std::vector<double> theta(nroots, 0.0), rn(nroots, 0.0), yv;
+    int iterations = 0, restarts = 0, n_sigma = 0, sub_max = 0;
+    bool converged = false;
+    S.k = 0;
+
+    for (int it = 1; it <= max_iter; ++it) {
+        iterations = it;
+        // ---- W_B = A B
+        {
+            auto t0 = std::chrono::steady_clock::now();
+            for (int b0 = 0; b0 < nb; b0 += RISP_MS) {
+                int mb = std::min(RISP_MS, nb - b0);
+                SOLVE_TRY(risp_ensure_workspace(ctx, mb));
+                SOLVE_TRY(risp_matvec_impl(ctx, mb, S.dB + (long long)b0 * dim, S.dWB + (long long)b0 * dim, S.st));
+            }
+            RISP_CUDA_TRY(cudaStreamSynchronize(S.st));
+            sec_mv += std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+            n_sigma += nb;
+        }
+        // ---- projected matrix: G[0:k][k:k+nb] = V_old^T W_B (stream V_old), G[k:,k:] = B^T W_B
+        {
+            const int k = S.k;
+            std::vector<double> blk;
+            SOLVE_TRY(stream_pass(S, S.hV, k, [&](const double *Vc, int first, int cnt) -> int {
+                int r = gram(S, Vc, cnt, S.dWB, nb, blk);
+                if (r) return r;
+                for (int i = 0; i < cnt; ++i)
+                    for (int j = 0; j < nb; ++j) G[(size_t)(first + i) * ldg + k + j] = G[(size_t)(k + j) * ldg + first + i] = blk[(size_t)i * nb + j];
+                return RISP_OK;
+            }));
+            SOLVE_TRY(gram(S, S.dB, nb, S.dWB, nb, blk));
+            for (int i = 0; i < nb; ++i)
+                for (int j = 0; j < nb; ++j) G[(size_t)(k + i) * ldg + k + j] = 0.5 * (blk[(size_t)i * nb + j] + blk[(size_t)j * nb + i]);
+            // append B, W_B to the pinned host subspace (side stream)
+            RISP_CUDA_TRY(cudaMemcpyAsync(S.hV + (long long)k * dim, S.dB, (size_t)nb * dim * 8, cudaMemcpyDeviceToHost, ctx->side));
+            RISP_CUDA_TRY(cudaMemcpyAsync(S.hW + (long long)k * dim, S.dWB, (size_t)nb * dim * 8, cudaMemcpyDeviceToHost, ctx->side));
+            RISP_CUDA_TRY(cudaEventRecord(S.evD2H, ctx->side));
+            S.bytes_d2h += 2.0 * nb * dim * 8;
+            S.k += nb;
+            sub_max = std::max(sub_max, S.k);
+        }
+        // ---- Ritz pairs of the projected matrix
+        const int k = S.k;
+        {
+            std::vector<double> a((size_t)k * k), w;
+            for (int i = 0; i < k; ++i)
+                for (int j = 0; j < k; ++j) a[(size_t)i * k + j] = G[(size_t)i * ldg + j];
+            sym_eig(a, k, w, yv);
+            for (int j = 0; j < nroots; ++j) theta[j] = w[j];
+        }
+        // ---- X = V y, AX = W y (stream V and W; needs the appended block on the host)
+        RISP_CUDA_TRY(cudaEventSynchronize(S.evD2H));
+        for (int pass = 0; pass < 2; ++pass) {
+            double *dst = pass == 0 ? S.dX : S.dAX;
+            bool first_chunk = true;
+            SOLVE_TRY(stream_pass(S, pass == 0 ? S.hV : S.hW, k, [&](const double *Vc, int first, int cnt) -> int {
+                std::vector<double> coef((size_t)nroots * cnt);
+                for (int j = 0; j < nroots; ++j)
+                    for (int i = 0; i < cnt; ++i) coef[(size_t)j * cnt + i] = yv[(size_t)(first + i) * k + j];
+                int r = lincomb(S, coef, nroots, cnt, Vc, dst, 1.0, first_chunk ? 0.0 : 1.0);
+                first_chunk = false;
+                return r;
+            }));
+        }
+        // ---- residuals
+        {
+            RISP_CUDA_TRY(cudaMemcpyAsync(S.dTheta, theta.data(), nroots * 8, cudaMemcpyHostToDevice, S.st));
+            const int gx = 256;
+            residual_kernel<<<dim3(gx, nroots), 256, 0, S.st>>>(S.dX, S.dAX, S.dTheta, S.dRes, dim, S.dPart);
+            std::vector<double> part((size_t)nroots * gx);
+            RISP_CUDA_TRY(cudaMemcpyAsync(part.data(), S.dPart, part.size() * 8, cudaMemcpyDeviceToHost, S.st));
+            RISP_CUDA_TRY(cudaStreamSynchronize(S.st));
+            for (int j = 0; j < nroots; ++j) {
+                double s = 0.0;
+                for (int b = 0; b < gx; ++b) s += part[(size_t)j * gx + b];
+                rn[j] = std::sqrt(s);
+            }
+        }
+        std::vector<int> src;
+        for (int j = 0; j < nroots; ++j) if (!(rn[j] < tol)) src.push_back(j);
+        if (src.empty()) { converged = true; break; }
+        if (it == max_iter) break;
+        // ---- restart from the Ritz vectors when the next block would not fit
+        if (k + (int)src.size() > S.cap) {
+            RISP_CUDA_TRY(cudaMemcpyAsync(S.hV, S.dX, (size_t)nroots * dim * 8, cudaMemcpyDeviceToHost, ctx->side));
+            RISP_CUDA_TRY(cudaMemcpyAsync(S.hW, S.dAX, (size_t)nroots * dim * 8, cudaMemcpyDeviceToHost, ctx->side));
+            RISP_CUDA_TRY(cudaEventRecord(S.evD2H, ctx->side));
+            RISP_CUDA_TRY(cudaEventSynchronize(S.evD2H));
+            S.bytes_d2h += 2.0 * nroots * dim * 8;
+            std::fill(G.begin(), G.end(), 0.0);
+            for (int j = 0; j < nroots; ++j) G[(size_t)j * ldg + j] = theta[j];
+            S.k = nroots;
+            ++restarts;
+        }
+        // ---- corrections t_j = r_j / (theta_j - Delta), normalised
+        nb = (int)src.size();
+        {
+            RISP_CUDA_TRY(cudaMemcpyAsync(S.dSrc, src.data(), nb * sizeof(int), cudaMemcpyHostToDevice, S.st));
+            precondition_kernel<<<dim3(256, nb), 256, 0, S.st>>>(S.dRes, S.dTheta, S.dSrc, ctx->d_eps, ctx->nocc, ctx->nvir, S.dT, dim);
+            RISP_CUDA_TRY(cudaStreamSynchronize(S.st));
+        }
+        auto normalise_rows = [&](double *T, int n, std::vector<double> &norms) -> int {
+            std::vector<double> g;
+            int r = gram(S, T, n, T, n, g);
+            if (r) return r;
+            norms.resize(n);
+            std::vector<double> coef((size_t)n * n, 0.0);
+            for (int j = 0; j < n; ++j) { norms[j] = std::sqrt(g[(size_t)j * n + j]); coef[(size_t)j * n + j] = norms[j] > 0 ? 1.0 / norms[j] : 0.0; }
+            // scale in place through a temporary: B = coef * T, then copy back
+            r = lincomb(S, coef, n, n, T, S.dB, 1.0, 0.0);
+            if (r) return r;
+            RISP_CUDA_TRY(cudaMemcpyAsync(T, S.dB, (size_t)n * dim * 8, cudaMemcpyDeviceToDevice, S.st));
+            return RISP_OK;
+        };
+        std::vector<double> norms;
+        SOLVE_TRY(normalise_rows(S.dT, nb, norms));
+        // ---- orthogonalise against V: per streamed chunk, two projections (block Gram-Schmidt with re-orthogonalisation)
+        SOLVE_TRY(stream_pass(S, S.hV, S.k, [&](const double *Vc, int first, int cnt) -> int {
+            for (int rep = 0; rep < 2; ++rep) {
+                std::vector<double> c;
+                int r = gram(S, S.dT, nb, Vc, cnt, c);       // c[j][i] = t_j . v_i
+                if (r) return r;
+                r = lincomb(S, c, nb, cnt, Vc, S.dT, -1.0, 1.0);
+                if (r) return r;
+            }
+            return RISP_OK;
+        }));
+        // ---- orthonormalise the corrections among themselves: Cholesky of their Gram matrix, twice; drop dependent ones
+        {
+            std::vector<int> keep(nb);
+            for (int j = 0; j < nb; ++j) keep[j] = j;
+            for (int rep = 0; rep < 2; ++rep) {
+                std::vector<double> g;
+                SOLVE_TRY(gram(S, S.dT, nb, S.dT, nb, g));
+                // after projection the rows have norm <= 1; a row whose remaining norm is tiny is (numerically) inside span(V)
+                std::vector<double> L((size_t)nb * nb, 0.0);
+                std::vector<char> ok(nb, 1);
+                for (int j = 0; j < nb; ++j) {
+                    for (int i = j; i < nb; ++i) {
+                        double s = g[(size_t)i * nb + j];
+                        for (int c = 0; c < j; ++c) s -= L[(size_t)i * nb + c] * L[(size_t)j * nb + c];
+                        if (i == j) {
+                            if (!(s > (rep == 0 ? 1e-16 : 1e-4))) { ok[j] = 0; L[(size_t)j * nb + j] = 1.0; break; }
+                            L[(size_t)j * nb + j] = std::sqrt(s);
+                        } else L[(size_t)i * nb + j] = ok[j] ? s / L[(size_t)j * nb + j] : 0.0;
+                    }
+                    if (!ok[j]) for (int i = 0; i < nb; ++i) if (i != j) L[(size_t)i * nb + j] = 0.0;
+                }
+                // Linv (lower), rows of dropped vectors zeroed
+                std::vector<double> Li((size_t)nb * nb, 0.0);
+                for (int c = 0; c < nb; ++c) {
+                    Li[(size_t)c * nb + c] = 1.0 / L[(size_t)c * nb + c];
+                    for (int i = c + 1; i < nb; ++i) {
+                        double s = 0.0;
+                        for (int q = c; q < i; ++q) s += L[(size_t)i * nb + q] * Li[(size_t)q * nb + c];
+                        Li[(size_t)i * nb + c] = -s / L[(size_t)i * nb + i];
+                    }
+                }
+                std::vector<int> newkeep;
+                std::vector<double> coef;
+                int nk = 0;
+                for (int j = 0; j < nb; ++j) if (ok[j]) ++nk;
+                coef.assign((size_t)nk * nb, 0.0);
+                int r = 0;
+                for (int j = 0; j < nb; ++j) {
+                    if (!ok[j]) continue;
+                    for (int c = 0; c < nb; ++c) coef[(size_t)r * nb + c] = ok[c] ? Li[(size_t)j * nb + c] : 0.0;
+                    newkeep.push_back(keep[j]);
+                    ++r;
+                }
+                if (nk == 0) { nb = 0; break; }
+                SOLVE_TRY(lincomb(S, coef, nk, nb, S.dT, S.dB, 1.0, 0.0));
+                RISP_CUDA_TRY(cudaMemcpyAsync(S.dT, S.dB, (size_t)nk * dim * 8, cudaMemcpyDeviceToDevice, S.st));
+                RISP_CUDA_TRY(cudaStreamSynchronize(S.st));
+                nb = nk; keep = newkeep;
+            }
+        }
+        if (nb == 0) break;     // nothing new to add: stagnated
+        RISP_CUDA_TRY(cudaMemcpyAsync(S.dB, S.dT, (size_t)nb * dim * 8, cudaMemcpyDeviceToDevice, S.st));
+        RISP_CUDA_TRY(cudaStreamSynchronize(S.st));
+    }
+    for (int j = 0; j < nroots; ++j) omega_out[j] = theta[j];
+    if (X_out) RISP_CUDA_TRY(cudaMemcpy(X_out, S.dX, (size_t)nroots * dim * 8, cudaMemcpyDeviceToDevice));
+    if (info) {
+        std::memset(info, 0, sizeof(*info));
+        info->iterations = iterations; info->restarts = restarts; info->n_sigma = n_sigma; info->converged = converged ? 1 : 0;
+        for (int j = 0; j < nroots; ++j) info->resid[j] = rn[j];
+        info->sec_total = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
+        info->sec_matvec = sec_mv; info->sec_subspace = info->sec_total - sec_mv;
+        info->bytes_h2d = S.bytes_h2d; info->bytes_d2h = S.bytes_d2h; info->subspace_max = sub_max;
+    }
+    cleanup();
+    if (!converged) { risp_set_error(ctx, "risp_tda_solve: not converged within max_iter"); return RISP_ENOTCONV; }
+    return RISP_OK;
+}
+
+// Debug export: the host eigen solver of the projected matrix (tests/test_host_logic.py pins it against LAPACK).
+extern "C" int risp_debug_sym_eig(int n, const double *a_in, double *w_out, double *z_out)
+{
+    if (n <= 0 || !a_in || !w_out || !z_out) return RISP_EINVAL;
+    std::vector<double> a(a_in, a_in + (size_t)n * n), w, z;
+    sym_eig(a, n, w, z);
+    std::memcpy(w_out, w.data(), (size_t)n * 8);
+    std::memcpy(z_out, z.data(), (size_t)n * n * 8);
+    return RISP_OK;
+}

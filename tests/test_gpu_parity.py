@@ -1,0 +1,276 @@
+"""GPU parity: the CUDA path (through the C ABI, paper_2603_29257_b200.binding) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json's: |d(mu nu|P)| <= 1e-12 absolute,
+||sigma_gpu - sigma_ref||_F / ||sigma_ref||_F <= 1e-10 (also per term for J and K), roots within 1e-6 eV."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+HARTREE_EV = 27.211386245988
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    return torch
+
+
+def _rel(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+# ------------------------------------------------------------------------------------------------ GEMM
+@pytest.mark.parametrize("a_kc,b_kc", [(1, 1), (1, 0), (0, 1), (0, 0)])
+@pytest.mark.parametrize("shape", [(129, 67, 33), (300, 257, 129), (5, 1000, 3), (128, 128, 16), (1, 1, 1)])
+def test_dgemm_against_torch(torch_cuda, a_kc, b_kc, shape):
+    torch = torch_cuda
+    from paper_2603_29257_b200 import load_library
+    lib = load_library()
+    M, N, K = shape
+    g = torch.Generator(device="cuda").manual_seed(M * 7 + N * 3 + K)
+    A = torch.randn((M, K) if a_kc else (K, M), dtype=torch.float64, device="cuda", generator=g)
+    B = torch.randn((N, K) if b_kc else (K, N), dtype=torch.float64, device="cuda", generator=g)
+    Cm = torch.randn((M, N), dtype=torch.float64, device="cuda", generator=g)
+    ref = 0.7 * (A if a_kc else A.T) @ (B.T if b_kc else B) - 0.3 * Cm
+    out = Cm.clone()
+    rc = lib.risp_debug_dgemm(M, N, K, A.data_ptr(), A.shape[1], a_kc, B.data_ptr(), B.shape[1], b_kc, out.data_ptr(), N, 0.7, -0.3,
+                              1, 0, 0, 0, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert rc == 0
+    assert float((out - ref).abs().max()) <= 1e-12 * max(1.0, K ** 0.5) * float(ref.abs().max() + 1)
+
+
+def test_dgemm_batched(torch_cuda):
+    torch = torch_cuda
+    from paper_2603_29257_b200 import load_library
+    lib = load_library()
+    nb, M, N, K = 5, 70, 90, 50
+    A = torch.randn((nb, M, K), dtype=torch.float64, device="cuda")
+    B = torch.randn((nb, K, N), dtype=torch.float64, device="cuda")
+    out = torch.zeros((nb, M, N), dtype=torch.float64, device="cuda")
+    rc = lib.risp_debug_dgemm(M, N, K, A.data_ptr(), K, 1, B.data_ptr(), N, 0, out.data_ptr(), N, 1.0, 0.0, nb, M * K, K * N, M * N,
+                              torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert rc == 0
+    assert float((out - A @ B).abs().max()) < 1e-11
+
+
+# ------------------------------------------------------------------------------------------------ integrals
+@pytest.fixture(scope="module")
+def ctx1(torch_cuda, sys1):
+    from paper_2603_29257_b200 import setup
+    c = setup(sys1)
+    yield c
+    c.close()
+
+
+@pytest.fixture(scope="module")
+def ctx_rsh(torch_cuda, sys_small_rsh):
+    from paper_2603_29257_b200 import setup
+    c = setup(sys_small_rsh)
+    yield c
+    c.close()
+
+
+def _shell_offsets(o):
+    return np.concatenate([[0], np.cumsum(2 * o.shl_l + 1)]), np.concatenate([[0], np.cumsum(2 * o.aux_l + 1)])
+
+
+@pytest.mark.parametrize("which", ["tiny", "rsh"])
+def test_eri3c_every_class_both_operators(which, ctx1, oracle1, ctx_rsh, oracle_small_rsh):
+    """|d(mu nu|P)| <= 1e-12 for shell triples covering all 6 pair classes x (s, p) aux, Coulomb and K operator."""
+    ctx, o = (ctx1, oracle1) if which == "tiny" else (ctx_rsh, oracle_small_rsh)
+    soff, aoff = _shell_offsets(o)
+    rng = np.random.default_rng(17)
+    by_l = {l: np.nonzero(o.shl_l == l)[0] for l in (0, 1, 2)}
+    worst = 0.0
+    for op, (ca, cb, w) in ((0, (1.0, 0.0, 0.0)), (1, (o.alpha, o.beta, o.omega))):
+        I3 = o.int3c(o.selJ, ca, cb, w)
+        for la in (0, 1, 2):
+            for lb in (0, 1, 2):
+                for _ in range(6):
+                    si, sj = int(rng.choice(by_l[la])), int(rng.choice(by_l[lb]))
+                    for ak in rng.choice(len(o.aux_l), size=4, replace=False):
+                        ak = int(ak)
+                        got = ctx.eri3c_shell(si, sj, ak, op)
+                        ref = I3[aoff[ak]:aoff[ak + 1], soff[si]:soff[si + 1], soff[sj]:soff[sj + 1]].transpose(1, 2, 0)
+                        worst = max(worst, float(np.abs(got - ref).max()))
+    assert worst <= 1e-12, worst
+
+
+def test_eri3c_same_shell_and_same_centre(ctx1, oracle1):
+    o = oracle1
+    soff, aoff = _shell_offsets(o)
+    I3 = o.int3c(o.selJ)
+    for si in range(0, 12):                      # shells of the first two carbons: includes (shell|shell) and same-atom pairs
+        for sj in (si, 0, 5):
+            for ak in (0, 1):
+                got = ctx1.eri3c_shell(si, sj, ak, 0)
+                ref = I3[aoff[ak]:aoff[ak + 1], soff[si]:soff[si + 1], soff[sj]:soff[sj + 1]].transpose(1, 2, 0)
+                assert np.abs(got - ref).max() <= 1e-12
+
+
+def test_metrics(ctx1, oracle1, ctx_rsh, oracle_small_rsh):
+    for ctx, o in ((ctx1, oracle1), (ctx_rsh, oracle_small_rsh)):
+        assert np.abs(ctx.stage("METRIC_J") - o.MJ).max() <= 1e-12
+        assert np.abs(ctx.stage("METRIC_K") - o.MK).max() <= 1e-12
+
+
+# ------------------------------------------------------------------------------------------------ sigma, per stage
+@pytest.mark.parametrize("which", ["tiny", "rsh"])
+def test_sigma_and_stages(which, torch_cuda, sys1, ctx1, oracle1, sys_small_rsh, ctx_rsh, oracle_small_rsh):
+    torch = torch_cuda
+    from workloads import trial_vectors
+    s, ctx, o = (sys1, ctx1, oracle1) if which == "tiny" else (sys_small_rsh, ctx_rsh, oracle_small_rsh)
+    m = 5
+    X = trial_vectors(s, m)
+    sig_ref, dg, J_ref, K_ref = o.sigma(X, parts=True)
+    Xd = torch.from_numpy(X).cuda()
+    sig = ctx.matvec(Xd).cpu().numpy()
+    d = ctx.dims()
+    assert (d["noccK"], d["nvirK"]) == (len(o.occK), len(o.virK))
+    assert d["occK_first"] == (o.occK[0] if len(o.occK) else 0)
+    # stages of the AO-direct J path against the oracle's literal Eq. 11-17
+    J_ao = o.coulomb_ao_direct(X)
+    R_ref = np.array([st[1] for st in o.ao_stages]).T
+    Rt_ref = np.array([st[2] for st in o.ao_stages]).T
+    assert _rel(ctx.stage("R", m), R_ref) <= 1e-11
+    assert _rel(ctx.stage("RTILDE", m), Rt_ref) <= 1e-9        # conditioning of (P|Q): compared again through J below
+    U = ctx.stage("U", m, sel=[2])
+    assert _rel(U, o.ao_stages[2][3]) <= 1e-10
+    assert _rel(ctx.stage("J", m), J_ref) <= 1e-10
+    assert _rel(ctx.stage("K", m), K_ref) <= 1e-10
+    assert _rel(sig, sig_ref) <= 1e-10
+    assert _rel(J_ao, J_ref) <= 1e-10
+
+
+def test_K_tensors(ctx_rsh, oracle_small_rsh):
+    o = oracle_small_rsh
+    sel = [0, len(o.selK) // 2, len(o.selK) - 1]
+    Tab = ctx_rsh.stage("TAB", sel=sel)
+    assert _rel(Tab, o.Bab[sel]) <= 1e-12                                   # Eq. 21 (reading G3): T_ab^P = (ab|P)
+    Tij_ref = np.einsum('qij,qp->pij', o.Bij, np.linalg.inv(o.MK))[sel]     # Eq. 20
+    assert _rel(ctx_rsh.stage("TIJ", sel=sel), Tij_ref) <= 1e-10
+
+
+def test_sigma_structured_vectors(torch_cuda, ctx_rsh, oracle_small_rsh):
+    """unit vectors e_jb inside / outside the window, and a vector supported on the window only."""
+    torch = torch_cuda
+    o = oracle_small_rsh
+    X = np.zeros((4, o.nocc, o.nvir))
+    X[0, o.occK[0], o.virK[0]] = 1.0
+    X[1, 0, o.nvir - 1] = 1.0                                   # outside the window (core-like occupied, high virtual)
+    X[2][np.ix_(o.occK, o.virK)] = np.random.default_rng(3).normal(size=(len(o.occK), len(o.virK)))
+    X[3, o.nocc - 1, 0] = 1.0                                   # HOMO -> LUMO
+    ref = o.sigma(X)
+    got = ctx_rsh.matvec(torch.from_numpy(X).cuda()).cpu().numpy()
+    for k in range(4):
+        assert _rel(got[k], ref[k]) <= 1e-10
+
+
+def test_matvec_host_equals_device(torch_cuda, sys1, ctx1):
+    torch = torch_cuda
+    from workloads import trial_vectors
+    X = trial_vectors(sys1, 3)
+    a = ctx1.matvec(torch.from_numpy(X).cuda()).cpu().numpy()
+    b = ctx1.matvec_host(X)
+    assert np.array_equal(a, b)
+
+
+def test_matvec_rejects_bad_arguments(torch_cuda, ctx1):
+    torch = torch_cuda
+    from paper_2603_29257_b200 import RispError
+    X = torch.zeros((2, ctx1.nocc, ctx1.nvir), dtype=torch.float64, device="cuda")
+    with pytest.raises(RispError):
+        ctx1.matvec(X, sigma=X)                                  # overlap
+    with pytest.raises(RispError):
+        ctx1.matvec(torch.zeros((33, ctx1.nocc, ctx1.nvir), dtype=torch.float64, device="cuda"))
+
+
+def test_no_truncation_and_empty_window(torch_cuda, sys_small_rsh):
+    """cutoff <= 0 keeps everything; a cutoff below every |eps| empties the window and K vanishes."""
+    torch = torch_cuda
+    from paper_2603_29257_b200 import setup
+    from oracle.risp_oracle import Oracle
+    from workloads import trial_vectors
+    X = trial_vectors(sys_small_rsh, 2)
+    for cut in (0.0, 0.5 * float(np.min(np.abs(sys_small_rsh["eps"]))) * HARTREE_EV):
+        s = dict(sys_small_rsh); s["cutoff_ev"] = cut
+        o = Oracle(s)
+        c = setup(s)
+        got = c.matvec(torch.from_numpy(X).cuda()).cpu().numpy()
+        assert _rel(got, o.sigma(X)) <= 1e-10
+        c.close()
+
+
+# ------------------------------------------------------------------------------------------------ screening
+def test_screened_pairs_are_negligible(ctx1, oracle1, torch_cuda, sys_small_rsh, oracle_small_rsh, ctx_rsh):
+    for ctx, o in ((ctx1, oracle1), (ctx_rsh, oracle_small_rsh)):
+        kept = {(int(a), int(b)) for a, b in ctx.stage("PAIRS")}
+        kept |= {(b, a) for a, b in kept}
+        soff, _ = _shell_offsets(o)
+        I3 = o.int3c(o.selJ)
+        for sa in range(o.nshl):
+            for sb in range(sa + 1):
+                if (sa, sb) not in kept:
+                    assert np.abs(I3[:, soff[sa]:soff[sa + 1], soff[sb]:soff[sb + 1]]).max() < 1e-13
+
+
+# ------------------------------------------------------------------------------------------------ Davidson
+@pytest.mark.parametrize("which", ["tiny", "rsh"])
+def test_tda_roots(which, ctx1, oracle1, ctx_rsh, oracle_small_rsh):
+    ctx, o = (ctx1, oracle1) if which == "tiny" else (ctx_rsh, oracle_small_rsh)
+    n = 5
+    w_ref = np.linalg.eigvalsh(o.full_A())[:n]
+    omega, X, info = ctx.tda_solve(n, tol=1e-8, n_guess=n if which == "tiny" else 0, want_vectors=True)
+    assert info["converged"] == 1
+    assert np.abs(omega - w_ref).max() * HARTREE_EV <= 1e-6
+    Xh = X.cpu().numpy()
+    res = o.sigma(Xh) - omega[:, None, None] * Xh
+    assert np.linalg.norm(res.reshape(n, -1), axis=1).max() < 1e-7
+
+
+def test_tda_restart_path(ctx1, oracle1):
+    w_ref = np.linalg.eigvalsh(oracle1.full_A())[:3]
+    omega, _, info = ctx1.tda_solve(3, tol=1e-8, max_sub=30, max_iter=300)
+    assert info["restarts"] > 0 and info["converged"] == 1
+    assert np.abs(omega - w_ref).max() * HARTREE_EV <= 1e-6
+
+
+# ------------------------------------------------------------------------------------------------ 100-atom config
+@pytest.fixture(scope="module")
+def cfg2(torch_cuda):
+    from workloads import make_system
+    from oracle.risp_oracle import Oracle
+    from paper_2603_29257_b200 import setup
+    s = make_system(2)
+    o = Oracle(s)
+    o.build()
+    c = setup(s)
+    yield s, o, c
+    c.close()
+
+
+def test_cfg2_sigma_parity(torch_cuda, cfg2):
+    """BASELINE.json configs[1] at full size and bench batch (m = 30): several tiles and ragged tails everywhere."""
+    torch = torch_cuda
+    from workloads import trial_vectors
+    s, o, c = cfg2
+    X = trial_vectors(s)
+    sig_ref, dg, J_ref, K_ref = o.sigma(X, parts=True)
+    sig = c.matvec(torch.from_numpy(X).cuda()).cpu().numpy()
+    m = X.shape[0]
+    assert _rel(c.stage("J", m), J_ref) <= 1e-10
+    assert _rel(c.stage("K", m), K_ref) <= 1e-10
+    assert _rel(sig, sig_ref) <= 1e-10
+
+
+def test_cfg2_roots(cfg2):
+    s, o, c = cfg2
+    th_ref, _, info_ref = o.davidson(15, tol=1e-8)
+    assert info_ref["converged"]
+    omega, _, info = c.tda_solve(15, tol=1e-8)
+    assert info["converged"] == 1
+    assert np.abs(omega - th_ref).max() * HARTREE_EV <= 1e-6
