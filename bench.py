@@ -1,0 +1,246 @@
+#!/usr/bin/env python
+"""bench.py -- sigma-builds/s of the TDA-risp hot path on seeded synthetic systems (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path: one `risp_matvec` over a batch of m trial vectors (J + K + diagonal,
+all SURVEY 8(a) rows a4-a12) with the setup (pair list, metrics, K tensors) already built and X resident in HBM.
+`value` = m * K / (sum of the K device-timed steps), max over ranks; `e2e` = the same through `risp_matvec_host`
+(pinned HOST buffers, H2D and D2H inside the timed region).  Between timed iterations L2 is flushed by writing a
+512 MiB buffer.  N > 1: every rank owns its own batch of m vectors (the path shards by trial vector with no
+collective), weak scaling.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on the same workload, metric and unit.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "TDA-risp sigma-builds/s (15-root wall time and % of FP64 tensor/HBM roofline alongside)"
+UNIT = "sigma-builds/s"
+FP64_PER_BF16 = 45.0 / 2250.0     # nominal B200 dense FP64-tensor : bf16-tensor ratio (blackwell guide: 45 TF vs 2.25 PF)
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=d["hbm_gbs"], bf16=d["bf16_tflops"], bf16_sustained=d.get("bf16_tflops_sustained", d["bf16_tflops"]), src="measured")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sustained=1400.0, src="fallback")
+
+
+class ClockSampler:
+    FIELDS = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index=0):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.proc.terminate()
+        rows = [r for t, r in self.rows if t0 <= t <= t1 + 0.2] or [r for _, r in self.rows]
+        if not rows:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["no samples"])
+        sm = sorted(float(r[0]) for r in rows if r[0].replace(".", "").isdigit())
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(len(r) > 2 + k and r[2 + k] == "Active" for r in rows)]
+        return dict(sm_mhz=sm[len(sm) // 2] if sm else None, sm_max_mhz=float(rows[0][1]) if rows[0][1].replace(".", "").isdigit() else None,
+                    reasons=reasons, samples=len(rows))
+
+
+def run_reference(args):
+    """The CPU oracle as the reference arm: sigma-builds/s of oracle.sigma on a bounded sample of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle.risp_oracle import Oracle
+    from workloads import make_system, trial_vectors
+    s = make_system(args.config)
+    o = Oracle(s)
+    t0 = time.time(); o.build(); t_build = time.time() - t0
+    m_s = min(s["m"], args.ref_vectors)
+    X = trial_vectors(s)[:m_s]
+    for _ in range(args.warmup):
+        o.sigma(X)
+    t0 = time.time()
+    for _ in range(args.steps):
+        o.sigma(X)
+    dt = time.time() - t0
+    val = m_s * args.steps / dt
+    cores = os.cpu_count()
+    line = dict(impl="reference", metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                ms_per_step=1e3 * dt / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+                config=dict(workload=s["name"], m=m_s, nao=s["nao"], nocc=s["nocc"], nvir=s["nvir"]),
+                cpu_baseline=dict(value=val, unit=UNIT, cores=cores, kind="oracle",
+                                  sample=f"oracle.sigma on {m_s} of the {s['m']} trial vectors per step; tensor build ({t_build:.1f} s) excluded like risp_setup"),
+                e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="risp", choices=["risp", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index + 1 (default 2: the 100-atom system)")
+    ap.add_argument("--ref-vectors", type=int, default=30, help="trial vectors per step of the CPU oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--solve", action="store_true", help="also time the 15-root risp_tda_solve (reported under 'solve')")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "risp" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2603_29257_b200 import setup
+    from workloads import make_system, trial_vectors
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    dev = torch.device(f"cuda:{local}")
+
+    s = make_system(args.config)
+    m = s["m"]
+    # every rank gets its own seeded batch of m trial vectors (weak scaling over trial vectors, no collective)
+    X_h = trial_vectors(s, base_seed=260329257 + 17 * rank)
+    t0 = time.time()
+    ctx = setup(s, device=local)
+    t_setup = time.time() - t0
+    d = ctx.dims()
+    X = torch.from_numpy(X_h).to(dev)
+    sigma = torch.empty_like(X)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream(dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident timing
+    for _ in range(args.warmup):
+        ctx.matvec(X, sigma)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    tw0 = time.time()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    phase = {}
+    for a, b in evs:
+        flush.zero_()
+        a.record(stream)
+        ctx.matvec(X, sigma)
+        b.record(stream)
+        b.synchronize()
+        for k, v in ctx.timings().items():
+            phase[k] = phase.get(k, 0.0) + (v if isinstance(v, float) else 0.0)
+    barrier()
+    tw1 = time.time()
+    clocks = sampler.stop(tw0, tw1) if sampler else None
+    t_dev = sum(a.elapsed_time(b) for a, b in evs) * 1e-3
+    tim = ctx.timings()
+    launches = tim["kernel_launches"] * args.steps
+
+    # ---- end to end: pinned host buffers through risp_matvec_host
+    Xp = torch.from_numpy(X_h).pin_memory()
+    Sp = torch.empty_like(Xp).pin_memory()
+    for _ in range(2):
+        ctx.matvec_host_ptr(m, Xp.data_ptr(), Sp.data_ptr())
+    barrier()
+    t_e2e = 0.0
+    for _ in range(args.steps):
+        flush.zero_(); torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        ctx.matvec_host_ptr(m, Xp.data_ptr(), Sp.data_ptr())
+        t_e2e += time.perf_counter() - t0
+    barrier()
+    if world > 1:
+        tt = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_dev, t_e2e = float(tt[0]), float(tt[1])
+    same = bool(np.array_equal(Sp.numpy(), sigma.cpu().numpy()))
+
+    if rank == 0:
+        pk = _peaks()
+        no, nv, nK = d["noccK"], d["nvirK"], d["nauxK"]
+        # dominant kernel: the DMMA GEMM launch M^P = X' T_ab^P (Eq. 22) of the first aux chunk
+        npf = tim["first_chunk_naux"]
+        flops_launch = 2.0 * m * no * nv * nv * npf
+        t_launch = phase["k_gemm1"] / args.steps
+        achieved = flops_launch / t_launch / 1e12 if t_launch > 0 else 0.0
+        peak = pk["bf16"] * FP64_PER_BF16
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", f"traffic_cfg{args.config}.json")
+        if os.path.exists(tpath):
+            traffic = json.load(open(tpath)).get("dgemm_k_gemm1_dram_bytes_per_launch")
+        flops_step = dict(K=2.0 * m * nK * no * nv * (no + nv), transforms=4.0 * m * s["nocc"] * s["nvir"] * s["nao"] + 4.0 * m * s["nao"] ** 2 * s["nocc"])
+        line = dict(
+            metric=METRIC, value=world * m * args.steps / t_dev, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+            ms_per_step=1e3 * t_dev / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+            config=dict(workload=s["name"], m=m, atoms=int(s["natm"]), nao=s["nao"], nocc=s["nocc"], nvir=s["nvir"], nauxJ=d["nauxJ"], nauxK=nK,
+                        noccK=no, nvirK=nv, shell_pairs_kept=d["n_shell_pairs_kept"], shell_pairs=d["n_shell_pairs"],
+                        ao_pair_survival=round(2.0 * d["n_ao_pairs_kept"] / (s["nao"] * (s["nao"] + 1)), 4),
+                        K_tensors="HBM", bytes_T=d["bytes_Tij"] + d["bytes_Tab"], aux_chunk=d["aux_chunk"], l2="flushed between steps (512 MiB write)",
+                        parallelism=f"trial-vector shards x{world}", setup_s=round(t_setup, 3)),
+            clocks=clocks,
+            e2e=dict(value=world * m * args.steps / t_e2e, unit=UNIT, h2d_bytes_per_step=int(X_h.nbytes), d2h_bytes_per_step=int(X_h.nbytes),
+                     bitwise_equal_to_device_path=same),
+            gpu_launches=launches,
+            roofline=dict(bound="tensor", kernel="dgemm_kernel<KC,KC> (K contraction M^P = X' T_ab^P, Eq. 22)", achieved=achieved, peak=peak,
+                          unit="TFLOP/s", frac=achieved / peak, traffic=traffic,
+                          peak_source=f"{pk['src']} bf16 burst {pk['bf16']} TFLOP/s x nominal FP64:bf16 ratio 45/2250",
+                          flops_per_launch=flops_launch, launch_ms=1e3 * t_launch),
+            phases_ms={k: round(1e3 * v / args.steps, 4) for k, v in phase.items() if k not in ("kernel_launches", "first_chunk_naux")},
+            flops_per_step=flops_step,
+        )
+        if not args.no_cpu_baseline and world == 1:
+            from oracle.risp_oracle import Oracle
+            o = Oracle(s)
+            t0 = time.time(); o.build(); tb = time.time() - t0
+            ms_ = min(m, 30)
+            t0 = time.time(); ref = o.sigma(X_h[:ms_]); dt = time.time() - t0
+            err = float(np.linalg.norm(sigma.cpu().numpy()[:ms_] - ref) / np.linalg.norm(ref))
+            line["cpu_baseline"] = dict(value=ms_ / dt, unit=UNIT, cores=os.cpu_count(), kind="oracle",
+                                        sample=f"one oracle.sigma call on {ms_} of the {m} trial vectors ({dt:.1f} s); tensor build ({tb:.1f} s) excluded like risp_setup",
+                                        gpu_vs_oracle_rel_err=err)
+        if args.solve:
+            omega, _, info = ctx.tda_solve(s["nroots"], tol=1e-5, allow_unconverged=True)
+            line["solve"] = dict(nroots=s["nroots"], tol=1e-5, wall_s=info["sec_total"], matvec_s=info["sec_matvec"], iterations=info["iterations"],
+                                 n_sigma=info["n_sigma"], restarts=info["restarts"], converged=info["converged"], omega_ev=[float(x) * 27.211386245988 for x in omega],
+                                 h2d_gb=info["bytes_h2d"] / 1e9, d2h_gb=info["bytes_d2h"] / 1e9)
+        print(json.dumps(line))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -109,8 +109,11 @@ typedef struct {
 
 /* per-phase device seconds of the last risp_matvec (CUDA events; valid after the stream was synchronised) */
 typedef struct {
-    double total, j_transform_in, j_pass1, j_solve, j_pass2, j_transform_out, k_gather, k_gemm1, k_gemm2, assemble;
-    int32_t kernel_launches;
+    double total, j_transform_in, j_pass1, j_solve, j_pass2, j_transform_out, k_gather;
+    double k_gemm1, k_gemm2;     /* the FIRST aux chunk's M^P = X' T_ab^P launch (Eq. 22) and K' += T_ij^P M^P launch (Eq. 23) */
+    double k_total, assemble;    /* all chunks of the K contraction; sigma assembly */
+    int32_t kernel_launches;     /* kernels launched by the last risp_matvec */
+    int32_t first_chunk_naux;    /* K aux functions in the first chunk (work of the two timed launches) */
 } risp_timings;
 
 /* Build everything that does not depend on X: screened shell-pair list, metrics (P|Q)_J, (P|J^|Q)_K and their

@@ -59,7 +59,8 @@ class _Dims(C.Structure):
 
 class _Timings(C.Structure):
     _fields_ = [(n, C.c_double) for n in ("total", "j_transform_in", "j_pass1", "j_solve", "j_pass2", "j_transform_out",
-                                          "k_gather", "k_gemm1", "k_gemm2", "assemble")] + [("kernel_launches", C.c_int32)]
+                                          "k_gather", "k_gemm1", "k_gemm2", "k_total", "assemble")] + \
+               [("kernel_launches", C.c_int32), ("first_chunk_naux", C.c_int32)]
 
 
 def library_path() -> str:

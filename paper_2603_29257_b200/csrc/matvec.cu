@@ -119,11 +119,13 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
             d.nb1 = np; d.sB1 = (long long)nv * nv; d.sC1 = (long long)no * nv;
             d.c_rpg = no; d.c_gstride = (long long)np * no * nv;
             RISP_CUDA_TRY(risp_dgemm(d, st)); ++launches;
+            if (p0 == 0) RISP_CUDA_TRY(cudaEventRecord(ev[9], st));
             // K'[mi][i][a] (+)= sum_{(P,j)} T_ij[i][(P,j)] M[mi][(P,j)][a]
             GemmDesc e = gemm_desc(no, nv, np * no, ctx->d_Tij + (long long)p0 * no, (long long)nK * no, true, ctx->w_M, nv, false, ctx->w_Kk, nv,
                                    1.0, p0 == 0 ? 0.0 : 1.0);
             e.nb1 = m; e.sB1 = (long long)np * no * nv; e.sC1 = (long long)no * nv;
             RISP_CUDA_TRY(risp_dgemm(e, st)); ++launches;
+            if (p0 == 0) { RISP_CUDA_TRY(cudaEventRecord(ev[10], st)); ctx->tim.first_chunk_naux = np; }
         }
     } else {
         RISP_CUDA_TRY(cudaEventRecord(ev[6], st));
