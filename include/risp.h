@@ -75,11 +75,18 @@ typedef struct {
 
 typedef struct {
     double screen_tol;          /* shell-pair screening threshold tau (0 -> default 1e-13; < 0 -> keep every pair) */
-    size_t hbm_budget_bytes;    /* 0 -> 85 % of the free device memory at setup */
+    size_t hbm_budget_bytes;    /* device memory the library may use (0 -> 85 % of what is free at setup); K-tensor slices that do
+                                   not fit are kept in pinned host memory and streamed per matvec */
     size_t host_budget_bytes;   /* pinned-host budget of the Davidson subspace; 0 -> 8 GiB */
     int32_t device;             /* CUDA device ordinal */
-    int32_t flags;              /* reserved, 0 */
+    int32_t flags;              /* RISP_FLAG_* */
+    int32_t max_batch;          /* largest m the caller will pass to risp_matvec (0 -> 32); HBM is reserved for its X, sigma
+                                   and work space before the K tensors are placed */
+    int32_t reserved;
 } risp_options;
+
+#define RISP_FLAG_KEEP_STAGES 1   /* keep J_mia of the last risp_matvec for risp_get_stage (costs one more [m][nocc][nvir] buffer) */
+#define RISP_FLAG_SPILL_HALF 2    /* testing: place the upper half of the K-tensor slices in pinned host memory regardless of the budget */
 
 typedef struct {
     double tol;                 /* residual 2-norm threshold (0 -> 1e-5) */
@@ -103,15 +110,18 @@ typedef struct {
     int32_t noccK, nvirK, occK_first, virK_first; /* window: occupied [occK_first, occK_first+noccK), virtual likewise
                                                      (indices within occ / within vir) */
     int64_t n_shell_pairs, n_shell_pairs_kept, n_ao_pairs_kept;
-    int64_t bytes_Tij, bytes_Tab, bytes_device_total;
+    int64_t bytes_Tij, bytes_Tab, bytes_device_total; /* K tensors as stored (packed lower triangles), all device allocations */
     int32_t aux_chunk;                   /* K auxiliary functions per chunk in the matvec */
+    int32_t nauxK_device;                /* K-tensor slices resident in HBM; the other nauxK - nauxK_device live in pinned host memory */
+    int64_t bytes_T_host;                /* pinned host bytes of the spilled slices */
+    int32_t j_sub_batch, j_panels;       /* J transforms: trial vectors per sub-batch, AO row panels per sub-batch (1 = dense) */
 } risp_dims;
 
 /* per-phase device seconds of the last risp_matvec (CUDA events; valid after the stream was synchronised) */
 typedef struct {
     double total, j_transform_in, j_pass1, j_solve, j_pass2, j_transform_out, k_gather;
     double k_gemm1, k_gemm2;     /* the FIRST aux chunk's M^P = X' T_ab^P launch (Eq. 22) and K' += T_ij^P M^P launch (Eq. 23) */
-    double k_total, assemble;    /* all chunks of the K contraction; sigma assembly */
+    double k_total, assemble;    /* all chunks of the K contraction (expansion of the packed slices included); sigma -= K' */
     int32_t kernel_launches;     /* kernels launched by the last risp_matvec */
     int32_t first_chunk_naux;    /* K aux functions in the first chunk (work of the two timed launches) */
 } risp_timings;
@@ -148,7 +158,7 @@ int risp_eri3c_shell(risp_ctx *ctx, int32_t shl_i, int32_t shl_j, int32_t aux_k,
 /* Intermediate of the LAST risp_matvec / setup, copied to out_host (HOST).  `which`: */
 #define RISP_STAGE_R 1       /* R_mQ (Eq. 14):  out[nauxJ][m]                                   sel ignored */
 #define RISP_STAGE_RTILDE 2  /* R~_mP (Eq. 15): out[nauxJ][m]                                                */
-#define RISP_STAGE_J 3       /* J_mia (Eq. 17): out[m][nocc][nvir]                                           */
+#define RISP_STAGE_J 3       /* J_mia (Eq. 17): out[m][nocc][nvir]            needs RISP_FLAG_KEEP_STAGES            */
 #define RISP_STAGE_K 4       /* K_mia (Eq. 23) scattered to the full space: out[m][nocc][nvir]               */
 #define RISP_STAGE_TIJ 5     /* T_ij^P for the K-aux functions P in sel: out[nsel][noccK][noccK]             */
 #define RISP_STAGE_TAB 6     /* T_ab^P:                                  out[nsel][nvirK][nvirK]             */

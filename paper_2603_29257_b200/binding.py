@@ -13,6 +13,7 @@ EXPORTED_SYMBOLS = ["risp_setup", "risp_matvec", "risp_matvec_host", "risp_tda_s
                     "risp_get_dims", "risp_get_timings", "risp_eri3c_shell", "risp_get_stage"]
 
 RISP_MAX_ROOTS = 64
+FLAG_KEEP_STAGES, FLAG_SPILL_HALF = 1, 2
 STAGE = dict(R=1, RTILDE=2, J=3, K=4, TIJ=5, TAB=6, PAIRS=7, METRIC_J=8, METRIC_K=9, U=10)
 _ERR = {-1: "RISP_EINVAL", -2: "RISP_ENOMEM", -3: "RISP_ECUDA", -4: "RISP_ENOTPD", -5: "RISP_ENOTCONV"}
 
@@ -37,7 +38,7 @@ class _System(C.Structure):
 
 class _Options(C.Structure):
     _fields_ = [("screen_tol", C.c_double), ("hbm_budget_bytes", C.c_size_t), ("host_budget_bytes", C.c_size_t),
-                ("device", C.c_int32), ("flags", C.c_int32)]
+                ("device", C.c_int32), ("flags", C.c_int32), ("max_batch", C.c_int32), ("reserved", C.c_int32)]
 
 
 class _SolveOptions(C.Structure):
@@ -54,7 +55,8 @@ class _Dims(C.Structure):
     _fields_ = [("nao", C.c_int32), ("nocc", C.c_int32), ("nvir", C.c_int32), ("nauxJ", C.c_int32), ("nauxK", C.c_int32),
                 ("noccK", C.c_int32), ("nvirK", C.c_int32), ("occK_first", C.c_int32), ("virK_first", C.c_int32),
                 ("n_shell_pairs", C.c_int64), ("n_shell_pairs_kept", C.c_int64), ("n_ao_pairs_kept", C.c_int64),
-                ("bytes_Tij", C.c_int64), ("bytes_Tab", C.c_int64), ("bytes_device_total", C.c_int64), ("aux_chunk", C.c_int32)]
+                ("bytes_Tij", C.c_int64), ("bytes_Tab", C.c_int64), ("bytes_device_total", C.c_int64), ("aux_chunk", C.c_int32),
+                ("nauxK_device", C.c_int32), ("bytes_T_host", C.c_int64), ("j_sub_batch", C.c_int32), ("j_panels", C.c_int32)]
 
 
 class _Timings(C.Structure):
@@ -90,6 +92,8 @@ def load_library():
     lib.risp_debug_dgemm.argtypes = [C.c_int, C.c_int, C.c_int, vp, C.c_longlong, C.c_int, vp, C.c_longlong, C.c_int, vp, C.c_longlong,
                                      dbl, dbl, C.c_int, C.c_longlong, C.c_longlong, C.c_longlong, vp]
     lib.risp_debug_sym_eig.argtypes = [C.c_int, vp, vp, vp]
+    lib.risp_debug_force_plan.argtypes = [vp, C.c_int, C.c_int, C.c_int]
+    lib.risp_debug_set_gemm_variant.argtypes = [C.c_int]
     _LIB = lib
     return lib
 
@@ -105,7 +109,8 @@ def _struct_dict(s):
 class RispContext:
     """Owns one `risp_ctx`.  X / sigma are torch CUDA tensors (device pointers go straight through the ABI)."""
 
-    def __init__(self, sys: dict, screen_tol: float = 0.0, hbm_budget_bytes: int = 0, host_budget_bytes: int = 0, device: int = 0):
+    def __init__(self, sys: dict, screen_tol: float = 0.0, hbm_budget_bytes: int = 0, host_budget_bytes: int = 0, device: int = 0,
+                 flags: int = 0, max_batch: int = 0):
         self.lib = load_library()
         keep = {}
 
@@ -125,7 +130,7 @@ class RispContext:
         s.nao, s.nocc, s.nvir = int(sys["nao"]), int(sys["nocc"]), int(sys["nvir"])
         s.C = arr("C", np.float64); s.eps = arr("eps", np.float64)
         s.alpha, s.beta, s.omega, s.cutoff_ev = float(sys["alpha"]), float(sys["beta"]), float(sys["omega"]), float(sys["cutoff_ev"])
-        o = _Options(float(screen_tol), int(hbm_budget_bytes), int(host_budget_bytes), int(device), 0)
+        o = _Options(float(screen_tol), int(hbm_budget_bytes), int(host_budget_bytes), int(device), int(flags), int(max_batch), 0)
         self.handle = C.c_void_p()
         self.nocc, self.nvir, self.nao = s.nocc, s.nvir, s.nao
         self.device = device
@@ -186,6 +191,10 @@ class RispContext:
         d = _struct_dict(info)
         d["resid"] = d["resid"][:nroots]
         return omega, X, d
+
+    def force_plan(self, mj: int = 0, prow: int = 0, pc: int = 0):
+        """Testing: override the work-space plan (J sub-batch, AO rows per panel, K aux chunk); 0 keeps the automatic choice."""
+        self._check(self.lib.risp_debug_force_plan(self.handle, mj, prow, pc))
 
     # ---- getters
     def dims(self) -> dict:

@@ -8,15 +8,22 @@ extern "C" void risp_destroy(risp_ctx *ctx)
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     cudaDeviceSynchronize();
-    double **bufs[] = {&ctx->d_C, &ctx->d_eps, &ctx->d_boys, &ctx->d_MJ, &ctx->d_LinvJ, &ctx->d_MK, &ctx->d_MKinv, &ctx->d_Tij, &ctx->d_Tab,
-                       &ctx->w_Y, &ctx->w_D, &ctx->w_dbar, &ctx->w_Rpart, &ctx->w_R, &ctx->w_Rt, &ctx->w_Rtmp, &ctx->w_J, &ctx->w_Xk, &ctx->w_Kk,
-                       &ctx->w_M, &ctx->w_Xin, &ctx->w_Sout};
+    risp_free_workspace(ctx);
+    if (ctx->w_Xin) cudaFree(ctx->w_Xin);
+    if (ctx->w_Sout) cudaFree(ctx->w_Sout);
+    double **bufs[] = {&ctx->d_Cocc, &ctx->d_Cvir, &ctx->d_eps, &ctx->d_boys, &ctx->d_MJ, &ctx->d_LinvJ, &ctx->d_MK, &ctx->d_MKinv, &ctx->d_TijP,
+                       &ctx->d_TabP};
     for (auto b : bufs) if (*b) cudaFree(*b);
+    if (ctx->h_TijP) cudaFreeHost(ctx->h_TijP);
+    if (ctx->h_TabP) cudaFreeHost(ctx->h_TabP);
     for (int c = 0; c < 6; ++c) if (ctx->cls[c].d_pairs) cudaFree(ctx->cls[c].d_pairs);
     if (ctx->d_prims) cudaFree(ctx->d_prims);
     if (ctx->d_cenJ) cudaFree(ctx->d_cenJ);
     if (ctx->d_cenK) cudaFree(ctx->d_cenK);
-    if (ctx->ev_ok) for (int i = 0; i < 12; ++i) cudaEventDestroy(ctx->ev[i]);
+    if (ctx->ev_ok) {
+        for (int i = 0; i < RISP_NEV; ++i) cudaEventDestroy(ctx->ev[i]);
+        for (int b = 0; b < 2; ++b) { cudaEventDestroy(ctx->evStage[b]); cudaEventDestroy(ctx->evStageFree[b]); }
+    }
     if (ctx->side) cudaStreamDestroy(ctx->side);
     delete ctx;
 }
@@ -34,10 +41,14 @@ extern "C" int risp_get_dims(const risp_ctx *ctx, risp_dims *out)
     out->nao = ctx->nao; out->nocc = ctx->nocc; out->nvir = ctx->nvir; out->nauxJ = ctx->nauxJ; out->nauxK = ctx->nauxK;
     out->noccK = ctx->noccK; out->nvirK = ctx->nvirK; out->occK_first = ctx->occK0; out->virK_first = ctx->virK0;
     out->n_shell_pairs = ctx->n_shell_pairs; out->n_shell_pairs_kept = ctx->n_shell_pairs_kept; out->n_ao_pairs_kept = ctx->n_ao_pairs_kept;
-    out->bytes_Tij = ctx->has_K ? (int64_t)ctx->nauxK * ctx->noccK * ctx->noccK * 8 : 0;
-    out->bytes_Tab = ctx->has_K ? (int64_t)ctx->nauxK * ctx->nvirK * ctx->nvirK * 8 : 0;
+    out->bytes_Tij = ctx->has_K ? (int64_t)ctx->nauxK * ctx->tri_o * 8 : 0;
+    out->bytes_Tab = ctx->has_K ? (int64_t)ctx->nauxK * ctx->tri_v * 8 : 0;
     out->bytes_device_total = (int64_t)(ctx->setup_bytes + ctx->w_bytes);
-    out->aux_chunk = ctx->aux_chunk;
+    out->aux_chunk = ctx->plan.pc;
+    out->nauxK_device = ctx->has_K ? ctx->nK_dev : 0;
+    out->bytes_T_host = ctx->has_K ? (int64_t)(ctx->nauxK - ctx->nK_dev) * (ctx->tri_o + ctx->tri_v) * 8 : 0;
+    out->j_sub_batch = ctx->plan.mj;
+    out->j_panels = ctx->plan.panel_r0.empty() ? 0 : (int)ctx->plan.panel_r0.size() - 1;
     return RISP_OK;
 }
 
@@ -126,6 +137,7 @@ extern "C" int risp_get_stage(risp_ctx *ctx, int32_t which, const int64_t *sel, 
     }
     case RISP_STAGE_J:
         if (need_mv()) return RISP_EINVAL;
+        if (!ctx->w_J) { risp_set_error(ctx, "risp_get_stage: J is kept only with RISP_FLAG_KEEP_STAGES"); return RISP_EINVAL; }
         RISP_CUDA_TRY(cudaMemcpy(out, ctx->w_J, (size_t)m * ctx->nocc * ctx->nvir * 8, cudaMemcpyDeviceToHost));
         return RISP_OK;
     case RISP_STAGE_K: {
@@ -134,7 +146,8 @@ extern "C" int risp_get_stage(risp_ctx *ctx, int32_t which, const int64_t *sel, 
         if (!ctx->has_K) { std::memset(out, 0, n * 8); return RISP_OK; }
         double *tmp = nullptr;
         RISP_CUDA_TRY(cudaMalloc((void **)&tmp, n * 8));
-        RISP_CUDA_TRY(risp_scatter_window(ctx->w_Kk, tmp, m, ctx->nocc, ctx->nvir, ctx->occK0, ctx->noccK, ctx->virK0, ctx->nvirK, 0));
+        const double *wKk = ctx->w_arena + (size_t)m * ctx->noccK * ctx->nv_p;     // K' of the last matvec (matvec.cu arena layout)
+        RISP_CUDA_TRY(risp_scatter_window(wKk, tmp, m, ctx->nocc, ctx->nvir, ctx->occK0, ctx->noccK, ctx->virK0, ctx->nvirK, ctx->nv_p, 0));
         RISP_CUDA_TRY(cudaMemcpy(out, tmp, n * 8, cudaMemcpyDeviceToHost));
         cudaFree(tmp);
         return RISP_OK;
@@ -142,14 +155,24 @@ extern "C" int risp_get_stage(risp_ctx *ctx, int32_t which, const int64_t *sel, 
     case RISP_STAGE_TIJ:
     case RISP_STAGE_TAB: {
         if (!ctx->has_K || !sel) { risp_set_error(ctx, "risp_get_stage: no K tensors / no selection"); return RISP_EINVAL; }
-        const size_t no = ctx->noccK, nv = ctx->nvirK, nK = ctx->nauxK;
+        const bool ij = which == RISP_STAGE_TIJ;
+        const size_t n = ij ? ctx->noccK : ctx->nvirK, nK = ctx->nauxK;
+        const long long tri = ij ? ctx->tri_o : ctx->tri_v;
+        double *full = nullptr, *pk = nullptr;
+        RISP_CUDA_TRY(cudaMalloc((void **)&full, n * n * 8));
+        RISP_CUDA_TRY(cudaMalloc((void **)&pk, (size_t)tri * 8));
         for (int64_t s = 0; s < nsel; ++s) {
-            if (sel[s] < 0 || sel[s] >= (int64_t)nK) { risp_set_error(ctx, "risp_get_stage: aux index out of range"); return RISP_EINVAL; }
-            if (which == RISP_STAGE_TIJ)
-                RISP_CUDA_TRY(cudaMemcpy2D(out + s * no * no, no * 8, ctx->d_Tij + sel[s] * no, nK * no * 8, no * 8, no, cudaMemcpyDeviceToHost));
-            else
-                RISP_CUDA_TRY(cudaMemcpy(out + s * nv * nv, ctx->d_Tab + sel[s] * nv * nv, nv * nv * 8, cudaMemcpyDeviceToHost));
+            if (sel[s] < 0 || sel[s] >= (int64_t)nK) { risp_set_error(ctx, "risp_get_stage: aux index out of range"); cudaFree(full); cudaFree(pk); return RISP_EINVAL; }
+            const double *src;
+            if (sel[s] < ctx->nK_dev) src = (ij ? ctx->d_TijP : ctx->d_TabP) + (size_t)sel[s] * tri;
+            else {
+                RISP_CUDA_TRY(cudaMemcpy(pk, (ij ? ctx->h_TijP : ctx->h_TabP) + (size_t)(sel[s] - ctx->nK_dev) * tri, (size_t)tri * 8, cudaMemcpyHostToDevice));
+                src = pk;
+            }
+            RISP_CUDA_TRY(risp_expand_sym(src, tri, (int)n, 1, full, (long long)n, 0, 0));
+            RISP_CUDA_TRY(cudaMemcpy(out + s * n * n, full, n * n * 8, cudaMemcpyDeviceToHost));
         }
+        cudaFree(full); cudaFree(pk);
         return RISP_OK;
     }
     case RISP_STAGE_PAIRS:
@@ -163,8 +186,16 @@ extern "C" int risp_get_stage(risp_ctx *ctx, int32_t which, const int64_t *sel, 
         RISP_CUDA_TRY(cudaMemcpy(out, ctx->d_MK, (size_t)ctx->nauxK * ctx->nauxK * 8, cudaMemcpyDeviceToHost));
         return RISP_OK;
     case RISP_STAGE_U: {
+        // rebuilt from the e0-space U-bar that the last matvec left in place (pass 2 output)
         if (need_mv() || !sel || sel[0] < 0 || sel[0] >= m) return RISP_EINVAL;
-        RISP_CUDA_TRY(cudaMemcpy(out, ctx->w_D + sel[0] * (size_t)ctx->nao * ctx->nao, (size_t)ctx->nao * ctx->nao * 8, cudaMemcpyDeviceToHost));
+        double *tmp = nullptr;
+        const size_t n = (size_t)ctx->nao * ctx->ldao;
+        RISP_CUDA_TRY(cudaMalloc((void **)&tmp, n * 8));
+        RISP_CUDA_TRY(cudaMemset(tmp, 0, n * 8));
+        for (int c = 0; c < 6; ++c)
+            RISP_CUDA_TRY(risp_e0_to_U(ctx->cls[c], 0, ctx->cls[c].npairs, 1, (int)sel[0], 0, ctx->ldao, (long long)n, 1, ctx->w_dbar, tmp, 0));
+        RISP_CUDA_TRY(cudaMemcpy2D(out, (size_t)ctx->nao * 8, tmp, (size_t)ctx->ldao * 8, (size_t)ctx->nao * 8, ctx->nao, cudaMemcpyDeviceToHost));
+        cudaFree(tmp);
         return RISP_OK;
     }
     default:
@@ -181,4 +212,10 @@ extern "C" int risp_debug_dgemm(int M, int N, int K, const double *A, long long 
     GemmDesc d = gemm_desc(M, N, K, A, lda, a_kc != 0, B, ldb, b_kc != 0, C, ldc, alpha, beta);
     d.nb1 = nbatch; d.sA1 = sA; d.sB1 = sB; d.sC1 = sC;
     return risp_dgemm(d, (cudaStream_t)stream) == cudaSuccess ? RISP_OK : RISP_ECUDA;
+}
+
+extern "C" int risp_debug_set_gemm_variant(int v)
+{
+    risp_dgemm_set_variant(v);
+    return RISP_OK;
 }

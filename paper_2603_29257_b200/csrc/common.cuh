@@ -39,6 +39,7 @@ struct GemmDesc {
     int c_rpg; long long c_gstride;
 };
 cudaError_t risp_dgemm(const GemmDesc &d, cudaStream_t st);
+void risp_dgemm_set_variant(int v);   // tile configuration (debug / tuning only)
 inline GemmDesc gemm_desc(int M, int N, int K, const double *A, long long lda, bool a_kc, const double *B, long long ldb, bool b_kc,
                           double *C, long long ldc, double alpha = 1.0, double beta = 0.0)
 {

@@ -5,16 +5,23 @@
 #include <type_traits>
 
 #define RISP_MS 32   // padded trial-vector stride of R, R~, D-bar, U-bar (one lane per trial vector)
+#define RISP_NEV 16
 
-struct PairClass {                 // kept shell pairs of one (la >= lb) class, sorted together
+struct PairClass {                 // kept shell pairs of one (la >= lb) class, sorted by the first AO of shell A
     int la, lb, npairs;
     risp_eri::ShellPair *d_pairs;  // device
     long long e_off;               // first e0 row of this class in D-bar / U-bar
     int chunk, nchunks, chunk_base; // pass-1 pair chunking (chunk_base: global index of the class's first chunk)
+    std::vector<int> h_aoA;        // host copy of sp.aoA (ascending): row panels of the J transforms are pair ranges
 };
 
-struct DevBuf {                    // grow-only device scratch buffer
-    void *p = nullptr; size_t cap = 0;
+// Plan of one risp_matvec (sizes depend on m and on what the HBM budget leaves after the K tensors).
+struct MatvecPlan {
+    int mj = 0;                    // trial vectors per sub-batch of the AO<->MO transforms of the J path
+    int prow = 0;                  // AO rows per panel of D / U (prow >= nao: one dense panel)
+    int pc = 0;                    // K auxiliary functions per chunk of the exchange contraction
+    std::vector<int> panel_r0;     // panel boundaries (AO rows, even, shell aligned), size npanel + 1
+    size_t arena_bytes = 0;
 };
 
 struct risp_ctx {
@@ -22,21 +29,25 @@ struct risp_ctx {
     int device = 0;
     // ---- dimensions
     int natm = 0, nshl = 0, nao = 0, nocc = 0, nvir = 0, nmo = 0;
+    int ldao = 0, ldocc = 0, ldvir = 0;          // even leading dimensions (TMA needs 16-byte strides)
     int nauxJ = 0, nauxK = 0, ncenJ = 0, ncenK = 0, ncenJ_pad = 0;
-    int noccK = 0, nvirK = 0, occK0 = 0, virK0 = 0;
+    int noccK = 0, nvirK = 0, occK0 = 0, virK0 = 0, no_p = 0, nv_p = 0;
     double alpha = 0, beta = 0, omega = 0;
     bool has_K = false;
     long long n_shell_pairs = 0, n_shell_pairs_kept = 0, n_ao_pairs_kept = 0, e_rows = 0;
     int total_chunks = 0;
     size_t hbm_budget = 0, host_budget = 0;
+    int max_batch = RISP_MS, flags = 0;
     // ---- host copies needed after setup (getters, solver)
     std::vector<double> h_xyz, h_prim_exp, h_prim_d /* coef*radial norm, shell-normalised */, h_eps;
     std::vector<int> h_shl_atom, h_shl_l, h_shl_nprim, h_shl_poff, h_shl_ao;
     std::vector<int> h_aux_atom, h_aux_l, h_aux_fn /* first J function of each aux shell */, h_aux_fnK /* first K function or -1 */;
     std::vector<double> h_aux_exp;
     std::vector<long long> h_kept_pairs;   // (shl_i, shl_j) of every kept pair
+    std::vector<int> h_even_shell_ao;      // AO offsets of shell starts that are even (candidate panel boundaries), ascending
     // ---- device data built by setup
-    double *d_C = nullptr;        // [nao][nmo]
+    double *d_Cocc = nullptr;     // [nao][ldocc]
+    double *d_Cvir = nullptr;     // [nao][ldvir]
     double *d_eps = nullptr;      // [nmo]
     double *d_boys = nullptr;     // Boys table
     PairClass cls[6];
@@ -44,33 +55,43 @@ struct risp_ctx {
     risp_eri::AuxCentre *d_cenJ = nullptr, *d_cenK = nullptr;
     double *d_MJ = nullptr, *d_LinvJ = nullptr;     // (P|Q)_J and the inverse of its Cholesky factor, [nauxJ][nauxJ]
     double *d_MK = nullptr, *d_MKinv = nullptr;     // (P|J^|Q)_K and its inverse, [nauxK][nauxK]
-    double *d_Tij = nullptr;      // [noccK][nauxK][noccK]   T_ij^P of Eq. 20 stored i-major: Tij[i][P][j]
-    double *d_Tab = nullptr;      // [nauxK][nvirK][nvirK]   T_ab^P of Eq. 21, P-major
-    int aux_chunk = 0;            // K aux functions per matvec chunk
+    // K tensors (Eq. 20-21), symmetric in (ij) / (ab): stored as packed lower triangles, P-major.  Slices P < nK_dev live
+    // in HBM, the rest in pinned host memory and are streamed per matvec on the side stream.
+    long long tri_o = 0, tri_v = 0;
+    int nK_dev = 0;
+    double *d_TijP = nullptr, *d_TabP = nullptr;    // [nK_dev][tri_o], [nK_dev][tri_v]
+    double *h_TijP = nullptr, *h_TabP = nullptr;    // pinned [nauxK - nK_dev][tri]
     // ---- matvec work space (sized for m_cap vectors)
     int m_cap = 0;
-    double *w_Y = nullptr;        // [m][nocc][nao]   (X C_vir^T, later C_occ^T U)
-    double *w_D = nullptr;        // [m][nao][nao]    AO density, reused for U
+    MatvecPlan plan;
+    int force_mj = 0, force_prow = 0, force_pc = 0; // debug overrides (risp_debug_force_plan)
+    double *w_arena = nullptr;    // J phase: Y [mj][nocc][ldao], D/U panel [mj][prow][ldao];  K phase: X', K', M, expanded T chunk
     double *w_dbar = nullptr;     // [e_rows][MS]     e0-space density, reused for U-bar
     double *w_Rpart = nullptr, *w_R = nullptr, *w_Rt = nullptr, *w_Rtmp = nullptr;
-    double *w_J = nullptr;        // [m][nocc][nvir]
-    double *w_Xk = nullptr, *w_Kk = nullptr;  // [m][noccK][nvirK]
-    double *w_M = nullptr;        // [m][aux_chunk][noccK][nvirK]
+    double *w_J = nullptr;        // [m][nocc][nvir], only with RISP_FLAG_KEEP_STAGES
+    double *w_stage[2] = {nullptr, nullptr};      // packed host-resident T chunks in flight
     double *w_Xin = nullptr, *w_Sout = nullptr;   // staging for risp_matvec_host
+    int xin_cap = 0;
     size_t w_bytes = 0, setup_bytes = 0;
     int last_m = 0;
-    cudaEvent_t ev[12];
+    cudaEvent_t ev[RISP_NEV];
+    cudaEvent_t evStage[2], evStageFree[2];
     bool ev_ok = false;
     risp_timings tim;
-    cudaStream_t side = nullptr;  // side stream of the Davidson subspace copies
+    cudaStream_t side = nullptr;  // side stream: host-resident K chunks, Davidson subspace copies
 };
 
 // ---- eri_kernels.cu
 cudaError_t risp_eri_fill(int la, int lb, bool hasp, bool erf_op, const risp_eri::ShellPair *pairs, int npairs, const risp_eri::PrimPair *prims,
                           const risp_eri::AuxCentre *cen, int ncen, risp_eri::OpParams op, const double *boys_tab, double *out,
                           long long stride_q, long long ld, int mirror, cudaStream_t st);
-cudaError_t risp_dens_to_e0(const PairClass &pc, int m, int nao, const double *D, double *dbar, cudaStream_t st);
-cudaError_t risp_e0_to_U(const PairClass &pc, int m, int nao, const double *ubar, double *U, cudaStream_t st);
+// D (rows [r0, ...), leading dimension ld, vector stride mstride) -> e0 space, lanes [lane0, lane0 + mj) of pairs [p0, p1).
+// presym: D already holds D + D^T (diagonal shell pairs are then halved).
+cudaError_t risp_dens_to_e0(const PairClass &pc, int p0, int p1, int mj, int lane0, int r0, long long ld, long long mstride, int presym,
+                            const double *D, double *dbar, cudaStream_t st);
+// e0 space -> U rows [r0, ...).  mirror: also write the transposed block (dense single panel); else diagonal shell pairs are halved.
+cudaError_t risp_e0_to_U(const PairClass &pc, int p0, int p1, int mj, int lane0, int r0, long long ld, long long mstride, int mirror,
+                         const double *ubar, double *U, cudaStream_t st);
 cudaError_t risp_j_pass1(const PairClass &pc, const risp_eri::PrimPair *prims, const risp_eri::AuxCentre *cen, int ncen, int ncen_pad,
                          const double *boys_tab, const double *dbar, double *Rpart, cudaStream_t st);
 cudaError_t risp_j_reduce_R(const double *Rpart, int nchunks, const risp_eri::AuxCentre *cen, int ncen, int ncen_pad, double *R, cudaStream_t st);
@@ -82,12 +103,18 @@ cudaError_t risp_j_pass2(const PairClass &pc, const risp_eri::PrimPair *prims, c
 cudaError_t risp_cholesky_inverse(double *A, double *Linv, int n, int *info_host, cudaStream_t st);
 
 // ---- elementwise.cu
-cudaError_t risp_gather_window(const double *X, double *Xk, int m, int nocc, int nvir, int o0, int no, int v0, int nv, cudaStream_t st);
-cudaError_t risp_assemble_sigma(const double *X, const double *J, const double *Kk, const double *eps, double *sigma, int m, int nocc, int nvir,
-                                int o0, int no, int v0, int nv, int has_K, cudaStream_t st);
-cudaError_t risp_scatter_window(const double *Kk, double *Kfull, int m, int nocc, int nvir, int o0, int no, int v0, int nv, cudaStream_t st);
+cudaError_t risp_gather_window(const double *X, double *Xk, int m, int nocc, int nvir, int o0, int no, int v0, int nv, int ldk, cudaStream_t st);
+cudaError_t risp_diag_sigma(const double *X, const double *eps, double *sigma, int m, int nocc, int nvir, cudaStream_t st);
+cudaError_t risp_sub_window(const double *Kk, double *sigma, int m, int nocc, int nvir, int o0, int no, int v0, int nv, int ldk, cudaStream_t st);
+cudaError_t risp_scatter_window(const double *Kk, double *Kfull, int m, int nocc, int nvir, int o0, int no, int v0, int nv, int ldk, cudaStream_t st);
+// packed lower triangle [n(n+1)/2] <-> full symmetric [n][ld]; batched over np slices
+cudaError_t risp_pack_sym(const double *full, long long full_stride, int ld, int n, int np, double *packed, long long tri, cudaStream_t st);
+cudaError_t risp_expand_sym(const double *packed, long long tri, int n, int np, double *full, long long row_stride, long long p_stride,
+                            cudaStream_t st);
 
 // ---- setup.cu / matvec.cu / solve.cu internals
 int risp_ensure_workspace(risp_ctx *ctx, int m);
+size_t risp_plan_workspace(const risp_ctx *ctx, int m, size_t avail, MatvecPlan &plan, bool spilled);
 int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaStream_t st);
 int risp_build_pair(risp_ctx *ctx, int shA, int shB, risp_eri::ShellPair &sp, std::vector<risp_eri::PrimPair> &pp, double prim_tol);
+void risp_free_workspace(risp_ctx *ctx);

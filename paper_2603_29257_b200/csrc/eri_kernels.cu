@@ -58,57 +58,63 @@ __global__ void __launch_bounds__(128) eri_fill_kernel(const ShellPair *__restri
 }
 
 // ------------------------------------------------------------------------------------------------- density -> e0
+// D: rows [r0, ...) of the AO matrices of mj trial vectors (leading dimension ld, vector stride mstride).
+// presym = 0: D is the plain (unsymmetrised) density with all rows present (r0 = 0); the lower-triangular pair takes
+//             D_ab + D_ba (reading G13).  presym = 1: the panel already holds D + D^T; diagonal shell pairs take half.
 template <int LA, int LB>
-__global__ void __launch_bounds__(128) dens_to_e0_kernel(const ShellPair *__restrict__ pairs, int npairs, long long e_off, int m, int nao,
+__global__ void __launch_bounds__(128) dens_to_e0_kernel(const ShellPair *__restrict__ pairs, int p0, int p1, long long e_off, int mj, int lane0,
+                                                         int r0, long long ld, long long mstride, int presym,
                                                          const double *__restrict__ D, double *__restrict__ dbar)
 {
     constexpr int NE = ne_of(LA, LB);
-    int mi = threadIdx.x;
-    int pi = blockIdx.x * blockDim.y + threadIdx.y;
-    if (pi >= npairs) return;
+    const int mi = threadIdx.x;
+    const int pi = p0 + blockIdx.x * blockDim.y + threadIdx.y;
+    if (pi >= p1 || mi >= mj) return;
     const ShellPair sp = pairs[pi];
-    double out[NE];
-    if (mi < m) {
-        const double *Dm = D + (long long)mi * nao * nao;
-        double d[2 * LA + 1][2 * LB + 1];
-#pragma unroll
-        for (int i = 0; i < 2 * LA + 1; ++i)
-#pragma unroll
-            for (int j = 0; j < 2 * LB + 1; ++j) {
-                double v = Dm[(long long)(sp.aoA + i) * nao + sp.aoB + j];
-                if (sp.shA != sp.shB) v += Dm[(long long)(sp.aoB + j) * nao + sp.aoA + i];   // sym(D) on a lower-triangular pair (reading G13)
-                d[i][j] = v;
-            }
-        sph_to_e0_adjoint<LA, LB>(d, sp.ABx, sp.ABy, sp.ABz, out);
-    } else {
-#pragma unroll
-        for (int e = 0; e < NE; ++e) out[e] = 0.0;
-    }
-#pragma unroll
-    for (int e = 0; e < NE; ++e) dbar[(e_off + (long long)pi * NE + e) * MS + mi] = out[e];
-}
-
-template <int LA, int LB>
-__global__ void __launch_bounds__(128) e0_to_U_kernel(const ShellPair *__restrict__ pairs, int npairs, long long e_off, int m, int nao,
-                                                      const double *__restrict__ ubar, double *__restrict__ U)
-{
-    constexpr int NE = ne_of(LA, LB);
-    int mi = threadIdx.x;
-    int pi = blockIdx.x * blockDim.y + threadIdx.y;
-    if (pi >= npairs || mi >= m) return;
-    const ShellPair sp = pairs[pi];
-    double e0[NE];
-#pragma unroll
-    for (int e = 0; e < NE; ++e) e0[e] = ubar[(e_off + (long long)pi * NE + e) * MS + mi];
-    double blk[2 * LA + 1][2 * LB + 1];
-    e0_to_sph<LA, LB>(e0, sp.ABx, sp.ABy, sp.ABz, blk);
-    double *Um = U + (long long)mi * nao * nao;
+    const double *Dm = D + (long long)mi * mstride;
+    double d[2 * LA + 1][2 * LB + 1];
+    const bool diag = sp.shA == sp.shB;
 #pragma unroll
     for (int i = 0; i < 2 * LA + 1; ++i)
 #pragma unroll
         for (int j = 0; j < 2 * LB + 1; ++j) {
-            Um[(long long)(sp.aoA + i) * nao + sp.aoB + j] = blk[i][j];
-            if (sp.shA != sp.shB) Um[(long long)(sp.aoB + j) * nao + sp.aoA + i] = blk[i][j];
+            double v = Dm[(long long)(sp.aoA - r0 + i) * ld + sp.aoB + j];
+            if (presym) { if (diag) v *= 0.5; }
+            else if (!diag) v += Dm[(long long)(sp.aoB + j) * ld + sp.aoA + i];
+            d[i][j] = v;
+        }
+    double out[NE];
+    sph_to_e0_adjoint<LA, LB>(d, sp.ABx, sp.ABy, sp.ABz, out);
+#pragma unroll
+    for (int e = 0; e < NE; ++e) dbar[(e_off + (long long)pi * NE + e) * MS + lane0 + mi] = out[e];
+}
+
+// mirror = 1 (single dense panel, r0 = 0): write the block and its transpose.  mirror = 0: write the block at rows aoA - r0 only,
+// diagonal shell pairs halved, so that U = P + P^T.
+template <int LA, int LB>
+__global__ void __launch_bounds__(128) e0_to_U_kernel(const ShellPair *__restrict__ pairs, int p0, int p1, long long e_off, int mj, int lane0,
+                                                      int r0, long long ld, long long mstride, int mirror,
+                                                      const double *__restrict__ ubar, double *__restrict__ U)
+{
+    constexpr int NE = ne_of(LA, LB);
+    const int mi = threadIdx.x;
+    const int pi = p0 + blockIdx.x * blockDim.y + threadIdx.y;
+    if (pi >= p1 || mi >= mj) return;
+    const ShellPair sp = pairs[pi];
+    double e0[NE];
+#pragma unroll
+    for (int e = 0; e < NE; ++e) e0[e] = ubar[(e_off + (long long)pi * NE + e) * MS + lane0 + mi];
+    double blk[2 * LA + 1][2 * LB + 1];
+    e0_to_sph<LA, LB>(e0, sp.ABx, sp.ABy, sp.ABz, blk);
+    double *Um = U + (long long)mi * mstride;
+    const bool diag = sp.shA == sp.shB;
+    const double f = (!mirror && diag) ? 0.5 : 1.0;
+#pragma unroll
+    for (int i = 0; i < 2 * LA + 1; ++i)
+#pragma unroll
+        for (int j = 0; j < 2 * LB + 1; ++j) {
+            Um[(long long)(sp.aoA - r0 + i) * ld + sp.aoB + j] = f * blk[i][j];
+            if (mirror && !diag) Um[(long long)(sp.aoB + j) * ld + sp.aoA + i] = blk[i][j];
         }
 }
 
@@ -293,22 +299,26 @@ cudaError_t risp_eri_fill(int la, int lb, bool hasp, bool erf_op, const ShellPai
     return cudaGetLastError();
 }
 
-cudaError_t risp_dens_to_e0(const PairClass &pc, int m, int nao, const double *D, double *dbar, cudaStream_t st)
+cudaError_t risp_dens_to_e0(const PairClass &pc, int p0, int p1, int mj, int lane0, int r0, long long ld, long long mstride, int presym,
+                            const double *D, double *dbar, cudaStream_t st)
 {
-    if (pc.npairs <= 0) return cudaSuccess;
-    dim3 block(32, 4), grid((pc.npairs + 3) / 4);
+    if (p1 <= p0) return cudaSuccess;
+    dim3 block(32, 4), grid((p1 - p0 + 3) / 4);
     dispatch_class(pc.la, pc.lb, [&](auto LA, auto LB) {
-        dens_to_e0_kernel<decltype(LA)::value, decltype(LB)::value><<<grid, block, 0, st>>>(pc.d_pairs, pc.npairs, pc.e_off, m, nao, D, dbar);
+        dens_to_e0_kernel<decltype(LA)::value, decltype(LB)::value><<<grid, block, 0, st>>>(pc.d_pairs, p0, p1, pc.e_off, mj, lane0, r0, ld, mstride,
+                                                                                            presym, D, dbar);
     });
     return cudaGetLastError();
 }
 
-cudaError_t risp_e0_to_U(const PairClass &pc, int m, int nao, const double *ubar, double *U, cudaStream_t st)
+cudaError_t risp_e0_to_U(const PairClass &pc, int p0, int p1, int mj, int lane0, int r0, long long ld, long long mstride, int mirror,
+                         const double *ubar, double *U, cudaStream_t st)
 {
-    if (pc.npairs <= 0) return cudaSuccess;
-    dim3 block(32, 4), grid((pc.npairs + 3) / 4);
+    if (p1 <= p0) return cudaSuccess;
+    dim3 block(32, 4), grid((p1 - p0 + 3) / 4);
     dispatch_class(pc.la, pc.lb, [&](auto LA, auto LB) {
-        e0_to_U_kernel<decltype(LA)::value, decltype(LB)::value><<<grid, block, 0, st>>>(pc.d_pairs, pc.npairs, pc.e_off, m, nao, ubar, U);
+        e0_to_U_kernel<decltype(LA)::value, decltype(LB)::value><<<grid, block, 0, st>>>(pc.d_pairs, p0, p1, pc.e_off, mj, lane0, r0, ld, mstride,
+                                                                                         mirror, ubar, U);
     });
     return cudaGetLastError();
 }

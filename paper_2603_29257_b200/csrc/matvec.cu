@@ -1,76 +1,180 @@
 // matvec.cu -- risp_matvec: sigma = A X for a batch of m trial vectors (Eq. 10).
 //
-//   J (Eq. 11-17):  Y = X C_vir^T ; D = C_occ Y (Eq. 12) ; D -> e0 space ; pass 1 (Eq. 14) ;
-//       R~ = L^-T L^-1 R (Eq. 15) ; pass 2 (Eq. 16) ; e0 space -> U ; Z = C_occ^T U ; J = Z C_vir (Eq. 17)
-//   K (Eq. 18-23):  X' = X[window] ; per aux chunk  M^P = X' T_ab^P (Eq. 22) ; K' += T_ij^P M^P (Eq. 23)
-//   sigma = (eps_a - eps_i) X + 2 J - K'  (K' only inside the window)
+//   sigma = (eps_a - eps_i) X                                                                         (diagonal)
+//   J (Eq. 11-17), per sub-batch of mj vectors and per panel of AO rows:
+//       Y = X C_vir^T ; D = C_occ Y (Eq. 12) ; D -> e0 space on the kept pairs ;
+//     then once for all m vectors: pass 1 (Eq. 14) ; R~ = L^-T L^-1 R (Eq. 15) ; pass 2 (Eq. 16) ;
+//     then per sub-batch / panel: e0 space -> U ; Z = C_occ^T U ; sigma += 2 Z C_vir (Eq. 17)
+//   K (Eq. 18-23):  X' = X[window] ; per aux chunk (from HBM, or from pinned host memory through the
+//       side stream): expand the packed slices ; M^P = X' T_ab^P (Eq. 22) ; K' += T_ij^P M^P (Eq. 23) ; sigma[window] -= K'
+//
+// One arena serves the J phase (Y, D/U panel) and then the K phase (X', K', M, expanded T chunk); its size, the sub-batch
+// mj, the panel height and the aux chunk follow from what the HBM budget leaves after the K tensors (risp_plan_workspace).
 #include "ctx.h"
+#include <algorithm>
 
-static void free_ws(risp_ctx *ctx)
+void risp_free_workspace(risp_ctx *ctx)
 {
-    double **bufs[] = {&ctx->w_Y, &ctx->w_D, &ctx->w_dbar, &ctx->w_Rpart, &ctx->w_R, &ctx->w_Rt, &ctx->w_Rtmp, &ctx->w_J,
-                       &ctx->w_Xk, &ctx->w_Kk, &ctx->w_M, &ctx->w_Xin, &ctx->w_Sout};
+    double **bufs[] = {&ctx->w_arena, &ctx->w_dbar, &ctx->w_Rpart, &ctx->w_R, &ctx->w_Rt, &ctx->w_Rtmp, &ctx->w_J,
+                       &ctx->w_stage[0], &ctx->w_stage[1]};
     for (auto b : bufs) { if (*b) cudaFree(*b); *b = nullptr; }
     ctx->m_cap = 0; ctx->w_bytes = 0;
+}
+
+static size_t fixed_ws_bytes(const risp_ctx *ctx)
+{
+    return ((size_t)ctx->e_rows * RISP_MS + (size_t)ctx->total_chunks * ctx->ncenJ_pad * 4 * RISP_MS + 3 * (size_t)ctx->nauxJ * RISP_MS) * sizeof(double);
+}
+
+// Choose (mj, panels, pc) for m vectors within `avail` bytes; returns the bytes needed (arena + staging), 0 if even the
+// smallest plan does not fit.
+size_t risp_plan_workspace(const risp_ctx *ctx, int m, size_t avail, MatvecPlan &pl, bool spilled)
+{
+    const size_t nao = ctx->nao, nocc = ctx->nocc, ldao = ctx->ldao, no = ctx->noccK, nv = ctx->nvirK, no_p = ctx->no_p, nv_p = ctx->nv_p;
+    const int nK = ctx->nauxK;
+    const size_t GiB = (size_t)1 << 30;
+    const size_t stage_per_fn = spilled ? 2 * (size_t)(ctx->tri_o + ctx->tri_v) * 8 : 0;
+    auto kneed = [&](size_t pc) { return (2 * (size_t)m * no * nv_p + (size_t)m * pc * no_p * nv_p + pc * nv * nv_p + no * pc * no_p) * 8 + pc * stage_per_fn; };
+    auto jneed = [&](size_t mj, size_t prow) { return (mj * nocc * ldao + mj * prow * ldao) * 8; };
+    // ---- K chunk
+    size_t karena = 0;
+    pl.pc = 1;
+    if (ctx->has_K) {
+        const size_t klimit = std::min(avail, std::max(6 * GiB, kneed(std::min(2, nK))));
+        if (kneed(1) > avail) return 0;
+        int pc = 1;
+        while (pc < nK && kneed(pc + 1) <= klimit) ++pc;
+        if (ctx->force_pc > 0) pc = std::min(ctx->force_pc, nK);
+        pl.pc = pc;
+        karena = kneed(pc) - pc * stage_per_fn;
+    }
+    // ---- J sub-batch and panels
+    const size_t jlimit = std::min(avail, std::max(karena, 6 * GiB));
+    int mj = m;
+    size_t prow = nao;
+    if (jneed(m, nao) > jlimit) {
+        bool ok = false;
+        for (int div = 1; div <= m && !ok; ++div) {
+            mj = (m + div - 1) / div;
+            const size_t yb = (size_t)mj * nocc * ldao * 8;
+            if (yb > jlimit / 2 && mj > 1) continue;
+            if (yb >= jlimit) break;
+            prow = (jlimit - yb) / ((size_t)mj * ldao * 8);
+            if (prow >= std::min<size_t>(nao, 256) || mj == 1) ok = prow >= 32;
+        }
+        if (!ok) return 0;
+        prow = std::min(prow, nao);
+    }
+    if (ctx->force_mj > 0) mj = std::min(ctx->force_mj, m);
+    if (ctx->force_prow > 0) prow = std::min<size_t>(ctx->force_prow, nao);
+    // panel boundaries: even, shell-aligned AO offsets (TMA coordinates of the MN-contiguous operand must be 16-byte aligned)
+    pl.panel_r0.clear();
+    pl.panel_r0.push_back(0);
+    size_t prow_max = 0;
+    if (prow >= nao) { pl.panel_r0.push_back((int)nao); prow_max = nao; }
+    else {
+        const std::vector<int> &ev = ctx->h_even_shell_ao;
+        int cur = 0;
+        while (cur < (int)nao) {
+            // largest candidate <= cur + prow, but at least the next candidate after cur
+            auto it = std::upper_bound(ev.begin(), ev.end(), cur + (int)prow);
+            int nxt = (it == ev.begin()) ? (int)nao : *(it - 1);
+            if (nxt <= cur) nxt = (it == ev.end()) ? (int)nao : *it;
+            if (cur + (int)prow >= (int)nao) nxt = (int)nao;
+            prow_max = std::max<size_t>(prow_max, nxt - cur);
+            pl.panel_r0.push_back(nxt);
+            cur = nxt;
+        }
+    }
+    pl.mj = mj; pl.prow = (int)prow_max;
+    pl.arena_bytes = std::max(karena, jneed(mj, prow_max));
+    return pl.arena_bytes + (ctx->has_K ? pl.pc * stage_per_fn : 0);
 }
 
 int risp_ensure_workspace(risp_ctx *ctx, int m)
 {
     if (m <= ctx->m_cap) return RISP_OK;
-    free_ws(ctx);
-    const size_t nao = ctx->nao, nocc = ctx->nocc, nvir = ctx->nvir, no = ctx->noccK, nv = ctx->nvirK;
-    size_t fixed = ((size_t)m * nocc * nao + (size_t)m * nao * nao + (size_t)ctx->e_rows * RISP_MS +
-                    (size_t)ctx->total_chunks * ctx->ncenJ_pad * 4 * RISP_MS + 3 * (size_t)ctx->nauxJ * RISP_MS + (size_t)m * nocc * nvir +
-                    2 * (size_t)m * no * nv) * sizeof(double);
-    // aux chunk of the K contraction: M[m][Pc][no][nv] within what is left of the budget (at most 4 GiB)
-    int pc = 1;
-    if (ctx->has_K) {
-        size_t per_fn = (size_t)m * no * nv * sizeof(double);
-        size_t avail = ctx->hbm_budget > ctx->setup_bytes + fixed ? ctx->hbm_budget - ctx->setup_bytes - fixed : 0;
-        avail = std::min<size_t>(avail, (size_t)4 << 30);
-        pc = (int)std::max<size_t>(1, std::min<size_t>((size_t)ctx->nauxK, avail / std::max<size_t>(per_fn, 1)));
-    }
-    ctx->aux_chunk = pc;
-    auto A = [&](double *&p, size_t n) -> int {
-        if (n == 0) { p = nullptr; return RISP_OK; }
-        RISP_CUDA_TRY(cudaMalloc((void **)&p, n * sizeof(double)));
-        ctx->w_bytes += n * sizeof(double);
+    risp_free_workspace(ctx);
+    size_t free_b = 0, total_b = 0;
+    RISP_CUDA_TRY(cudaMemGetInfo(&free_b, &total_b));
+    const size_t fixed = fixed_ws_bytes(ctx) + ((ctx->flags & RISP_FLAG_KEEP_STAGES) ? (size_t)m * ctx->nocc * ctx->nvir * 8 : 0);
+    size_t avail = ctx->hbm_budget > ctx->setup_bytes + fixed ? ctx->hbm_budget - ctx->setup_bytes - fixed : 0;
+    avail = std::min(avail, free_b > fixed + ((size_t)256 << 20) ? free_b - fixed - ((size_t)256 << 20) : 0);
+    const bool spilled = ctx->has_K && ctx->nK_dev < ctx->nauxK;
+    size_t need = risp_plan_workspace(ctx, m, avail, ctx->plan, spilled);
+    if (need == 0) { risp_set_error(ctx, "risp_matvec: the HBM budget leaves no room for the work space of this batch size"); return RISP_ENOMEM; }
+    auto A = [&](double *&p, size_t bytes) -> int {
+        if (bytes == 0) { p = nullptr; return RISP_OK; }
+        RISP_CUDA_TRY(cudaMalloc((void **)&p, bytes));
+        ctx->w_bytes += bytes;
         return RISP_OK;
     };
     int rc;
-    if ((rc = A(ctx->w_Y, (size_t)m * nocc * nao))) return rc;
-    if ((rc = A(ctx->w_D, (size_t)m * nao * nao))) return rc;
-    if ((rc = A(ctx->w_dbar, (size_t)ctx->e_rows * RISP_MS))) return rc;
-    if ((rc = A(ctx->w_Rpart, (size_t)ctx->total_chunks * ctx->ncenJ_pad * 4 * RISP_MS))) return rc;
-    if ((rc = A(ctx->w_R, (size_t)ctx->nauxJ * RISP_MS))) return rc;
-    if ((rc = A(ctx->w_Rt, (size_t)ctx->nauxJ * RISP_MS))) return rc;
-    if ((rc = A(ctx->w_Rtmp, (size_t)ctx->nauxJ * RISP_MS))) return rc;
-    if ((rc = A(ctx->w_J, (size_t)m * nocc * nvir))) return rc;
-    if (ctx->has_K) {
-        if ((rc = A(ctx->w_Xk, (size_t)m * no * nv))) return rc;
-        if ((rc = A(ctx->w_Kk, (size_t)m * no * nv))) return rc;
-        if ((rc = A(ctx->w_M, (size_t)m * pc * no * nv))) return rc;
-    }
+    if ((rc = A(ctx->w_arena, ctx->plan.arena_bytes))) return rc;
+    if ((rc = A(ctx->w_dbar, (size_t)ctx->e_rows * RISP_MS * 8))) return rc;
+    if ((rc = A(ctx->w_Rpart, (size_t)ctx->total_chunks * ctx->ncenJ_pad * 4 * RISP_MS * 8))) return rc;
+    if ((rc = A(ctx->w_R, (size_t)ctx->nauxJ * RISP_MS * 8))) return rc;
+    if ((rc = A(ctx->w_Rt, (size_t)ctx->nauxJ * RISP_MS * 8))) return rc;
+    if ((rc = A(ctx->w_Rtmp, (size_t)ctx->nauxJ * RISP_MS * 8))) return rc;
+    if (ctx->flags & RISP_FLAG_KEEP_STAGES) { if ((rc = A(ctx->w_J, (size_t)m * ctx->nocc * ctx->nvir * 8))) return rc; }
+    if (spilled)
+        for (int b = 0; b < 2; ++b)
+            if ((rc = A(ctx->w_stage[b], (size_t)ctx->plan.pc * (ctx->tri_o + ctx->tri_v) * 8))) return rc;
     RISP_CUDA_TRY(cudaMemset(ctx->w_Rpart, 0, (size_t)ctx->total_chunks * ctx->ncenJ_pad * 4 * RISP_MS * sizeof(double)));
+    RISP_CUDA_TRY(cudaMemset(ctx->w_dbar, 0, (size_t)ctx->e_rows * RISP_MS * sizeof(double)));
+    RISP_CUDA_TRY(cudaMemset(ctx->w_R, 0, (size_t)ctx->nauxJ * RISP_MS * sizeof(double)));
     ctx->m_cap = m;
     return RISP_OK;
 }
 
+// pair range of class c whose shell A starts in AO rows [r0, r1)
+static void panel_pairs(const PairClass &pc, int r0, int r1, int &p0, int &p1)
+{
+    p0 = (int)(std::lower_bound(pc.h_aoA.begin(), pc.h_aoA.end(), r0) - pc.h_aoA.begin());
+    p1 = (int)(std::lower_bound(pc.h_aoA.begin(), pc.h_aoA.end(), r1) - pc.h_aoA.begin());
+}
+
 int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaStream_t st)
 {
-    const int nao = ctx->nao, nocc = ctx->nocc, nvir = ctx->nvir, nmo = ctx->nmo, nJ = ctx->nauxJ;
-    const int no = ctx->noccK, nv = ctx->nvirK, nK = ctx->nauxK;
+    const int nao = ctx->nao, nocc = ctx->nocc, nvir = ctx->nvir, nJ = ctx->nauxJ;
+    const int no = ctx->noccK, nv = ctx->nvirK, nK = ctx->nauxK, no_p = ctx->no_p, nv_p = ctx->nv_p;
+    const long long ldao = ctx->ldao, ldocc = ctx->ldocc, ldvir = ctx->ldvir;
+    const MatvecPlan &pl = ctx->plan;
+    const int npanel = (int)pl.panel_r0.size() - 1;
+    const bool dense = npanel == 1;
     int launches = 0;
     cudaEvent_t *ev = ctx->ev;
     RISP_CUDA_TRY(cudaEventRecord(ev[0], st));
-    // ---------------- J: AO transition density (Eq. 12)
-    {
-        GemmDesc d = gemm_desc(m * nocc, nao, nvir, X, nvir, true, ctx->d_C + nocc, nmo, true, ctx->w_Y, nao);
+    // ---------------- diagonal (Eq. 10)
+    RISP_CUDA_TRY(risp_diag_sigma(X, ctx->d_eps, sigma, m, nocc, nvir, st)); ++launches;
+    // J-phase views of the arena
+    double *wY = ctx->w_arena;                                   // [mj][nocc][ldao]
+    double *wD = wY + (size_t)pl.mj * nocc * ldao;               // [mj][prow][ldao]
+    // ---------------- J: AO transition density (Eq. 12) on the kept pairs, in e0 space
+    for (int l0 = 0; l0 < m; l0 += pl.mj) {
+        const int mj = std::min(pl.mj, m - l0);
+        const double *Xb = X + (size_t)l0 * nocc * nvir;
+        GemmDesc d = gemm_desc(mj * nocc, nao, nvir, Xb, nvir, true, ctx->d_Cvir, ldvir, true, wY, ldao);
         RISP_CUDA_TRY(risp_dgemm(d, st)); ++launches;
-        GemmDesc e = gemm_desc(nao, nao, nocc, ctx->d_C, nmo, true, ctx->w_Y, nao, false, ctx->w_D, nao);
-        e.nb1 = m; e.sB1 = (long long)nocc * nao; e.sC1 = (long long)nao * nao;
-        RISP_CUDA_TRY(risp_dgemm(e, st)); ++launches;
-        for (int c = 0; c < 6; ++c) if (ctx->cls[c].npairs) { RISP_CUDA_TRY(risp_dens_to_e0(ctx->cls[c], m, nao, ctx->w_D, ctx->w_dbar, st)); ++launches; }
+        for (int p = 0; p < npanel; ++p) {
+            const int r0 = pl.panel_r0[p], r1 = pl.panel_r0[p + 1], pr = r1 - r0;
+            const long long mstride = (long long)pr * ldao;
+            // D[mu in panel][nu] = sum_i C_occ[mu][i] Y[i][nu]
+            GemmDesc e = gemm_desc(pr, nao, nocc, ctx->d_Cocc + (size_t)r0 * ldocc, ldocc, true, wY, ldao, false, wD, ldao);
+            e.nb1 = mj; e.sB1 = (long long)nocc * ldao; e.sC1 = mstride;
+            RISP_CUDA_TRY(risp_dgemm(e, st)); ++launches;
+            if (!dense) {
+                // + D^T rows: sum_i Y[i][mu] C_occ[nu][i]   (only sym(D) matters, reading G13)
+                GemmDesc f = gemm_desc(pr, nao, nocc, wY + r0, ldao, false, ctx->d_Cocc, ldocc, true, wD, ldao, 1.0, 1.0);
+                f.nb1 = mj; f.sA1 = (long long)nocc * ldao; f.sC1 = mstride;
+                RISP_CUDA_TRY(risp_dgemm(f, st)); ++launches;
+            }
+            for (int c = 0; c < 6; ++c) {
+                int p0, p1;
+                panel_pairs(ctx->cls[c], r0, r1, p0, p1);
+                if (p1 > p0) { RISP_CUDA_TRY(risp_dens_to_e0(ctx->cls[c], p0, p1, mj, l0, r0, ldao, mstride, dense ? 0 : 1, wD, ctx->w_dbar, st)); ++launches; }
+            }
+        }
     }
     RISP_CUDA_TRY(cudaEventRecord(ev[1], st));
     // ---------------- pass 1: R_mQ (Eq. 14)
@@ -96,44 +200,118 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
             ++launches;
         }
     RISP_CUDA_TRY(cudaEventRecord(ev[4], st));
-    // ---------------- back-transform (Eq. 17)
-    {
-        RISP_CUDA_TRY(cudaMemsetAsync(ctx->w_D, 0, (size_t)m * nao * nao * sizeof(double), st));
-        for (int c = 0; c < 6; ++c) if (ctx->cls[c].npairs) { RISP_CUDA_TRY(risp_e0_to_U(ctx->cls[c], m, nao, ctx->w_dbar, ctx->w_D, st)); ++launches; }
-        GemmDesc d = gemm_desc(nocc, nao, nao, ctx->d_C, nmo, false, ctx->w_D, nao, false, ctx->w_Y, nao);
-        d.nb1 = m; d.sB1 = (long long)nao * nao; d.sC1 = (long long)nocc * nao;
-        RISP_CUDA_TRY(risp_dgemm(d, st)); ++launches;
-        GemmDesc e = gemm_desc(m * nocc, nvir, nao, ctx->w_Y, nao, true, ctx->d_C + nocc, nmo, false, ctx->w_J, nvir);
+    // ---------------- back-transform (Eq. 17), sigma += 2 J
+    for (int l0 = 0; l0 < m; l0 += pl.mj) {
+        const int mj = std::min(pl.mj, m - l0);
+        for (int p = 0; p < npanel; ++p) {
+            const int r0 = pl.panel_r0[p], r1 = pl.panel_r0[p + 1], pr = r1 - r0;
+            const long long mstride = (long long)pr * ldao;
+            RISP_CUDA_TRY(cudaMemsetAsync(wD, 0, (size_t)mj * mstride * sizeof(double), st));
+            for (int c = 0; c < 6; ++c) {
+                int p0, p1;
+                panel_pairs(ctx->cls[c], r0, r1, p0, p1);
+                if (p1 > p0) { RISP_CUDA_TRY(risp_e0_to_U(ctx->cls[c], p0, p1, mj, l0, r0, ldao, mstride, dense ? 1 : 0, ctx->w_dbar, wD, st)); ++launches; }
+            }
+            // Z[i][nu] (+)= sum_{mu in panel} C_occ[mu][i] P[mu][nu]
+            GemmDesc d = gemm_desc(nocc, nao, pr, ctx->d_Cocc + (size_t)r0 * ldocc, ldocc, false, wD, ldao, false, wY, ldao, 1.0, p == 0 ? 0.0 : 1.0);
+            d.nb1 = mj; d.sB1 = mstride; d.sC1 = (long long)nocc * ldao;
+            RISP_CUDA_TRY(risp_dgemm(d, st)); ++launches;
+            if (!dense) {
+                // U = P + P^T: Z[i][nu in panel] += sum_mu' P[nu][mu'] C_occ[mu'][i]
+                GemmDesc f = gemm_desc(nocc, pr, nao, ctx->d_Cocc, ldocc, false, wD, ldao, true, wY + r0, ldao, 1.0, 1.0);
+                f.nb1 = mj; f.sB1 = mstride; f.sC1 = (long long)nocc * ldao;
+                RISP_CUDA_TRY(risp_dgemm(f, st)); ++launches;
+            }
+        }
+        double *Sb = sigma + (size_t)l0 * nocc * nvir;
+        if (ctx->w_J) {
+            GemmDesc e = gemm_desc(mj * nocc, nvir, nao, wY, ldao, true, ctx->d_Cvir, ldvir, false, ctx->w_J + (size_t)l0 * nocc * nvir, nvir);
+            RISP_CUDA_TRY(risp_dgemm(e, st)); ++launches;
+        }
+        GemmDesc e = gemm_desc(mj * nocc, nvir, nao, wY, ldao, true, ctx->d_Cvir, ldvir, false, Sb, nvir, 2.0, 1.0);
         RISP_CUDA_TRY(risp_dgemm(e, st)); ++launches;
     }
     RISP_CUDA_TRY(cudaEventRecord(ev[5], st));
     // ---------------- K (Eq. 22-23)
     if (ctx->has_K) {
-        RISP_CUDA_TRY(risp_gather_window(X, ctx->w_Xk, m, nocc, nvir, ctx->occK0, no, ctx->virK0, nv, st)); ++launches;
-        RISP_CUDA_TRY(cudaEventRecord(ev[6], st));
-        const int pc = ctx->aux_chunk;
-        for (int p0 = 0; p0 < nK; p0 += pc) {
-            int np = std::min(pc, nK - p0);
-            // M[mi][P][j][a] = sum_b X'[mi][j][b] T_ab^P[a][b]; rows (mi,j) of one P are split by mi
-            GemmDesc d = gemm_desc(m * no, nv, nv, ctx->w_Xk, nv, true, ctx->d_Tab + (long long)p0 * nv * nv, nv, true, ctx->w_M, nv);
-            d.nb1 = np; d.sB1 = (long long)nv * nv; d.sC1 = (long long)no * nv;
-            d.c_rpg = no; d.c_gstride = (long long)np * no * nv;
-            RISP_CUDA_TRY(risp_dgemm(d, st)); ++launches;
-            if (p0 == 0) RISP_CUDA_TRY(cudaEventRecord(ev[9], st));
-            // K'[mi][i][a] (+)= sum_{(P,j)} T_ij[i][(P,j)] M[mi][(P,j)][a]
-            GemmDesc e = gemm_desc(no, nv, np * no, ctx->d_Tij + (long long)p0 * no, (long long)nK * no, true, ctx->w_M, nv, false, ctx->w_Kk, nv,
-                                   1.0, p0 == 0 ? 0.0 : 1.0);
-            e.nb1 = m; e.sB1 = (long long)np * no * nv; e.sC1 = (long long)no * nv;
-            RISP_CUDA_TRY(risp_dgemm(e, st)); ++launches;
-            if (p0 == 0) { RISP_CUDA_TRY(cudaEventRecord(ev[10], st)); ctx->tim.first_chunk_naux = np; }
+        const int pc = pl.pc;
+        double *wXk = ctx->w_arena;                                  // [m][no][nv_p]
+        double *wKk = wXk + (size_t)m * no * nv_p;                   // [m][no][nv_p]
+        double *wM = wKk + (size_t)m * no * nv_p;                    // [m][pc][no_p][nv_p]
+        double *wTab = wM + (size_t)m * pc * no_p * nv_p;            // [pc][nv][nv_p]
+        double *wTij = wTab + (size_t)pc * nv * nv_p;                // [no][pc][no_p]
+        if (nv_p != nv) {   // padding columns of X' must not carry NaNs of the J phase into the TMA boxes (they are never read
+                            // as operands -- K = nv bounds the boxes -- but keep the buffers clean anyway)
+            RISP_CUDA_TRY(cudaMemsetAsync(wXk, 0, (size_t)m * no * nv_p * sizeof(double), st));
         }
+        RISP_CUDA_TRY(risp_gather_window(X, wXk, m, nocc, nvir, ctx->occK0, no, ctx->virK0, nv, nv_p, st)); ++launches;
+        if (no_p != no) {
+            // the contraction index (P, j) of Eq. 23 runs over no_p per P: the padding row of M and the padding column of T_ij are zero
+            RISP_CUDA_TRY(cudaMemset2DAsync(wM + (size_t)no * nv_p, (size_t)no_p * nv_p * 8, 0, (size_t)nv_p * 8, (size_t)m * pc, st));
+            RISP_CUDA_TRY(cudaMemset2DAsync(wTij + no, (size_t)no_p * 8, 0, 8, (size_t)no * pc, st));
+        }
+        RISP_CUDA_TRY(cudaEventRecord(ev[6], st));
+        // chunk list: [p0, p0+np) never straddles the device / host boundary
+        struct Chunk { int p0, np; bool host; };
+        std::vector<Chunk> chunks;
+        for (int p0 = 0; p0 < nK;) {
+            const bool host = p0 >= ctx->nK_dev;
+            const int lim = host ? nK : ctx->nK_dev;
+            const int np = std::min(pc, lim - p0);
+            chunks.push_back({p0, np, host});
+            p0 += np;
+        }
+        const size_t stage_tab_off = (size_t)pc * ctx->tri_o;        // staging buffer: [pc][tri_o] then [pc][tri_v]
+        auto prefetch = [&](int ci, int buf) -> int {
+            const Chunk &c = chunks[ci];
+            const size_t h0 = (size_t)(c.p0 - ctx->nK_dev);
+            RISP_CUDA_TRY(cudaStreamWaitEvent(ctx->side, ctx->evStageFree[buf], 0));
+            RISP_CUDA_TRY(cudaMemcpyAsync(ctx->w_stage[buf], ctx->h_TijP + h0 * ctx->tri_o, (size_t)c.np * ctx->tri_o * 8, cudaMemcpyHostToDevice, ctx->side));
+            RISP_CUDA_TRY(cudaMemcpyAsync(ctx->w_stage[buf] + stage_tab_off, ctx->h_TabP + h0 * ctx->tri_v, (size_t)c.np * ctx->tri_v * 8,
+                                          cudaMemcpyHostToDevice, ctx->side));
+            RISP_CUDA_TRY(cudaEventRecord(ctx->evStage[buf], ctx->side));
+            return RISP_OK;
+        };
+        int first_host = -1;
+        for (size_t i = 0; i < chunks.size(); ++i) if (chunks[i].host) { first_host = (int)i; break; }
+        int nhost_seen = 0, rc;
+        if (first_host >= 0 && (rc = prefetch(first_host, 0))) return rc;
+        for (size_t ci = 0; ci < chunks.size(); ++ci) {
+            const Chunk &c = chunks[ci];
+            const double *pij, *pab;
+            int buf = -1;
+            if (c.host) {
+                buf = nhost_seen & 1;
+                if (ci + 1 < chunks.size() && (rc = prefetch((int)ci + 1, buf ^ 1))) return rc;   // every later chunk is host resident too
+                RISP_CUDA_TRY(cudaStreamWaitEvent(st, ctx->evStage[buf], 0));
+                pij = ctx->w_stage[buf]; pab = ctx->w_stage[buf] + stage_tab_off;
+                ++nhost_seen;
+            } else {
+                pij = ctx->d_TijP + (size_t)c.p0 * ctx->tri_o; pab = ctx->d_TabP + (size_t)c.p0 * ctx->tri_v;
+            }
+            // packed lower triangles -> T_ab [P][a][b] and T_ij [i][(P, j)]
+            RISP_CUDA_TRY(risp_expand_sym(pab, ctx->tri_v, nv, c.np, wTab, nv_p, (long long)nv * nv_p, st)); ++launches;
+            RISP_CUDA_TRY(risp_expand_sym(pij, ctx->tri_o, no, c.np, wTij, (long long)pc * no_p, no_p, st)); ++launches;
+            if (c.host) RISP_CUDA_TRY(cudaEventRecord(ctx->evStageFree[buf], st));
+            if (ci == 0) RISP_CUDA_TRY(cudaEventRecord(ev[11], st));
+            // M[mi][P][j][a] = sum_b X'[mi][j][b] T_ab^P[a][b]; rows (mi,j) of one P are split by mi
+            GemmDesc d = gemm_desc(m * no, nv, nv, wXk, nv_p, true, wTab, nv_p, true, wM, nv_p);
+            d.nb1 = c.np; d.sB1 = (long long)nv * nv_p; d.sC1 = (long long)no_p * nv_p;
+            d.c_rpg = no; d.c_gstride = (long long)pc * no_p * nv_p;
+            RISP_CUDA_TRY(risp_dgemm(d, st)); ++launches;
+            if (ci == 0) RISP_CUDA_TRY(cudaEventRecord(ev[9], st));
+            // K'[mi][i][a] (+)= sum_{(P,j)} T_ij[i][(P,j)] M[mi][(P,j)][a]
+            GemmDesc e = gemm_desc(no, nv, c.np * no_p, wTij, (long long)pc * no_p, true, wM, nv_p, false, wKk, nv_p, 1.0, ci == 0 ? 0.0 : 1.0);
+            e.nb1 = m; e.sB1 = (long long)pc * no_p * nv_p; e.sC1 = (long long)no * nv_p;
+            RISP_CUDA_TRY(risp_dgemm(e, st)); ++launches;
+            if (ci == 0) { RISP_CUDA_TRY(cudaEventRecord(ev[10], st)); ctx->tim.first_chunk_naux = c.np; }
+        }
+        RISP_CUDA_TRY(cudaEventRecord(ev[7], st));
+        RISP_CUDA_TRY(risp_sub_window(wKk, sigma, m, nocc, nvir, ctx->occK0, no, ctx->virK0, nv, nv_p, st)); ++launches;
     } else {
         RISP_CUDA_TRY(cudaEventRecord(ev[6], st));
+        RISP_CUDA_TRY(cudaEventRecord(ev[7], st));
     }
-    RISP_CUDA_TRY(cudaEventRecord(ev[7], st));
-    // ---------------- sigma (Eq. 10)
-    RISP_CUDA_TRY(risp_assemble_sigma(X, ctx->w_J, ctx->w_Kk, ctx->d_eps, sigma, m, nocc, nvir, ctx->occK0, no, ctx->virK0, nv, ctx->has_K ? 1 : 0, st));
-    ++launches;
     RISP_CUDA_TRY(cudaEventRecord(ev[8], st));
     ctx->tim.kernel_launches = launches;
     ctx->last_m = m;
@@ -158,18 +336,32 @@ extern "C" int risp_matvec_host(risp_ctx *ctx, int32_t m, const double *X_host, 
     if (!ctx) return RISP_EINVAL;
     if (m <= 0 || m > RISP_MS || !X_host || !sigma_host) { risp_set_error(ctx, "risp_matvec_host: need 1 <= m <= 32 and non-NULL host pointers"); return RISP_EINVAL; }
     RISP_CUDA_TRY(cudaSetDevice(ctx->device));
+    const size_t bytes = (size_t)m * ctx->nocc * ctx->nvir * sizeof(double);
+    if (m > ctx->xin_cap) {
+        // the staging copies of X and sigma are the caller's share of HBM in this entry point: allocate them before the work space is planned
+        risp_free_workspace(ctx);
+        if (ctx->w_Xin) { cudaFree(ctx->w_Xin); cudaFree(ctx->w_Sout); ctx->w_Xin = ctx->w_Sout = nullptr; ctx->xin_cap = 0; }
+        RISP_CUDA_TRY(cudaMalloc((void **)&ctx->w_Xin, bytes));
+        RISP_CUDA_TRY(cudaMalloc((void **)&ctx->w_Sout, bytes));
+        ctx->xin_cap = m;
+    }
     int rc = risp_ensure_workspace(ctx, m);
     if (rc) return rc;
-    size_t n = (size_t)ctx->m_cap * ctx->nocc * ctx->nvir, bytes = (size_t)m * ctx->nocc * ctx->nvir * sizeof(double);
-    if (!ctx->w_Xin) {
-        RISP_CUDA_TRY(cudaMalloc((void **)&ctx->w_Xin, n * sizeof(double)));
-        RISP_CUDA_TRY(cudaMalloc((void **)&ctx->w_Sout, n * sizeof(double)));
-        ctx->w_bytes += 2 * n * sizeof(double);
-    }
     RISP_CUDA_TRY(cudaMemcpyAsync(ctx->w_Xin, X_host, bytes, cudaMemcpyHostToDevice, 0));
     rc = risp_matvec_impl(ctx, m, ctx->w_Xin, ctx->w_Sout, 0);
     if (rc) return rc;
     RISP_CUDA_TRY(cudaMemcpyAsync(sigma_host, ctx->w_Sout, bytes, cudaMemcpyDeviceToHost, 0));
     RISP_CUDA_TRY(cudaStreamSynchronize(0));
+    return RISP_OK;
+}
+
+// Testing: override the work-space plan of the next risp_matvec (0 = automatic).
+extern "C" int risp_debug_force_plan(risp_ctx *ctx, int mj, int prow, int pc)
+{
+    if (!ctx) return RISP_EINVAL;
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+    risp_free_workspace(ctx);
+    ctx->force_mj = mj; ctx->force_prow = prow; ctx->force_pc = pc;
     return RISP_OK;
 }

@@ -271,13 +271,26 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
     }
 
     // ---------------------------------------------------------------- device constants
+    ctx->flags = opt.flags;
+    ctx->max_batch = opt.max_batch > 0 ? std::min(opt.max_batch, RISP_MS) : RISP_MS;
+    auto even = [](int n) { return (n + 1) & ~1; };
+    ctx->ldao = even(ctx->nao); ctx->ldocc = even(ctx->nocc); ctx->ldvir = even(ctx->nvir);
+    ctx->no_p = even(ctx->noccK); ctx->nv_p = even(ctx->nvirK);
     {
         std::vector<double> tab = make_boys_table();
         int rc;
         if ((rc = upload(ctx, ctx->d_boys, tab.data(), tab.size()))) return rc;
-        if ((rc = upload(ctx, ctx->d_C, sys->C, (size_t)ctx->nao * ctx->nmo))) return rc;
+        // C split into its occupied and virtual column blocks, each with an even leading dimension (16-byte TMA strides)
+        std::vector<double> co((size_t)ctx->nao * ctx->ldocc, 0.0), cv((size_t)ctx->nao * ctx->ldvir, 0.0);
+        for (int mu = 0; mu < ctx->nao; ++mu) {
+            std::memcpy(&co[(size_t)mu * ctx->ldocc], sys->C + (size_t)mu * ctx->nmo, (size_t)ctx->nocc * sizeof(double));
+            std::memcpy(&cv[(size_t)mu * ctx->ldvir], sys->C + (size_t)mu * ctx->nmo + ctx->nocc, (size_t)ctx->nvir * sizeof(double));
+        }
+        if ((rc = upload(ctx, ctx->d_Cocc, co.data(), co.size()))) return rc;
+        if ((rc = upload(ctx, ctx->d_Cvir, cv.data(), cv.size()))) return rc;
         if ((rc = upload(ctx, ctx->d_eps, sys->eps, (size_t)ctx->nmo))) return rc;
     }
+    for (int s = 0; s < sys->nshl; ++s) if ((ctx->h_shl_ao[s] & 1) == 0) ctx->h_even_shell_ao.push_back(ctx->h_shl_ao[s]);
     std::vector<AuxCentre> cenJ, cenK;
     build_centres(ctx, ctx->h_aux_fn, cenJ);
     build_centres(ctx, ctx->h_aux_fnK, cenK);
@@ -316,7 +329,11 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
         static const int LA[6] = {0, 1, 1, 2, 2, 2}, LB[6] = {0, 0, 1, 0, 1, 2};
         for (int c = 0; c < 6; ++c) {
             PairClass &pc = ctx->cls[c];
+            // sorted by the first AO of shell A: a panel of AO rows of D / U is then a contiguous pair range
+            std::stable_sort(pairs[c].begin(), pairs[c].end(), [](const ShellPair &x, const ShellPair &y) { return x.aoA < y.aoA; });
             pc.la = LA[c]; pc.lb = LB[c]; pc.npairs = (int)pairs[c].size();
+            pc.h_aoA.resize(pc.npairs);
+            for (int k = 0; k < pc.npairs; ++k) pc.h_aoA[k] = pairs[c][k].aoA;
             pc.e_off = e_off; e_off += (long long)pc.npairs * ne_of(pc.la, pc.lb);
             pc.chunk = chunk; pc.nchunks = (pc.npairs + chunk - 1) / chunk; pc.chunk_base = chunk_base; chunk_base += pc.nchunks;
             int rc;
@@ -363,80 +380,141 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
     }
 
     // ---------------------------------------------------------------- budgets
-    {
-        size_t free_b = 0, total_b = 0;
-        RISP_CUDA_TRY(cudaMemGetInfo(&free_b, &total_b));
-        ctx->hbm_budget = opt.hbm_budget_bytes ? opt.hbm_budget_bytes : (size_t)(0.85 * (double)free_b);
-        ctx->host_budget = opt.host_budget_bytes ? opt.host_budget_bytes : ((size_t)8 << 30);
-    }
+    size_t free_b = 0, total_b = 0;
+    RISP_CUDA_TRY(cudaMemGetInfo(&free_b, &total_b));
+    ctx->hbm_budget = opt.hbm_budget_bytes ? opt.hbm_budget_bytes : (size_t)(0.85 * (double)free_b) + ctx->setup_bytes;
+    ctx->host_budget = opt.host_budget_bytes ? opt.host_budget_bytes : ((size_t)8 << 30);
 
-    // ---------------------------------------------------------------- a3: K tensors
+    // ---------------------------------------------------------------- a3: K tensors, packed lower triangles (Eq. 20-21)
     if (ctx->has_K) {
         int rc;
-        const int nao = ctx->nao, no = ctx->noccK, nv = ctx->nvirK, nK = ctx->nauxK, nmo = ctx->nmo;
-        size_t bytes_T = ((size_t)nK * no * no + (size_t)nK * nv * nv) * sizeof(double);
-        if (bytes_T > ctx->hbm_budget) { risp_set_error(ctx, "risp_setup: K tensors exceed the HBM budget (host spill not built yet)"); return RISP_ENOMEM; }
-        if ((rc = dalloc(ctx, ctx->d_Tij, (size_t)nK * no * no))) return rc;
-        if ((rc = dalloc(ctx, ctx->d_Tab, (size_t)nK * nv * nv))) return rc;
-        double *Bij = nullptr;
-        RISP_CUDA_TRY(cudaMalloc((void **)&Bij, (size_t)nK * no * no * sizeof(double)));
-        // chunk of K centres: G[Pc][nao][nao] + H[Pc][nao][max(no,nv)] within ~2 GiB
-        size_t per_fn = ((size_t)nao * nao + (size_t)nao * std::max(no, nv)) * sizeof(double);
-        int max_fn = (int)std::max<size_t>(4, std::min<size_t>((size_t)nK, ((size_t)2 << 30) / per_fn));
-        double *G = nullptr, *H = nullptr;
-        RISP_CUDA_TRY(cudaMalloc((void **)&G, (size_t)max_fn * nao * nao * sizeof(double)));
-        RISP_CUDA_TRY(cudaMalloc((void **)&H, (size_t)max_fn * nao * std::max(no, nv) * sizeof(double)));
-        OpParams opK{sys->alpha, sys->beta, sys->omega * sys->omega};
+        const int nao = ctx->nao, no = ctx->noccK, nv = ctx->nvirK, nK = ctx->nauxK, no_p = ctx->no_p, nv_p = ctx->nv_p;
+        const long long ldao = ctx->ldao;
+        ctx->tri_o = (long long)no * (no + 1) / 2; ctx->tri_v = (long long)nv * (nv + 1) / 2;
+        const long long tri_o = ctx->tri_o, tri_v = ctx->tri_v;
+        // ---- placement: what the budget leaves after the work space of a max_batch matvec (and, with the default budget, the
+        //      caller's X and sigma) holds the first nK_dev slices; the others go to pinned host memory
+        {
+            const size_t slice = (size_t)(tri_o + tri_v) * 8;
+            const size_t dimb = (size_t)ctx->nocc * ctx->nvir * 8;
+            size_t reserve = ((size_t)ctx->e_rows * RISP_MS + (size_t)ctx->total_chunks * ctx->ncenJ_pad * 4 * RISP_MS + 3 * (size_t)ctx->nauxJ * RISP_MS) * 8;
+            if (!opt.hbm_budget_bytes) reserve += 2 * (size_t)ctx->max_batch * dimb;
+            if (ctx->flags & RISP_FLAG_KEEP_STAGES) reserve += (size_t)ctx->max_batch * dimb;
+            size_t left = ctx->hbm_budget > ctx->setup_bytes + reserve ? ctx->hbm_budget - ctx->setup_bytes - reserve : 0;
+            // work space if everything had to be streamed (upper bound of the staging need), then the slices
+            MatvecPlan tmp;
+            ctx->nK_dev = 0;
+            size_t ws = risp_plan_workspace(ctx, ctx->max_batch, left, tmp, true);
+            if (ws == 0) { risp_set_error(ctx, "risp_setup: the HBM budget is too small for the matvec work space"); return RISP_ENOMEM; }
+            left -= std::min(left, ws);
+            ctx->nK_dev = (int)std::min<size_t>((size_t)nK, left / slice);
+            if (ctx->flags & RISP_FLAG_SPILL_HALF) ctx->nK_dev = std::min(ctx->nK_dev, nK / 2);
+        }
+        const int nK_host = nK - ctx->nK_dev;
+        // ---- scratch for a chunk of aux functions: G[f][nao][ldao], H[f][nao][max(no_p,nv_p)], full B / T[f][n][n_p], packed
+        const size_t nmax_p = (size_t)std::max(no_p, nv_p), sq = std::max((size_t)no * no_p, (size_t)nv * nv_p);
+        const size_t per_fn = ((size_t)nao * ldao + (size_t)nao * nmax_p + sq + (size_t)std::max(tri_o, tri_v)) * sizeof(double);
         bool haspK = false;
         for (auto &c : cenK) if (c.qp >= 0) haspK = true;
-        int c0 = 0;
-        while (c0 < ctx->ncenK) {
-            // centres are created in function order, so a run of centres covers a contiguous function range only if
-            // each centre's functions are contiguous; take function range [f0, f1)
-            int c1 = c0, f0 = 1 << 30, f1 = -1;
-            while (c1 < ctx->ncenK) {
-                int lo = 1 << 30, hi = -1;
-                if (cenK[c1].qs >= 0) { lo = std::min(lo, cenK[c1].qs); hi = std::max(hi, cenK[c1].qs + 1); }
-                if (cenK[c1].qp >= 0) { lo = std::min(lo, cenK[c1].qp); hi = std::max(hi, cenK[c1].qp + 3); }
-                int nf0 = std::min(f0, lo), nf1 = std::max(f1, hi);
-                if (c1 > c0 && nf1 - nf0 > max_fn) break;
-                f0 = nf0; f1 = nf1; ++c1;
-            }
-            int nf = f1 - f0;
-            if (nf > max_fn) { risp_set_error(ctx, "risp_setup: K aux functions of one centre are not contiguous"); return RISP_EINVAL; }
-            RISP_CUDA_TRY(cudaMemsetAsync(G, 0, (size_t)nf * nao * nao * sizeof(double), 0));
-            for (int c = 0; c < 6; ++c) {
-                const PairClass &pc = ctx->cls[c];
-                RISP_CUDA_TRY(risp_eri_fill(pc.la, pc.lb, haspK, true, pc.d_pairs, pc.npairs, ctx->d_prims, ctx->d_cenK + c0, c1 - c0, opK, ctx->d_boys,
-                                            G - (long long)f0 * nao * nao, (long long)nao * nao, nao, 1, 0));
-            }
-            // occupied window: H[P] = G[P] C_o' ; B_ij[P] = C_o'^T H[P]
-            GemmDesc d1 = gemm_desc(nao, no, nao, G, nao, true, ctx->d_C + ctx->occK0, nmo, false, H, no);
-            d1.nb1 = nf; d1.sA1 = (long long)nao * nao; d1.sC1 = (long long)nao * no;
-            RISP_CUDA_TRY(risp_dgemm(d1, 0));
-            GemmDesc d2 = gemm_desc(no, no, nao, ctx->d_C + ctx->occK0, nmo, false, H, no, false, Bij + (long long)f0 * no * no, no);
-            d2.nb1 = nf; d2.sB1 = (long long)nao * no; d2.sC1 = (long long)no * no;
-            RISP_CUDA_TRY(risp_dgemm(d2, 0));
-            // virtual window: T_ab^P = C_v'^T G[P] C_v'   (Eq. 21)
-            const double *Cv = ctx->d_C + ctx->nocc + ctx->virK0;
-            GemmDesc d3 = gemm_desc(nao, nv, nao, G, nao, true, Cv, nmo, false, H, nv);
-            d3.nb1 = nf; d3.sA1 = (long long)nao * nao; d3.sC1 = (long long)nao * nv;
-            RISP_CUDA_TRY(risp_dgemm(d3, 0));
-            GemmDesc d4 = gemm_desc(nv, nv, nao, Cv, nmo, false, H, nv, false, ctx->d_Tab + (long long)f0 * nv * nv, nv);
-            d4.nb1 = nf; d4.sB1 = (long long)nao * nv; d4.sC1 = (long long)nv * nv;
-            RISP_CUDA_TRY(risp_dgemm(d4, 0));
-            c0 = c1;
+        const int max_fn = (int)std::max<size_t>(haspK ? 4 : 1, std::min<size_t>((size_t)nK, ((size_t)3 << 30) / per_fn));
+        double *G = nullptr, *H = nullptr, *F = nullptr, *Pk = nullptr, *CoK = nullptr, *CvK = nullptr, *BP = nullptr;
+        RISP_CUDA_TRY(cudaMalloc((void **)&G, (size_t)max_fn * nao * ldao * sizeof(double)));
+        RISP_CUDA_TRY(cudaMalloc((void **)&H, (size_t)max_fn * nao * nmax_p * sizeof(double)));
+        RISP_CUDA_TRY(cudaMalloc((void **)&F, (size_t)max_fn * sq * sizeof(double)));
+        RISP_CUDA_TRY(cudaMalloc((void **)&Pk, (size_t)max_fn * std::max(tri_o, tri_v) * sizeof(double)));
+        // window blocks of C with even leading dimensions and aligned bases
+        RISP_CUDA_TRY(cudaMalloc((void **)&CoK, (size_t)nao * no_p * sizeof(double)));
+        RISP_CUDA_TRY(cudaMalloc((void **)&CvK, (size_t)nao * nv_p * sizeof(double)));
+        RISP_CUDA_TRY(cudaMemset(CoK, 0, (size_t)nao * no_p * sizeof(double)));
+        RISP_CUDA_TRY(cudaMemset(CvK, 0, (size_t)nao * nv_p * sizeof(double)));
+        RISP_CUDA_TRY(cudaMemcpy2D(CoK, (size_t)no_p * 8, ctx->d_Cocc + ctx->occK0, (size_t)ctx->ldocc * 8, (size_t)no * 8, nao, cudaMemcpyDeviceToDevice));
+        RISP_CUDA_TRY(cudaMemcpy2D(CvK, (size_t)nv_p * 8, ctx->d_Cvir + ctx->virK0, (size_t)ctx->ldvir * 8, (size_t)nv * 8, nao, cudaMemcpyDeviceToDevice));
+        // all (ij|Q) slices, packed, in HBM until the metric has been applied (Eq. 20 mixes every Q)
+        RISP_CUDA_TRY(cudaMalloc((void **)&BP, (size_t)nK * tri_o * sizeof(double)));
+        if (nK_host > 0) {
+            RISP_CUDA_TRY(cudaHostAlloc((void **)&ctx->h_TijP, (size_t)nK_host * tri_o * sizeof(double), cudaHostAllocDefault));
+            RISP_CUDA_TRY(cudaHostAlloc((void **)&ctx->h_TabP, (size_t)nK_host * tri_v * sizeof(double), cudaHostAllocDefault));
         }
-        // T_ij^P = sum_Q (P|Q)^-1 B_ij^Q   (Eq. 20), stored Tij[i][P][j]
-        GemmDesc d5 = gemm_desc(nK, no, nK, ctx->d_MKinv, nK, true, Bij, (long long)no * no, false, ctx->d_Tij, no);
-        d5.nb1 = no; d5.sB1 = no; d5.sC1 = (long long)nK * no;
-        RISP_CUDA_TRY(risp_dgemm(d5, 0));
+        if (ctx->nK_dev > 0) { if ((rc = dalloc(ctx, ctx->d_TabP, (size_t)ctx->nK_dev * tri_v))) return rc; }
+        OpParams opK{sys->alpha, sys->beta, sys->omega * sys->omega};
+        for (int pass = 0; pass < 2; ++pass) {          // pass 0: occupied window -> BP ; pass 1: virtual window -> T_ab
+            const int n = pass == 0 ? no : nv, n_p = pass == 0 ? no_p : nv_p;
+            const long long tri = pass == 0 ? tri_o : tri_v;
+            const double *Cw = pass == 0 ? CoK : CvK;
+            int c0 = 0;
+            while (c0 < ctx->ncenK) {
+                // centres are created in function order: a run of centres covers the contiguous function range [f0, f1)
+                int c1 = c0, f0 = 1 << 30, f1 = -1;
+                while (c1 < ctx->ncenK) {
+                    int lo = 1 << 30, hi = -1;
+                    if (cenK[c1].qs >= 0) { lo = std::min(lo, cenK[c1].qs); hi = std::max(hi, cenK[c1].qs + 1); }
+                    if (cenK[c1].qp >= 0) { lo = std::min(lo, cenK[c1].qp); hi = std::max(hi, cenK[c1].qp + 3); }
+                    int nf0 = std::min(f0, lo), nf1 = std::max(f1, hi);
+                    if (c1 > c0 && nf1 - nf0 > max_fn) break;
+                    f0 = nf0; f1 = nf1; ++c1;
+                }
+                const int nf = f1 - f0;
+                if (nf > max_fn) { risp_set_error(ctx, "risp_setup: K aux functions of one centre are not contiguous"); return RISP_EINVAL; }
+                RISP_CUDA_TRY(cudaMemsetAsync(G, 0, (size_t)nf * nao * ldao * sizeof(double), 0));
+                for (int c = 0; c < 6; ++c) {
+                    const PairClass &pc = ctx->cls[c];
+                    RISP_CUDA_TRY(risp_eri_fill(pc.la, pc.lb, haspK, true, pc.d_pairs, pc.npairs, ctx->d_prims, ctx->d_cenK + c0, c1 - c0, opK, ctx->d_boys,
+                                                G - (long long)f0 * nao * ldao, (long long)nao * ldao, ldao, 1, 0));
+                }
+                // H[P] = (mu nu|P) C_w ; F[P] = C_w^T H[P]      (Eq. 20-21 before the metric)
+                GemmDesc d1 = gemm_desc(nao, n, nao, G, ldao, true, Cw, n_p, false, H, n_p);
+                d1.nb1 = nf; d1.sA1 = (long long)nao * ldao; d1.sC1 = (long long)nao * n_p;
+                RISP_CUDA_TRY(risp_dgemm(d1, 0));
+                GemmDesc d2 = gemm_desc(n, n, nao, Cw, n_p, false, H, n_p, false, F, n_p);
+                d2.nb1 = nf; d2.sB1 = (long long)nao * n_p; d2.sC1 = (long long)n * n_p;
+                RISP_CUDA_TRY(risp_dgemm(d2, 0));
+                if (pass == 0) {
+                    RISP_CUDA_TRY(risp_pack_sym(F, (long long)n * n_p, n_p, n, nf, BP + (size_t)f0 * tri, tri, 0));
+                } else {
+                    RISP_CUDA_TRY(risp_pack_sym(F, (long long)n * n_p, n_p, n, nf, Pk, tri, 0));
+                    for (int f = f0; f < f1; ++f) {
+                        const double *src = Pk + (size_t)(f - f0) * tri;
+                        if (f < ctx->nK_dev) RISP_CUDA_TRY(cudaMemcpyAsync(ctx->d_TabP + (size_t)f * tri, src, (size_t)tri * 8, cudaMemcpyDeviceToDevice, 0));
+                        else RISP_CUDA_TRY(cudaMemcpyAsync(ctx->h_TabP + (size_t)(f - ctx->nK_dev) * tri, src, (size_t)tri * 8, cudaMemcpyDeviceToHost, 0));
+                    }
+                    RISP_CUDA_TRY(cudaStreamSynchronize(0));
+                }
+                c0 = c1;
+            }
+            if (pass == 0) {
+                // T_ij^P = sum_Q (P|Q)^-1 (ij|Q)   (Eq. 20): BP <- MKinv BP, in column panels, in place
+                long long w = std::min<long long>(tri_o, std::max<long long>(2, (((long long)1 << 30) / ((long long)nK * 8)) & ~1LL));
+                double *tmpc = nullptr;
+                RISP_CUDA_TRY(cudaMalloc((void **)&tmpc, (size_t)nK * w * sizeof(double)));
+                for (long long col = 0; col < tri_o; col += w) {
+                    const int wc = (int)std::min<long long>(w, tri_o - col);
+                    GemmDesc d5 = gemm_desc(nK, wc, nK, ctx->d_MKinv, nK, true, BP + col, tri_o, false, tmpc, w);
+                    RISP_CUDA_TRY(risp_dgemm(d5, 0));
+                    RISP_CUDA_TRY(cudaMemcpy2DAsync(BP + col, (size_t)tri_o * 8, tmpc, (size_t)w * 8, (size_t)wc * 8, nK, cudaMemcpyDeviceToDevice, 0));
+                }
+                RISP_CUDA_TRY(cudaDeviceSynchronize());
+                cudaFree(tmpc);
+                if (nK_host == 0) { ctx->d_TijP = BP; BP = nullptr; ctx->setup_bytes += (size_t)nK * tri_o * 8; }
+                else {
+                    RISP_CUDA_TRY(cudaMemcpy(ctx->h_TijP, BP + (size_t)ctx->nK_dev * tri_o, (size_t)nK_host * tri_o * 8, cudaMemcpyDeviceToHost));
+                    if (ctx->nK_dev > 0) {
+                        if ((rc = dalloc(ctx, ctx->d_TijP, (size_t)ctx->nK_dev * tri_o))) return rc;
+                        RISP_CUDA_TRY(cudaMemcpy(ctx->d_TijP, BP, (size_t)ctx->nK_dev * tri_o * 8, cudaMemcpyDeviceToDevice));
+                    }
+                    cudaFree(BP); BP = nullptr;
+                }
+            }
+        }
         RISP_CUDA_TRY(cudaDeviceSynchronize());
-        cudaFree(G); cudaFree(H); cudaFree(Bij);
+        cudaFree(G); cudaFree(H); cudaFree(F); cudaFree(Pk); cudaFree(CoK); cudaFree(CvK);
     }
     RISP_CUDA_TRY(cudaDeviceSynchronize());
     RISP_CUDA_TRY(cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking));
-    for (int i = 0; i < 12; ++i) RISP_CUDA_TRY(cudaEventCreate(&ctx->ev[i]));
+    for (int i = 0; i < RISP_NEV; ++i) RISP_CUDA_TRY(cudaEventCreate(&ctx->ev[i]));
+    for (int b = 0; b < 2; ++b) {
+        RISP_CUDA_TRY(cudaEventCreateWithFlags(&ctx->evStage[b], cudaEventDisableTiming));
+        RISP_CUDA_TRY(cudaEventCreateWithFlags(&ctx->evStageFree[b], cudaEventDisableTiming));
+    }
     ctx->ev_ok = true;
     std::memset(&ctx->tim, 0, sizeof(ctx->tim));
     return RISP_OK;

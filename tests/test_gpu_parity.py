@@ -61,7 +61,7 @@ def test_dgemm_batched(torch_cuda):
 @pytest.fixture(scope="module")
 def ctx1(torch_cuda, sys1):
     from paper_2603_29257_b200 import setup
-    c = setup(sys1)
+    c = setup(sys1, flags=1)              # RISP_FLAG_KEEP_STAGES: J_mia stays available to the getter
     yield c
     c.close()
 
@@ -69,7 +69,7 @@ def ctx1(torch_cuda, sys1):
 @pytest.fixture(scope="module")
 def ctx_rsh(torch_cuda, sys_small_rsh):
     from paper_2603_29257_b200 import setup
-    c = setup(sys_small_rsh)
+    c = setup(sys_small_rsh, flags=1)
     yield c
     c.close()
 
@@ -205,6 +205,92 @@ def test_no_truncation_and_empty_window(torch_cuda, sys_small_rsh):
         c.close()
 
 
+# ------------------------------------------------------------------------------------------------ memory plans
+@pytest.mark.parametrize("plan", [dict(mj=2, prow=0, pc=0), dict(mj=0, prow=40, pc=1), dict(mj=3, prow=24, pc=2), dict(mj=1, prow=1, pc=5)])
+@pytest.mark.parametrize("which", ["tiny", "rsh"])
+def test_sub_batched_and_panelled_plans(which, plan, torch_cuda, sys1, ctx1, oracle1, sys_small_rsh, ctx_rsh, oracle_small_rsh):
+    """The large-system layouts on a small system: J transforms in trial-vector sub-batches and AO row panels (D + D^T per
+    panel, U = P + P^T), K in small aux chunks.  Every plan must reproduce the oracle, term by term."""
+    torch = torch_cuda
+    from workloads import trial_vectors
+    s, ctx, o = (sys1, ctx1, oracle1) if which == "tiny" else (sys_small_rsh, ctx_rsh, oracle_small_rsh)
+    m = 5
+    X = trial_vectors(s, m)
+    sig_ref, dg, J_ref, K_ref = o.sigma(X, parts=True)
+    try:
+        ctx.force_plan(**plan)
+        sig = ctx.matvec(torch.from_numpy(X).cuda()).cpu().numpy()
+        d = ctx.dims()
+        if plan["mj"]:
+            assert d["j_sub_batch"] == plan["mj"]
+        if plan["prow"]:
+            assert d["j_panels"] > 1
+        if plan["pc"]:
+            assert d["aux_chunk"] == min(plan["pc"], d["nauxK"])
+        assert _rel(ctx.stage("J", m), J_ref) <= 1e-10
+        assert _rel(ctx.stage("K", m), K_ref) <= 1e-10
+        assert _rel(sig, sig_ref) <= 1e-10
+    finally:
+        ctx.force_plan(0, 0, 0)
+
+
+@pytest.mark.parametrize("pc", [0, 1, 2])
+def test_host_spilled_K_tensors(pc, torch_cuda, sys_small_rsh, oracle_small_rsh):
+    """Half of the K-tensor slices in pinned host memory, streamed through the side stream: same sigma, same
+    slices, and the Davidson roots are unchanged."""
+    torch = torch_cuda
+    from paper_2603_29257_b200 import setup
+    from workloads import trial_vectors
+    o = oracle_small_rsh
+    c = setup(sys_small_rsh, flags=1 | 2)             # KEEP_STAGES | SPILL_HALF
+    try:
+        c.force_plan(0, 0, pc)
+        m = 4
+        X = trial_vectors(sys_small_rsh, m)
+        sig_ref, dg, J_ref, K_ref = o.sigma(X, parts=True)
+        Xd = torch.from_numpy(X).cuda()
+        for _ in range(3):                              # repeated calls reuse the two staging buffers
+            sig = c.matvec(Xd).cpu().numpy()
+        d = c.dims()
+        assert 0 < d["nauxK_device"] < d["nauxK"] and d["bytes_T_host"] > 0
+        assert _rel(c.stage("K", m), K_ref) <= 1e-10
+        assert _rel(sig, sig_ref) <= 1e-10
+        sel = [0, d["nauxK_device"] - 1, d["nauxK_device"], d["nauxK"] - 1]
+        assert _rel(c.stage("TAB", sel=sel), o.Bab[sel]) <= 1e-12
+        Tij_ref = np.einsum('qij,qp->pij', o.Bij, np.linalg.inv(o.MK))[sel]
+        assert _rel(c.stage("TIJ", sel=sel), Tij_ref) <= 1e-10
+        if pc == 0:
+            w_ref = np.linalg.eigvalsh(o.full_A())[:3]
+            omega, _, info = c.tda_solve(3, tol=1e-8)
+            assert info["converged"] == 1 and np.abs(omega - w_ref).max() * HARTREE_EV <= 1e-6
+    finally:
+        c.close()
+
+
+def test_small_hbm_budget_spills_and_panels(torch_cuda, sys_small_rsh, oracle_small_rsh):
+    """An explicit tiny HBM budget makes the planner itself choose host spill, sub-batches and panels."""
+    torch = torch_cuda
+    from paper_2603_29257_b200 import setup
+    from workloads import trial_vectors
+    o = oracle_small_rsh
+    m = 6
+    X = trial_vectors(sys_small_rsh, m)
+    ref = o.sigma(X)
+    big = setup(sys_small_rsh, max_batch=m)
+    big.matvec(torch.from_numpy(X).cuda())
+    d = big.dims()
+    need = d["bytes_device_total"] - (d["bytes_Tij"] + d["bytes_Tab"]) // 2     # room for about half of the slices
+    big.close()
+    c = setup(sys_small_rsh, hbm_budget_bytes=int(need), max_batch=m)
+    try:
+        sig = c.matvec(torch.from_numpy(X).cuda()).cpu().numpy()
+        d = c.dims()
+        assert d["nauxK_device"] < d["nauxK"], d
+        assert _rel(sig, ref) <= 1e-10
+    finally:
+        c.close()
+
+
 # ------------------------------------------------------------------------------------------------ screening
 def test_screened_pairs_are_negligible(ctx1, oracle1, torch_cuda, sys_small_rsh, oracle_small_rsh, ctx_rsh):
     for ctx, o in ((ctx1, oracle1), (ctx_rsh, oracle_small_rsh)):
@@ -248,7 +334,7 @@ def cfg2(torch_cuda):
     s = make_system(2)
     o = Oracle(s)
     o.build()
-    c = setup(s)
+    c = setup(s, flags=1)
     yield s, o, c
     c.close()
 
