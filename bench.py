@@ -133,9 +133,8 @@ def main():
     # every rank gets its own seeded batch of m trial vectors (weak scaling over trial vectors, no collective)
     X_h = trial_vectors(s, base_seed=260329257 + 17 * rank)
     t0 = time.time()
-    ctx = setup(s, device=local)
+    ctx = setup(s, device=local, max_batch=m)
     t_setup = time.time() - t0
-    d = ctx.dims()
     X = torch.from_numpy(X_h).to(dev)
     sigma = torch.empty_like(X)
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
@@ -167,6 +166,7 @@ def main():
     clocks = sampler.stop(tw0, tw1) if sampler else None
     t_dev = sum(a.elapsed_time(b) for a, b in evs) * 1e-3
     tim = ctx.timings()
+    d = ctx.dims()
     launches = tim["kernel_launches"] * args.steps
 
     # ---- end to end: pinned host buffers through risp_matvec_host
@@ -208,13 +208,15 @@ def main():
             config=dict(workload=s["name"], m=m, atoms=int(s["natm"]), nao=s["nao"], nocc=s["nocc"], nvir=s["nvir"], nauxJ=d["nauxJ"], nauxK=nK,
                         noccK=no, nvirK=nv, shell_pairs_kept=d["n_shell_pairs_kept"], shell_pairs=d["n_shell_pairs"],
                         ao_pair_survival=round(2.0 * d["n_ao_pairs_kept"] / (s["nao"] * (s["nao"] + 1)), 4),
-                        K_tensors="HBM", bytes_T=d["bytes_Tij"] + d["bytes_Tab"], aux_chunk=d["aux_chunk"], l2="flushed between steps (512 MiB write)",
+                        K_tensors=f"packed lower triangles; {d['nauxK_device']} of {nK} aux slices in HBM, {d['bytes_T_host']} B in pinned host memory",
+                        bytes_T=d["bytes_Tij"] + d["bytes_Tab"], aux_chunk=d["aux_chunk"], j_sub_batch=d["j_sub_batch"], j_panels=d["j_panels"],
+                        l2="flushed between steps (512 MiB write)",
                         parallelism=f"trial-vector shards x{world}", setup_s=round(t_setup, 3)),
             clocks=clocks,
             e2e=dict(value=world * m * args.steps / t_e2e, unit=UNIT, h2d_bytes_per_step=int(X_h.nbytes), d2h_bytes_per_step=int(X_h.nbytes),
                      bitwise_equal_to_device_path=same),
             gpu_launches=launches,
-            roofline=dict(bound="tensor", kernel="dgemm_kernel<KC,KC> (K contraction M^P = X' T_ab^P, Eq. 22)", achieved=achieved, peak=peak,
+            roofline=dict(bound="tensor", kernel="dgemm_tma_kernel<KC,KC,MI> (K contraction M^P = X' T_ab^P, Eq. 22)", achieved=achieved, peak=peak,
                           unit="TFLOP/s", frac=achieved / peak, traffic=traffic,
                           peak_source=f"{pk['src']} bf16 burst {pk['bf16']} TFLOP/s x nominal FP64:bf16 ratio 45/2250",
                           flops_per_launch=flops_launch, launch_ms=1e3 * t_launch),

@@ -93,8 +93,11 @@ typedef struct {
     int32_t max_iter;           /* 0 -> 100 */
     int32_t n_guess;            /* initial unit vectors on the smallest e_a - e_i (0 -> 2*nroots) */
     int32_t max_sub;            /* restart when the subspace would exceed this (0 -> 20*nroots) */
-    int32_t flags;              /* reserved, 0 */
+    int32_t flags;              /* RISP_SOLVE_* */
 } risp_solve_options;
+
+#define RISP_SOLVE_NO_CACHE 1     /* every pass over V, W streams from pinned host memory (no device cache) */
+#define RISP_SOLVE_TINY_CACHE 2   /* testing: cache only nroots + 2 vectors, the rest is streamed */
 
 #define RISP_MAX_ROOTS 64
 typedef struct {
@@ -103,6 +106,7 @@ typedef struct {
     double sec_total, sec_matvec, sec_subspace; /* wall seconds */
     double bytes_h2d, bytes_d2h;         /* subspace traffic over the host link */
     int32_t subspace_max;                /* largest subspace held */
+    int32_t cached_vectors;              /* leading vectors of V and of W kept in HBM as well */
 } risp_solve_info;
 
 typedef struct {

@@ -48,7 +48,7 @@ class _SolveOptions(C.Structure):
 class _SolveInfo(C.Structure):
     _fields_ = [("iterations", C.c_int32), ("restarts", C.c_int32), ("n_sigma", C.c_int32), ("converged", C.c_int32),
                 ("resid", C.c_double * RISP_MAX_ROOTS), ("sec_total", C.c_double), ("sec_matvec", C.c_double),
-                ("sec_subspace", C.c_double), ("bytes_h2d", C.c_double), ("bytes_d2h", C.c_double), ("subspace_max", C.c_int32)]
+                ("sec_subspace", C.c_double), ("bytes_h2d", C.c_double), ("bytes_d2h", C.c_double), ("subspace_max", C.c_int32), ("cached_vectors", C.c_int32)]
 
 
 class _Dims(C.Structure):
@@ -178,11 +178,11 @@ class RispContext:
         """Host buffers given as raw addresses (e.g. pinned torch tensors)."""
         self._check(self.lib.risp_matvec_host(self.handle, m, x_ptr, s_ptr))
 
-    def tda_solve(self, nroots, tol=1e-5, max_iter=100, n_guess=0, max_sub=0, want_vectors=False, allow_unconverged=False):
+    def tda_solve(self, nroots, tol=1e-5, max_iter=100, n_guess=0, max_sub=0, want_vectors=False, allow_unconverged=False, flags=0):
         import torch
         omega = np.zeros(nroots)
         info = _SolveInfo()
-        opt = _SolveOptions(float(tol), int(max_iter), int(n_guess), int(max_sub), 0)
+        opt = _SolveOptions(float(tol), int(max_iter), int(n_guess), int(max_sub), int(flags))
         X = torch.empty((nroots, self.nocc, self.nvir), dtype=torch.float64, device=f"cuda:{self.device}") if want_vectors else None
         rc = self.lib.risp_tda_solve(self.handle, nroots, C.byref(opt), omega.ctypes.data_as(C.POINTER(C.c_double)),
                                      X.data_ptr() if X is not None else None, C.byref(info))

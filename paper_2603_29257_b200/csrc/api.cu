@@ -63,7 +63,7 @@ extern "C" int risp_get_timings(const risp_ctx *cctx, risp_timings *out)
     out->total = el(0, 8);
     out->j_transform_in = el(0, 1); out->j_pass1 = el(1, 2); out->j_solve = el(2, 3); out->j_pass2 = el(3, 4); out->j_transform_out = el(4, 5);
     out->k_gather = el(5, 6); out->k_total = el(6, 7); out->assemble = el(7, 8);
-    if (ctx->has_K) { out->k_gemm1 = el(6, 9); out->k_gemm2 = el(9, 10); }
+    if (ctx->has_K) { out->k_gemm1 = el(11, 9); out->k_gemm2 = el(9, 10); }
     out->kernel_launches = ctx->tim.kernel_launches;
     out->first_chunk_naux = ctx->tim.first_chunk_naux;
     return RISP_OK;

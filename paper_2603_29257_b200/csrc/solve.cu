@@ -6,6 +6,9 @@
 // corrections) streams V / W through the device in chunks on a side stream, double buffered against the compute
 // stream.  When the subspace would outgrow its budget the solver restarts from the current Ritz vectors
 // (reading G17: W <- W y by linearity, no extra sigma-build).
+// "Assisted": whatever HBM is left after the K tensors and the matvec work space caches the leading part of V and W on the
+// device, so only the vectors beyond that cache cross the host link (none for the small configurations, most of them at
+// 3000 atoms).  The pinned host copy is always complete: restarts and the uncached tail read it.
 // The Davidson recipe itself (guess, preconditioner, Gram-Schmidt) is the "standard" one of DESIGN.md reading G16.
 #include "ctx.h"
 #include <algorithm>
@@ -167,9 +170,11 @@ struct Solver {
     double *dB = nullptr, *dWB = nullptr;          // newest block and its image [32][dim]
     double *dX = nullptr, *dAX = nullptr, *dRes = nullptr, *dT = nullptr;   // [nroots][dim]
     double *dChunk[2] = {nullptr, nullptr};        // streaming buffers [CH][dim]
+    double *dVc = nullptr, *dWc = nullptr;         // device cache of the first ncache subspace vectors [ncache][dim]
+    int ncache = 0;
     double *dCoef = nullptr, *dPart = nullptr, *dSmall = nullptr, *dTheta = nullptr;
     int *dSrc = nullptr;
-    cudaEvent_t evUp[2], evFree[2], evD2H;
+    cudaEvent_t evUp[2], evFree[2], evD2H, evReady;
     double bytes_h2d = 0, bytes_d2h = 0;
     cudaStream_t st = 0;                           // compute stream (default)
 };
@@ -210,29 +215,48 @@ int lincomb(Solver &S, const std::vector<double> &coef, int nc, int na, const do
     return RISP_OK;
 }
 
-// stream host vectors [0, n) of `h` through the device in chunks; fn(dev_ptr, first, count) runs on the compute stream
+// pass over subspace vectors [0, n): the first ncache come from the device cache `dc` (chunks of up to 64), the others are
+// streamed from the pinned host array `h` in chunks on the side stream; fn(dev_ptr, first, count) runs on the compute stream
 template <class F>
-int stream_pass(Solver &S, const double *h, int n, F &&fn)
+int stream_pass(Solver &S, const double *h, const double *dc, int n, F &&fn)
 {
     risp_ctx *ctx = S.ctx;
-    int nchunk = (n + S.CH - 1) / S.CH;
+    int rc;
+    const int nc = std::min(n, S.ncache);
+    for (int first = 0; first < nc; first += 64)
+        if ((rc = fn(dc + (long long)first * S.dim, first, std::min(64, nc - first)))) return rc;
+    const int rest = n - nc;
+    int nchunk = (rest + S.CH - 1) / S.CH;
     auto upload = [&](int c) -> int {
-        int b = c & 1, first = c * S.CH, cnt = std::min(S.CH, n - first);
+        int b = c & 1, first = nc + c * S.CH, cnt = std::min(S.CH, n - first);
         RISP_CUDA_TRY(cudaStreamWaitEvent(ctx->side, S.evFree[b], 0));
         RISP_CUDA_TRY(cudaMemcpyAsync(S.dChunk[b], h + (long long)first * S.dim, (size_t)cnt * S.dim * 8, cudaMemcpyHostToDevice, ctx->side));
         RISP_CUDA_TRY(cudaEventRecord(S.evUp[b], ctx->side));
         S.bytes_h2d += (double)cnt * S.dim * 8;
         return RISP_OK;
     };
-    int rc;
     if (nchunk > 0 && (rc = upload(0))) return rc;
     for (int c = 0; c < nchunk; ++c) {
         if (c + 1 < nchunk && (rc = upload(c + 1))) return rc;
-        int b = c & 1, first = c * S.CH, cnt = std::min(S.CH, n - first);
+        int b = c & 1, first = nc + c * S.CH, cnt = std::min(S.CH, n - first);
         RISP_CUDA_TRY(cudaStreamWaitEvent(S.st, S.evUp[b], 0));
         if ((rc = fn(S.dChunk[b], first, cnt))) return rc;
         RISP_CUDA_TRY(cudaEventRecord(S.evFree[b], S.st));
     }
+    return RISP_OK;
+}
+
+// store device vectors src[0, n) as subspace vectors [k, k+n) of (hV|hW, dVc|dWc): always to the pinned host array (side
+// stream, after the compute stream has produced them), and to the device cache where it reaches
+int store_vectors(Solver &S, double *h, double *dc, int k, const double *src, int n)
+{
+    risp_ctx *ctx = S.ctx;
+    RISP_CUDA_TRY(cudaEventRecord(S.evReady, S.st));
+    RISP_CUDA_TRY(cudaStreamWaitEvent(ctx->side, S.evReady, 0));
+    RISP_CUDA_TRY(cudaMemcpyAsync(h + (long long)k * S.dim, src, (size_t)n * S.dim * 8, cudaMemcpyDeviceToHost, ctx->side));
+    S.bytes_d2h += (double)n * S.dim * 8;
+    const int nc = std::max(0, std::min(n, S.ncache - k));
+    if (nc > 0) RISP_CUDA_TRY(cudaMemcpyAsync(dc + (long long)k * S.dim, src, (size_t)nc * S.dim * 8, cudaMemcpyDeviceToDevice, S.st));
     return RISP_OK;
 }
 
@@ -280,6 +304,25 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
     RISP_CUDA_TRY(cudaMalloc((void **)&S.dSrc, RISP_MAX_ROOTS * sizeof(int)));
     for (int b = 0; b < 2; ++b) { RISP_CUDA_TRY(cudaEventCreateWithFlags(&S.evUp[b], cudaEventDisableTiming)); RISP_CUDA_TRY(cudaEventCreateWithFlags(&S.evFree[b], cudaEventDisableTiming)); }
     RISP_CUDA_TRY(cudaEventCreateWithFlags(&S.evD2H, cudaEventDisableTiming));
+    RISP_CUDA_TRY(cudaEventCreateWithFlags(&S.evReady, cudaEventDisableTiming));
+
+    // device cache of the subspace: what is left of HBM once the matvec work space for the largest block exists
+    {
+        int rcw = risp_ensure_workspace(ctx, std::min(nbmax, RISP_MS));
+        if (rcw) return rcw;
+        size_t free_b = 0, total_b = 0;
+        RISP_CUDA_TRY(cudaMemGetInfo(&free_b, &total_b));
+        const size_t keep = (size_t)1 << 30;
+        size_t room = free_b > keep ? (size_t)(0.9 * (double)(free_b - keep)) : 0;
+        if (!(opt.flags & 1)) {      // flags bit 0: no device cache (testing the streamed path)
+            S.ncache = (int)std::min<size_t>((size_t)slots, room / (2 * (size_t)dim * 8));
+            if (opt.flags & 2) S.ncache = std::min(S.ncache, nroots + 2);   // flags bit 1: tiny cache (testing the mixed path)
+        }
+        if (S.ncache > 0) {
+            RISP_CUDA_TRY(cudaMalloc((void **)&S.dVc, (size_t)S.ncache * dim * 8));
+            RISP_CUDA_TRY(cudaMalloc((void **)&S.dWc, (size_t)S.ncache * dim * 8));
+        }
+    }
 
     auto cleanup = [&]() {
         cudaDeviceSynchronize();
@@ -288,7 +331,9 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
         for (double *b : bufs) if (b) cudaFree(b);
         if (S.dSrc) cudaFree(S.dSrc);
         for (int b = 0; b < 2; ++b) { cudaEventDestroy(S.evUp[b]); cudaEventDestroy(S.evFree[b]); }
-        cudaEventDestroy(S.evD2H);
+        cudaEventDestroy(S.evD2H); cudaEventDestroy(S.evReady);
+        if (S.dVc) cudaFree(S.dVc);
+        if (S.dWc) cudaFree(S.dWc);
     };
 #define SOLVE_TRY(x) do { int rc_ = (x); if (rc_) { cleanup(); return rc_; } } while (0)
 
@@ -338,7 +383,7 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
         {
             const int k = S.k;
             std::vector<double> blk;
-            SOLVE_TRY(stream_pass(S, S.hV, k, [&](const double *Vc, int first, int cnt) -> int {
+            SOLVE_TRY(stream_pass(S, S.hV, S.dVc, k, [&](const double *Vc, int first, int cnt) -> int {
                 int r = gram(S, Vc, cnt, S.dWB, nb, blk);
                 if (r) return r;
                 for (int i = 0; i < cnt; ++i)
@@ -349,10 +394,9 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
             for (int i = 0; i < nb; ++i)
                 for (int j = 0; j < nb; ++j) G[(size_t)(k + i) * ldg + k + j] = 0.5 * (blk[(size_t)i * nb + j] + blk[(size_t)j * nb + i]);
             // append B, W_B to the pinned host subspace (side stream)
-            RISP_CUDA_TRY(cudaMemcpyAsync(S.hV + (long long)k * dim, S.dB, (size_t)nb * dim * 8, cudaMemcpyDeviceToHost, ctx->side));
-            RISP_CUDA_TRY(cudaMemcpyAsync(S.hW + (long long)k * dim, S.dWB, (size_t)nb * dim * 8, cudaMemcpyDeviceToHost, ctx->side));
+            SOLVE_TRY(store_vectors(S, S.hV, S.dVc, k, S.dB, nb));
+            SOLVE_TRY(store_vectors(S, S.hW, S.dWc, k, S.dWB, nb));
             RISP_CUDA_TRY(cudaEventRecord(S.evD2H, ctx->side));
-            S.bytes_d2h += 2.0 * nb * dim * 8;
             S.k += nb;
             sub_max = std::max(sub_max, S.k);
         }
@@ -370,7 +414,7 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
         for (int pass = 0; pass < 2; ++pass) {
             double *dst = pass == 0 ? S.dX : S.dAX;
             bool first_chunk = true;
-            SOLVE_TRY(stream_pass(S, pass == 0 ? S.hV : S.hW, k, [&](const double *Vc, int first, int cnt) -> int {
+            SOLVE_TRY(stream_pass(S, pass == 0 ? S.hV : S.hW, pass == 0 ? S.dVc : S.dWc, k, [&](const double *Vc, int first, int cnt) -> int {
                 std::vector<double> coef((size_t)nroots * cnt);
                 for (int j = 0; j < nroots; ++j)
                     for (int i = 0; i < cnt; ++i) coef[(size_t)j * cnt + i] = yv[(size_t)(first + i) * k + j];
@@ -399,11 +443,10 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
         if (it == max_iter) break;
         // ---- restart from the Ritz vectors when the next block would not fit
         if (k + (int)src.size() > S.cap) {
-            RISP_CUDA_TRY(cudaMemcpyAsync(S.hV, S.dX, (size_t)nroots * dim * 8, cudaMemcpyDeviceToHost, ctx->side));
-            RISP_CUDA_TRY(cudaMemcpyAsync(S.hW, S.dAX, (size_t)nroots * dim * 8, cudaMemcpyDeviceToHost, ctx->side));
+            SOLVE_TRY(store_vectors(S, S.hV, S.dVc, 0, S.dX, nroots));
+            SOLVE_TRY(store_vectors(S, S.hW, S.dWc, 0, S.dAX, nroots));
             RISP_CUDA_TRY(cudaEventRecord(S.evD2H, ctx->side));
             RISP_CUDA_TRY(cudaEventSynchronize(S.evD2H));
-            S.bytes_d2h += 2.0 * nroots * dim * 8;
             std::fill(G.begin(), G.end(), 0.0);
             for (int j = 0; j < nroots; ++j) G[(size_t)j * ldg + j] = theta[j];
             S.k = nroots;
@@ -432,7 +475,7 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
         std::vector<double> norms;
         SOLVE_TRY(normalise_rows(S.dT, nb, norms));
         // ---- orthogonalise against V: per streamed chunk, two projections (block Gram-Schmidt with re-orthogonalisation)
-        SOLVE_TRY(stream_pass(S, S.hV, S.k, [&](const double *Vc, int first, int cnt) -> int {
+        SOLVE_TRY(stream_pass(S, S.hV, S.dVc, S.k, [&](const double *Vc, int first, int cnt) -> int {
             for (int rep = 0; rep < 2; ++rep) {
                 std::vector<double> c;
                 int r = gram(S, S.dT, nb, Vc, cnt, c);       // c[j][i] = t_j . v_i
@@ -504,7 +547,7 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
         for (int j = 0; j < nroots; ++j) info->resid[j] = rn[j];
         info->sec_total = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
         info->sec_matvec = sec_mv; info->sec_subspace = info->sec_total - sec_mv;
-        info->bytes_h2d = S.bytes_h2d; info->bytes_d2h = S.bytes_d2h; info->subspace_max = sub_max;
+        info->bytes_h2d = S.bytes_h2d; info->bytes_d2h = S.bytes_d2h; info->subspace_max = sub_max; info->cached_vectors = S.ncache;
     }
     cleanup();
     if (!converged) { risp_set_error(ctx, "risp_tda_solve: not converged within max_iter"); return RISP_ENOTCONV; }

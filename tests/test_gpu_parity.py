@@ -318,11 +318,19 @@ def test_tda_roots(which, ctx1, oracle1, ctx_rsh, oracle_small_rsh):
     assert np.linalg.norm(res.reshape(n, -1), axis=1).max() < 1e-7
 
 
-def test_tda_restart_path(ctx1, oracle1):
+@pytest.mark.parametrize("flags", [0, 1, 2])
+def test_tda_restart_path(flags, ctx1, oracle1):
+    """restart path with the subspace fully cached in HBM (0), fully streamed from pinned host memory (1), and mixed (2)"""
     w_ref = np.linalg.eigvalsh(oracle1.full_A())[:3]
-    omega, _, info = ctx1.tda_solve(3, tol=1e-8, max_sub=30, max_iter=300)
+    omega, _, info = ctx1.tda_solve(3, tol=1e-8, max_sub=30, max_iter=300, flags=flags)
     assert info["restarts"] > 0 and info["converged"] == 1
     assert np.abs(omega - w_ref).max() * HARTREE_EV <= 1e-6
+    if flags == 1:
+        assert info["cached_vectors"] == 0 and info["bytes_h2d"] > 0
+    if flags == 2:
+        assert info["cached_vectors"] == 5 and info["bytes_h2d"] > 0
+    if flags == 0:
+        assert info["bytes_h2d"] == 0
 
 
 # ------------------------------------------------------------------------------------------------ 100-atom config
