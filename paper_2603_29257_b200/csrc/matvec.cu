@@ -40,7 +40,7 @@ size_t risp_plan_workspace(const risp_ctx *ctx, int m, size_t avail, MatvecPlan 
     size_t karena = 0;
     pl.pc = 1;
     if (ctx->has_K) {
-        const size_t klimit = std::min(avail, std::max(6 * GiB, kneed(std::min(2, nK))));
+        const size_t klimit = std::min(avail, std::max(kneed(std::min(2, nK)), std::min(avail / 2, 32 * GiB)));
         if (kneed(1) > avail) return 0;
         int pc = 1;
         while (pc < nK && kneed(pc + 1) <= klimit) ++pc;
@@ -49,7 +49,7 @@ size_t risp_plan_workspace(const risp_ctx *ctx, int m, size_t avail, MatvecPlan 
         karena = kneed(pc) - pc * stage_per_fn;
     }
     // ---- J sub-batch and panels
-    const size_t jlimit = std::min(avail, std::max(karena, 6 * GiB));
+    const size_t jlimit = std::min(avail, std::max(karena, std::min(avail / 2, 32 * GiB)));
     int mj = m;
     size_t prow = nao;
     if (jneed(m, nao) > jlimit) {

@@ -435,9 +435,9 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
             RISP_CUDA_TRY(cudaHostAlloc((void **)&ctx->h_TijP, (size_t)nK_host * tri_o * sizeof(double), cudaHostAllocDefault));
             RISP_CUDA_TRY(cudaHostAlloc((void **)&ctx->h_TabP, (size_t)nK_host * tri_v * sizeof(double), cudaHostAllocDefault));
         }
-        if (ctx->nK_dev > 0) { if ((rc = dalloc(ctx, ctx->d_TabP, (size_t)ctx->nK_dev * tri_v))) return rc; }
         OpParams opK{sys->alpha, sys->beta, sys->omega * sys->omega};
         for (int pass = 0; pass < 2; ++pass) {          // pass 0: occupied window -> BP ; pass 1: virtual window -> T_ab
+            if (pass == 1 && ctx->nK_dev > 0) { if ((rc = dalloc(ctx, ctx->d_TabP, (size_t)ctx->nK_dev * tri_v))) return rc; }
             const int n = pass == 0 ? no : nv, n_p = pass == 0 ? no_p : nv_p;
             const long long tri = pass == 0 ? tri_o : tri_v;
             const double *Cw = pass == 0 ? CoK : CvK;
