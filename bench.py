@@ -109,6 +109,7 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index + 1 (default 2: the 100-atom system)")
     ap.add_argument("--ref-vectors", type=int, default=30, help="trial vectors per step of the CPU oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--batch", type=int, default=0, help="trial vectors per step (0: the config's m)")
     ap.add_argument("--solve", action="store_true", help="also time the 15-root risp_tda_solve (reported under 'solve')")
     args = ap.parse_args()
     # contract: >= 3 warm-up steps; the 1000/3000-atom configs (tens of seconds to minutes per step) are allowed 1 and say so
@@ -130,14 +131,14 @@ def main():
     dev = torch.device(f"cuda:{local}")
 
     s = make_system(args.config)
-    m = s["m"]
+    m = args.batch if args.batch > 0 else s["m"]
     # every rank gets its own seeded batch of m trial vectors (weak scaling over trial vectors, no collective)
-    big = s["nocc"] * s["nvir"] * m > 2e9
+    big = s["nocc"] * s["nvir"] * m > 1e9
     if big:    # 3000-atom scale: one pinned copy of X on the host, filled in place
         Xp = torch.empty((m, s["nocc"], s["nvir"]), dtype=torch.float64, pin_memory=True)
-        X_h = trial_vectors(s, base_seed=260329257 + 17 * rank, out=Xp.numpy())
+        X_h = trial_vectors(s, m, base_seed=260329257 + 17 * rank, out=Xp.numpy())
     else:
-        X_h = trial_vectors(s, base_seed=260329257 + 17 * rank)
+        X_h = trial_vectors(s, m, base_seed=260329257 + 17 * rank)
         Xp = None
     t0 = time.time()
     ctx = setup(s, device=local, max_batch=m)

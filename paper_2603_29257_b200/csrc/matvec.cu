@@ -34,13 +34,14 @@ size_t risp_plan_workspace(const risp_ctx *ctx, int m, size_t avail, MatvecPlan 
     const int nK = ctx->nauxK;
     const size_t GiB = (size_t)1 << 30;
     const size_t stage_per_fn = spilled ? 2 * (size_t)(ctx->tri_o + ctx->tri_v) * 8 : 0;
+    const size_t soft = (spilled ? 12 : 32) * GiB;      // arena target: every GiB of it is a GiB of K tensor streamed from the host when HBM is short
     auto kneed = [&](size_t pc) { return (2 * (size_t)m * no * nv_p + (size_t)m * pc * no_p * nv_p + pc * nv * nv_p + no * pc * no_p) * 8 + pc * stage_per_fn; };
     auto jneed = [&](size_t mj, size_t prow) { return (mj * nocc * ldao + mj * prow * ldao) * 8; };
     // ---- K chunk
     size_t karena = 0;
     pl.pc = 1;
     if (ctx->has_K) {
-        const size_t klimit = std::min(avail, std::max(kneed(std::min(2, nK)), std::min(avail / 2, 32 * GiB)));
+        const size_t klimit = std::min(avail, std::max(kneed(std::min(2, nK)), std::min(avail / 2, soft)));
         if (kneed(1) > avail) return 0;
         int pc = 1;
         while (pc < nK && kneed(pc + 1) <= klimit) ++pc;
@@ -49,7 +50,7 @@ size_t risp_plan_workspace(const risp_ctx *ctx, int m, size_t avail, MatvecPlan 
         karena = kneed(pc) - pc * stage_per_fn;
     }
     // ---- J sub-batch and panels
-    const size_t jlimit = std::min(avail, std::max(karena, std::min(avail / 2, 32 * GiB)));
+    const size_t jlimit = std::min(avail, std::max(karena, std::min(avail / 2, soft)));
     int mj = m;
     size_t prow = nao;
     if (jneed(m, nao) > jlimit) {

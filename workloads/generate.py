@@ -285,6 +285,52 @@ def _torch_cuda():
         return None
 
 
+def _chol_blocked(torch, A, nb=4096):
+    """Lower Cholesky factor of a (device) SPD matrix with panel-sized library calls only (in place on a copy)."""
+    n = A.shape[0]
+    L = A.clone()
+    for k in range(0, n, nb):
+        e = min(n, k + nb)
+        L[k:e, k:e] = torch.linalg.cholesky(L[k:e, k:e])
+        if e < n:
+            # L21 = A21 L11^-T ; A22 -= L21 L21^T
+            L[e:, k:e] = torch.linalg.solve_triangular(L[k:e, k:e], L[e:, k:e].T, upper=False).T
+            L[e:, e:] -= L[e:, k:e] @ L[e:, k:e].T
+    return torch.tril(L)
+
+
+def _mos_by_cholesky(torch, S, rng, device="cuda"):
+    """C with C^T S C = 1 and the distribution of S^-1/2 Q (Q Haar): C = L^-T Q with S = L L^T, because S^-1/2 = L^-T W for an
+    orthogonal W and W Q is Haar again.  Q = the orthogonal factor of a seeded Gaussian matrix with positive-diagonal R, obtained
+    by CholeskyQR2 (two rounds of G <- G chol(G^T G)^-T).  Also returns an estimate of lambda_min(S) by inverse iteration."""
+    n = S.shape[0]
+    St = torch.from_numpy(S).to(device)
+    L = _chol_blocked(torch, St)
+    x = torch.from_numpy(rng.normal(size=(n, 1))).to(device)
+    lam = 0.0
+    for _ in range(40):
+        x = x / torch.linalg.norm(x)
+        y = torch.linalg.solve_triangular(L, x, upper=False)
+        y = torch.linalg.solve_triangular(L.T, y, upper=True)
+        lam = float(1.0 / torch.linalg.norm(y))
+        x = y
+    G = torch.from_numpy(rng.normal(size=(n, n))).to(device)
+    for _ in range(2):
+        Lg = _chol_blocked(torch, G.T @ G)
+        G = torch.linalg.solve_triangular(Lg, G.T, upper=False).T.contiguous()
+        del Lg
+    C = torch.linalg.solve_triangular(L.T, G, upper=True)
+    del G, L
+    E = C.T @ (St @ C)
+    E.diagonal().sub_(1.0)
+    err = float(E.abs().max())
+    out = C.cpu().numpy()
+    del C, E, St
+    if device == "cuda":
+        torch.cuda.empty_cache()
+    return np.ascontiguousarray(out), lam, err
+
+
 def make_system(cfg: int, *, base_seed: int = BASE_SEED, counts=None, check: bool = True) -> dict:
     """Build the seeded synthetic system for BASELINE.json configs[cfg-1].
 
@@ -317,6 +363,15 @@ def make_system(cfg: int, *, base_seed: int = BASE_SEED, counts=None, check: boo
         nao = int(np.sum(2 * shl_l + 1))
         S = _overlap(xyz, shl_atom, shl_l, shl_nprim, shl_poff, pe, pc)
         gpu = _torch_cuda() if nao >= 6000 else None    # harness only: dense eigh / QR of the generator on the GPU when there is one
+        if gpu is not None and nao > 25000:
+            # 3000-atom scale: cuSOLVER's eigen solver and QR stop near n = 30 000 (32-bit work space, the limit PAPER.md:211
+            # mentions), so the same distribution of MOs is drawn with Cholesky factors only (see _mos_by_cholesky)
+            C, w0, ortho_err = _mos_by_cholesky(gpu, S, _seed(cfg, 2, base_seed))
+            w = np.array([w0]); U = None
+            if w0 > 1e-6 or not check:
+                break
+            geom_seed += 1
+            continue
         if gpu is not None:
             St = gpu.from_numpy(S).cuda()
             wt, Ut = gpu.linalg.eigh(St)
@@ -336,8 +391,10 @@ def make_system(cfg: int, *, base_seed: int = BASE_SEED, counts=None, check: boo
         g = THETA / _AUX_RADIUS[int(z)] ** 2
         aux_atom += [ia, ia]; aux_l += [0, 1]; aux_exp += [g, g]; aux_in_K += [1, 0]
     # MOs: C = S^-1/2 Q, Q Haar orthogonal
-    G = _seed(cfg, 2, base_seed).normal(size=(nao, nao))
-    if gpu is not None:
+    if U is None:
+        pass                                              # built by _mos_by_cholesky above
+    elif gpu is not None:
+        G = _seed(cfg, 2, base_seed).normal(size=(nao, nao))
         Qt, Rt = gpu.linalg.qr(gpu.from_numpy(G).cuda())
         del G
         Qt = Qt * gpu.sign(gpu.diagonal(Rt))[None, :]
@@ -351,6 +408,7 @@ def make_system(cfg: int, *, base_seed: int = BASE_SEED, counts=None, check: boo
         del Ct, St, E
         gpu.cuda.empty_cache()
     else:
+        G = _seed(cfg, 2, base_seed).normal(size=(nao, nao))
         Q, R = np.linalg.qr(G)
         Q = Q * np.sign(np.diag(R))[None, :]
         C = (U * (w ** -0.5)[None, :]) @ U.T @ Q
@@ -390,7 +448,7 @@ def trial_vectors(sys: dict, m: int | None = None, *, base_seed: int = BASE_SEED
     """m seeded Gaussian trial vectors [m][nocc][nvir], orthonormalised (DESIGN.md recipe)."""
     m = sys["m"] if m is None else m
     dim = sys["nocc"] * sys["nvir"]
-    if dim * m > 2e9:
+    if dim * m > 1e9:
         # 3000-atom scale: m seeded Gaussian vectors, normalised only (in 1e8 dimensions they are orthogonal to ~1e-4; the
         # sigma-build is linear, so orthonormality is not needed for a throughput run)
         rng = _seed(sys["cfg"], 4, base_seed)
