@@ -236,6 +236,16 @@ def main():
                           peak_source=f"{pk['src']} bf16 burst {pk['bf16']} TFLOP/s x nominal FP64:bf16 ratio 45/2250",
                           flops_per_launch=flops_launch, launch_ms=1e3 * t_launch),
             phases_ms={k: round(1e3 * v / args.steps, 4) for k, v in phase.items() if k not in ("kernel_launches", "first_chunk_naux")},
+            rooflines_other=[
+                dict(phase="K contraction, all chunks (Eq. 22-23, packed-slice expansion included)", bound="tensor", unit="TFLOP/s",
+                     achieved=flops_step["K"] / (phase["k_total"] / args.steps) / 1e12 if phase.get("k_total") else None, peak=peak),
+                dict(phase="J AO<->MO transforms (Eq. 12, 17; e0 gather/scatter and the diagonal term included)", bound="tensor", unit="TFLOP/s",
+                     achieved=flops_step["transforms"] / ((phase["j_transform_in"] + phase["j_transform_out"]) / args.steps) / 1e12, peak=peak),
+                dict(phase="sigma[window] -= K' (Eq. 10)", bound="hbm", unit="GB/s",
+                     achieved=24.0 * m * no * nv / (phase["assemble"] / args.steps) / 1e9 if phase.get("assemble") else None, peak=pk["hbm"]),
+                dict(phase="ERI passes (Eq. 14, 16): (pair, aux centre) tasks per second, both passes", bound="alu", unit="Gtask/s",
+                     achieved=2.0 * d["n_shell_pairs_kept"] * (d["nauxJ"] / 4) / ((phase["j_pass1"] + phase["j_pass2"]) / args.steps) / 1e9, peak=None),
+            ],
             flops_per_step=flops_step,
         )
         if not args.no_cpu_baseline and world == 1 and not big:

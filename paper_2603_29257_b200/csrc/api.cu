@@ -23,6 +23,8 @@ extern "C" void risp_destroy(risp_ctx *ctx)
     if (ctx->ev_ok) {
         for (int i = 0; i < RISP_NEV; ++i) cudaEventDestroy(ctx->ev[i]);
         for (int b = 0; b < 2; ++b) { cudaEventDestroy(ctx->evStage[b]); cudaEventDestroy(ctx->evStageFree[b]); }
+        cudaEventDestroy(ctx->evFork);
+        for (int c = 0; c < 6; ++c) { cudaEventDestroy(ctx->evJoin[c]); cudaStreamDestroy(ctx->cls_st[c]); }
     }
     if (ctx->side) cudaStreamDestroy(ctx->side);
     delete ctx;

@@ -79,6 +79,8 @@ struct risp_ctx {
     bool ev_ok = false;
     risp_timings tim;
     cudaStream_t side = nullptr;  // side stream: host-resident K chunks, Davidson subspace copies
+    cudaStream_t cls_st[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // the six pair classes of a J step run concurrently
+    cudaEvent_t evFork = nullptr, evJoin[6];
 };
 
 // ---- eri_kernels.cu
@@ -101,6 +103,7 @@ cudaError_t risp_j_pass2(const PairClass &pc, const risp_eri::PrimPair *prims, c
 // ---- linalg.cu: Cholesky A = L L^T (lower, in place; upper triangle zeroed) and Linv = L^-1, both [n][n] row-major on the device.
 // *info_host = 0 on success, k+1 if the k-th pivot is not positive.
 cudaError_t risp_cholesky_inverse(double *A, double *Linv, int n, int *info_host, cudaStream_t st);
+cudaError_t risp_metric_solve32(const double *Linv, int n, const double *R, double *tmp, double *Rt, cudaStream_t st);
 
 // ---- elementwise.cu
 cudaError_t risp_gather_window(const double *X, double *Xk, int m, int nocc, int nvir, int o0, int no, int v0, int nv, int ldk, cudaStream_t st);

@@ -245,17 +245,20 @@ __global__ void __launch_bounds__(32 * JW) j_pass1_kernel(const ShellPair *__res
     }
 }
 
-__global__ void j_reduce_R_kernel(const double *__restrict__ Rpart, int nchunks, const AuxCentre *__restrict__ cen, int ncen, int ncen_pad,
-                                  double *__restrict__ R)
+// R[q][lane] = sum over pair chunks of the pass-1 partials, fixed order (4 interleaved partial sums, then their sum)
+__global__ void __launch_bounds__(128) j_reduce_R_kernel(const double *__restrict__ Rpart, int nchunks, const AuxCentre *__restrict__ cen, int ncen,
+                                                         int ncen_pad, double *__restrict__ R)
 {
-    const int lane = threadIdx.x, k = blockIdx.x;          // k = centre*4 + comp
+    __shared__ double part[4][32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, k = blockIdx.x;          // k = centre*4 + comp
     const int ci = k >> 2, c = k & 3;
-    if (ci >= ncen) return;
     const int q = c == 0 ? cen[ci].qs : (cen[ci].qp < 0 ? -1 : cen[ci].qp + c - 1);
     if (q < 0) return;
     double s = 0.0;
-    for (int ch = 0; ch < nchunks; ++ch) s += Rpart[(((long long)ch * ncen_pad + ci) * 4 + c) * MS + lane];
-    R[(long long)q * MS + lane] = s;
+    for (int ch = w; ch < nchunks; ch += 4) s += Rpart[(((long long)ch * ncen_pad + ci) * 4 + c) * MS + lane];
+    part[w][lane] = s;
+    __syncthreads();
+    if (w == 0) R[(long long)q * MS + lane] = (part[0][lane] + part[1][lane]) + (part[2][lane] + part[3][lane]);
 }
 
 template <class F>
@@ -342,7 +345,7 @@ cudaError_t risp_j_pass1(const PairClass &pc, const PrimPair *prims, const AuxCe
 
 cudaError_t risp_j_reduce_R(const double *Rpart, int nchunks, const AuxCentre *cen, int ncen, int ncen_pad, double *R, cudaStream_t st)
 {
-    j_reduce_R_kernel<<<ncen * 4, 32, 0, st>>>(Rpart, nchunks, cen, ncen, ncen_pad, R);
+    j_reduce_R_kernel<<<ncen * 4, 128, 0, st>>>(Rpart, nchunks, cen, ncen, ncen_pad, R);
     return cudaGetLastError();
 }
 

@@ -135,6 +135,24 @@ static void panel_pairs(const PairClass &pc, int r0, int r1, int &p0, int &p1)
     p1 = (int)(std::lower_bound(pc.h_aoA.begin(), pc.h_aoA.end(), r1) - pc.h_aoA.begin());
 }
 
+// The six pair classes of one J step touch disjoint rows of D-bar / U-bar / R partials and disjoint AO blocks, so their kernels
+// run concurrently on six internal streams between a fork and a join on the caller's stream (the small classes -- a few dozen
+// CTAs at 100 atoms -- would otherwise each leave most of the 148 SMs idle).
+static int fork_classes(risp_ctx *ctx, cudaStream_t st)
+{
+    RISP_CUDA_TRY(cudaEventRecord(ctx->evFork, st));
+    for (int c = 0; c < 6; ++c) RISP_CUDA_TRY(cudaStreamWaitEvent(ctx->cls_st[c], ctx->evFork, 0));
+    return RISP_OK;
+}
+static int join_classes(risp_ctx *ctx, cudaStream_t st)
+{
+    for (int c = 0; c < 6; ++c) {
+        RISP_CUDA_TRY(cudaEventRecord(ctx->evJoin[c], ctx->cls_st[c]));
+        RISP_CUDA_TRY(cudaStreamWaitEvent(st, ctx->evJoin[c], 0));
+    }
+    return RISP_OK;
+}
+
 int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaStream_t st)
 {
     const int nao = ctx->nao, nocc = ctx->nocc, nvir = ctx->nvir, nJ = ctx->nauxJ;
@@ -143,7 +161,7 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
     const MatvecPlan &pl = ctx->plan;
     const int npanel = (int)pl.panel_r0.size() - 1;
     const bool dense = npanel == 1;
-    int launches = 0;
+    int launches = 0, rc;
     cudaEvent_t *ev = ctx->ev;
     RISP_CUDA_TRY(cudaEventRecord(ev[0], st));
     // ---------------- diagonal (Eq. 10)
@@ -170,36 +188,37 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
                 f.nb1 = mj; f.sA1 = (long long)nocc * ldao; f.sC1 = mstride;
                 RISP_CUDA_TRY(risp_dgemm(f, st)); ++launches;
             }
+            if ((rc = fork_classes(ctx, st))) return rc;
             for (int c = 0; c < 6; ++c) {
                 int p0, p1;
                 panel_pairs(ctx->cls[c], r0, r1, p0, p1);
-                if (p1 > p0) { RISP_CUDA_TRY(risp_dens_to_e0(ctx->cls[c], p0, p1, mj, l0, r0, ldao, mstride, dense ? 0 : 1, wD, ctx->w_dbar, st)); ++launches; }
+                if (p1 > p0) { RISP_CUDA_TRY(risp_dens_to_e0(ctx->cls[c], p0, p1, mj, l0, r0, ldao, mstride, dense ? 0 : 1, wD, ctx->w_dbar, ctx->cls_st[c])); ++launches; }
             }
+            if ((rc = join_classes(ctx, st))) return rc;
         }
     }
     RISP_CUDA_TRY(cudaEventRecord(ev[1], st));
     // ---------------- pass 1: R_mQ (Eq. 14)
-    for (int c = 0; c < 6; ++c)
+    if ((rc = fork_classes(ctx, st))) return rc;
+    for (int c = 5; c >= 0; --c)          // heaviest recursion first
         if (ctx->cls[c].npairs) {
-            RISP_CUDA_TRY(risp_j_pass1(ctx->cls[c], ctx->d_prims, ctx->d_cenJ, ctx->ncenJ, ctx->ncenJ_pad, ctx->d_boys, ctx->w_dbar, ctx->w_Rpart, st));
+            RISP_CUDA_TRY(risp_j_pass1(ctx->cls[c], ctx->d_prims, ctx->d_cenJ, ctx->ncenJ, ctx->ncenJ_pad, ctx->d_boys, ctx->w_dbar, ctx->w_Rpart, ctx->cls_st[c]));
             ++launches;
         }
+    if ((rc = join_classes(ctx, st))) return rc;
     RISP_CUDA_TRY(risp_j_reduce_R(ctx->w_Rpart, ctx->total_chunks, ctx->d_cenJ, ctx->ncenJ, ctx->ncenJ_pad, ctx->w_R, st)); ++launches;
     RISP_CUDA_TRY(cudaEventRecord(ev[2], st));
     // ---------------- R~ = (P|Q)^-1 R = L^-T (L^-1 R)  (Eq. 15)
-    {
-        GemmDesc d = gemm_desc(nJ, RISP_MS, nJ, ctx->d_LinvJ, nJ, true, ctx->w_R, RISP_MS, false, ctx->w_Rtmp, RISP_MS);
-        RISP_CUDA_TRY(risp_dgemm(d, st)); ++launches;
-        GemmDesc e = gemm_desc(nJ, RISP_MS, nJ, ctx->d_LinvJ, nJ, false, ctx->w_Rtmp, RISP_MS, false, ctx->w_Rt, RISP_MS);
-        RISP_CUDA_TRY(risp_dgemm(e, st)); ++launches;
-    }
+    RISP_CUDA_TRY(risp_metric_solve32(ctx->d_LinvJ, nJ, ctx->w_R, ctx->w_Rtmp, ctx->w_Rt, st)); launches += 2;
     RISP_CUDA_TRY(cudaEventRecord(ev[3], st));
     // ---------------- pass 2: U (Eq. 16), into the e0 buffer
-    for (int c = 0; c < 6; ++c)
+    if ((rc = fork_classes(ctx, st))) return rc;
+    for (int c = 5; c >= 0; --c)
         if (ctx->cls[c].npairs) {
-            RISP_CUDA_TRY(risp_j_pass2(ctx->cls[c], ctx->d_prims, ctx->d_cenJ, ctx->ncenJ, ctx->d_boys, ctx->w_Rt, ctx->w_dbar, st));
+            RISP_CUDA_TRY(risp_j_pass2(ctx->cls[c], ctx->d_prims, ctx->d_cenJ, ctx->ncenJ, ctx->d_boys, ctx->w_Rt, ctx->w_dbar, ctx->cls_st[c]));
             ++launches;
         }
+    if ((rc = join_classes(ctx, st))) return rc;
     RISP_CUDA_TRY(cudaEventRecord(ev[4], st));
     // ---------------- back-transform (Eq. 17), sigma += 2 J
     for (int l0 = 0; l0 < m; l0 += pl.mj) {
@@ -208,11 +227,13 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
             const int r0 = pl.panel_r0[p], r1 = pl.panel_r0[p + 1], pr = r1 - r0;
             const long long mstride = (long long)pr * ldao;
             RISP_CUDA_TRY(cudaMemsetAsync(wD, 0, (size_t)mj * mstride * sizeof(double), st));
+            if ((rc = fork_classes(ctx, st))) return rc;
             for (int c = 0; c < 6; ++c) {
                 int p0, p1;
                 panel_pairs(ctx->cls[c], r0, r1, p0, p1);
-                if (p1 > p0) { RISP_CUDA_TRY(risp_e0_to_U(ctx->cls[c], p0, p1, mj, l0, r0, ldao, mstride, dense ? 1 : 0, ctx->w_dbar, wD, st)); ++launches; }
+                if (p1 > p0) { RISP_CUDA_TRY(risp_e0_to_U(ctx->cls[c], p0, p1, mj, l0, r0, ldao, mstride, dense ? 1 : 0, ctx->w_dbar, wD, ctx->cls_st[c])); ++launches; }
             }
+            if ((rc = join_classes(ctx, st))) return rc;
             // Z[i][nu] (+)= sum_{mu in panel} C_occ[mu][i] P[mu][nu]
             GemmDesc d = gemm_desc(nocc, nao, pr, ctx->d_Cocc + (size_t)r0 * ldocc, ldocc, false, wD, ldao, false, wY, ldao, 1.0, p == 0 ? 0.0 : 1.0);
             d.nb1 = mj; d.sB1 = mstride; d.sC1 = (long long)nocc * ldao;
@@ -275,7 +296,7 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
         };
         int first_host = -1;
         for (size_t i = 0; i < chunks.size(); ++i) if (chunks[i].host) { first_host = (int)i; break; }
-        int nhost_seen = 0, rc;
+        int nhost_seen = 0;
         if (first_host >= 0 && (rc = prefetch(first_host, 0))) return rc;
         for (size_t ci = 0; ci < chunks.size(); ++ci) {
             const Chunk &c = chunks[ci];

@@ -323,8 +323,9 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
         long long e_off = 0, total_pairs = 0;
         for (int c = 0; c < 6; ++c) total_pairs += (long long)pairs[c].size();
         ctx->n_shell_pairs_kept = total_pairs;
-        int chunk = (int)std::max<long long>(64, (total_pairs + 511) / 512);
-        chunk = (chunk + 15) / 16 * 16;
+        // pass-1 chunking per class: about 16 CTAs per SM over (pair chunks) x (groups of 8 aux centres), at least 16 pairs per chunk
+        const int cta_per_chunk = (ctx->ncenJ + 7) / 8;
+        const int want_chunks = std::max(1, (16 * 148 + cta_per_chunk - 1) / cta_per_chunk);
         int chunk_base = 0;
         static const int LA[6] = {0, 1, 1, 2, 2, 2}, LB[6] = {0, 0, 1, 0, 1, 2};
         for (int c = 0; c < 6; ++c) {
@@ -335,7 +336,12 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
             pc.h_aoA.resize(pc.npairs);
             for (int k = 0; k < pc.npairs; ++k) pc.h_aoA[k] = pairs[c][k].aoA;
             pc.e_off = e_off; e_off += (long long)pc.npairs * ne_of(pc.la, pc.lb);
-            pc.chunk = chunk; pc.nchunks = (pc.npairs + chunk - 1) / chunk; pc.chunk_base = chunk_base; chunk_base += pc.nchunks;
+            {
+                const int nch = std::max(1, std::min((pc.npairs + 15) / 16, want_chunks));
+                int chunk = (pc.npairs + nch - 1) / nch;
+                chunk = std::max(16, (chunk + 15) / 16 * 16);
+                pc.chunk = chunk; pc.nchunks = (pc.npairs + chunk - 1) / chunk; pc.chunk_base = chunk_base; chunk_base += pc.nchunks;
+            }
             int rc;
             if ((rc = upload(ctx, pc.d_pairs, pairs[c].data(), pairs[c].size()))) return rc;
         }
@@ -429,8 +435,13 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
         RISP_CUDA_TRY(cudaMemset(CvK, 0, (size_t)nao * nv_p * sizeof(double)));
         RISP_CUDA_TRY(cudaMemcpy2D(CoK, (size_t)no_p * 8, ctx->d_Cocc + ctx->occK0, (size_t)ctx->ldocc * 8, (size_t)no * 8, nao, cudaMemcpyDeviceToDevice));
         RISP_CUDA_TRY(cudaMemcpy2D(CvK, (size_t)nv_p * 8, ctx->d_Cvir + ctx->virK0, (size_t)ctx->ldvir * 8, (size_t)nv * 8, nao, cudaMemcpyDeviceToDevice));
-        // all (ij|Q) slices, packed, in HBM until the metric has been applied (Eq. 20 mixes every Q)
-        RISP_CUDA_TRY(cudaMalloc((void **)&BP, (size_t)nK * tri_o * sizeof(double)));
+        // all (ij|Q) slices, packed, in HBM until the metric has been applied (Eq. 20 mixes every Q): the first nK_dev of them
+        // in their final place, the others in a block that is copied to the host and freed afterwards
+        double *BPr = nullptr;
+        if (ctx->nK_dev > 0) { if ((rc = dalloc(ctx, ctx->d_TijP, (size_t)ctx->nK_dev * tri_o))) return rc; }
+        if (nK_host > 0) RISP_CUDA_TRY(cudaMalloc((void **)&BPr, (size_t)nK_host * tri_o * sizeof(double)));
+        BP = ctx->d_TijP;
+        auto bp_slice = [&](int f) { return f < ctx->nK_dev ? BP + (size_t)f * tri_o : BPr + (size_t)(f - ctx->nK_dev) * tri_o; };
         if (nK_host > 0) {
             RISP_CUDA_TRY(cudaHostAlloc((void **)&ctx->h_TijP, (size_t)nK_host * tri_o * sizeof(double), cudaHostAllocDefault));
             RISP_CUDA_TRY(cudaHostAlloc((void **)&ctx->h_TabP, (size_t)nK_host * tri_v * sizeof(double), cudaHostAllocDefault));
@@ -469,7 +480,8 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
                 d2.nb1 = nf; d2.sB1 = (long long)nao * n_p; d2.sC1 = (long long)n * n_p;
                 RISP_CUDA_TRY(risp_dgemm(d2, 0));
                 if (pass == 0) {
-                    RISP_CUDA_TRY(risp_pack_sym(F, (long long)n * n_p, n_p, n, nf, BP + (size_t)f0 * tri, tri, 0));
+                    for (int f = f0; f < f1; ++f)
+                        RISP_CUDA_TRY(risp_pack_sym(F + (size_t)(f - f0) * n * n_p, (long long)n * n_p, n_p, n, 1, bp_slice(f), tri, 0));
                 } else {
                     RISP_CUDA_TRY(risp_pack_sym(F, (long long)n * n_p, n_p, n, nf, Pk, tri, 0));
                     for (int f = f0; f < f1; ++f) {
@@ -482,26 +494,32 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
                 c0 = c1;
             }
             if (pass == 0) {
-                // T_ij^P = sum_Q (P|Q)^-1 (ij|Q)   (Eq. 20): BP <- MKinv BP, in column panels, in place
+                // T_ij^P = sum_Q (P|Q)^-1 (ij|Q)   (Eq. 20): [BP; BPr] <- MKinv [BP; BPr], in column panels, in place
+                const int nKd = ctx->nK_dev;
                 long long w = std::min<long long>(tri_o, std::max<long long>(2, (((long long)1 << 30) / ((long long)nK * 8)) & ~1LL));
                 double *tmpc = nullptr;
                 RISP_CUDA_TRY(cudaMalloc((void **)&tmpc, (size_t)nK * w * sizeof(double)));
                 for (long long col = 0; col < tri_o; col += w) {
                     const int wc = (int)std::min<long long>(w, tri_o - col);
-                    GemmDesc d5 = gemm_desc(nK, wc, nK, ctx->d_MKinv, nK, true, BP + col, tri_o, false, tmpc, w);
-                    RISP_CUDA_TRY(risp_dgemm(d5, 0));
-                    RISP_CUDA_TRY(cudaMemcpy2DAsync(BP + col, (size_t)tri_o * 8, tmpc, (size_t)w * 8, (size_t)wc * 8, nK, cudaMemcpyDeviceToDevice, 0));
+                    if (nKd > 0) {
+                        GemmDesc d5 = gemm_desc(nK, wc, nKd, ctx->d_MKinv, nK, true, BP + col, tri_o, false, tmpc, w);
+                        RISP_CUDA_TRY(risp_dgemm(d5, 0));
+                    }
+                    if (nK_host > 0) {
+                        GemmDesc d6 = gemm_desc(nK, wc, nK_host, ctx->d_MKinv + nKd, nK, true, BPr + col, tri_o, false, tmpc, w, 1.0, nKd > 0 ? 1.0 : 0.0);
+                        RISP_CUDA_TRY(risp_dgemm(d6, 0));
+                    }
+                    if (nKd > 0)
+                        RISP_CUDA_TRY(cudaMemcpy2DAsync(BP + col, (size_t)tri_o * 8, tmpc, (size_t)w * 8, (size_t)wc * 8, nKd, cudaMemcpyDeviceToDevice, 0));
+                    if (nK_host > 0)
+                        RISP_CUDA_TRY(cudaMemcpy2DAsync(BPr + col, (size_t)tri_o * 8, tmpc + (size_t)nKd * w, (size_t)w * 8, (size_t)wc * 8, nK_host,
+                                                        cudaMemcpyDeviceToDevice, 0));
                 }
                 RISP_CUDA_TRY(cudaDeviceSynchronize());
                 cudaFree(tmpc);
-                if (nK_host == 0) { ctx->d_TijP = BP; BP = nullptr; ctx->setup_bytes += (size_t)nK * tri_o * 8; }
-                else {
-                    RISP_CUDA_TRY(cudaMemcpy(ctx->h_TijP, BP + (size_t)ctx->nK_dev * tri_o, (size_t)nK_host * tri_o * 8, cudaMemcpyDeviceToHost));
-                    if (ctx->nK_dev > 0) {
-                        if ((rc = dalloc(ctx, ctx->d_TijP, (size_t)ctx->nK_dev * tri_o))) return rc;
-                        RISP_CUDA_TRY(cudaMemcpy(ctx->d_TijP, BP, (size_t)ctx->nK_dev * tri_o * 8, cudaMemcpyDeviceToDevice));
-                    }
-                    cudaFree(BP); BP = nullptr;
+                if (nK_host > 0) {
+                    RISP_CUDA_TRY(cudaMemcpy(ctx->h_TijP, BPr, (size_t)nK_host * tri_o * 8, cudaMemcpyDeviceToHost));
+                    cudaFree(BPr); BPr = nullptr;
                 }
             }
         }
@@ -511,6 +529,11 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
     RISP_CUDA_TRY(cudaDeviceSynchronize());
     RISP_CUDA_TRY(cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking));
     for (int i = 0; i < RISP_NEV; ++i) RISP_CUDA_TRY(cudaEventCreate(&ctx->ev[i]));
+    RISP_CUDA_TRY(cudaEventCreateWithFlags(&ctx->evFork, cudaEventDisableTiming));
+    for (int c = 0; c < 6; ++c) {
+        RISP_CUDA_TRY(cudaStreamCreateWithFlags(&ctx->cls_st[c], cudaStreamNonBlocking));
+        RISP_CUDA_TRY(cudaEventCreateWithFlags(&ctx->evJoin[c], cudaEventDisableTiming));
+    }
     for (int b = 0; b < 2; ++b) {
         RISP_CUDA_TRY(cudaEventCreateWithFlags(&ctx->evStage[b], cudaEventDisableTiming));
         RISP_CUDA_TRY(cudaEventCreateWithFlags(&ctx->evStageFree[b], cudaEventDisableTiming));
