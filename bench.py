@@ -260,7 +260,7 @@ def main():
                                         gpu_vs_oracle_rel_err=err)
         if args.solve:
             omega, _, info = ctx.tda_solve(s["nroots"], tol=1e-5, allow_unconverged=True)
-            line["solve"] = dict(nroots=s["nroots"], tol=1e-5, wall_s=info["sec_total"], matvec_s=info["sec_matvec"], iterations=info["iterations"],
+            line["solve"] = dict(nroots=s["nroots"], tol=1e-5, wall_s=info["sec_total"], matvec_s=info["sec_matvec"], alloc_s=info["sec_alloc"], subspace_s=info["sec_subspace"], cached_vectors=info["cached_vectors"], iterations=info["iterations"],
                                  n_sigma=info["n_sigma"], restarts=info["restarts"], converged=info["converged"], omega_ev=[float(x) * 27.211386245988 for x in omega],
                                  h2d_gb=info["bytes_h2d"] / 1e9, d2h_gb=info["bytes_d2h"] / 1e9)
         print(json.dumps(line))

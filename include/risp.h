@@ -103,10 +103,11 @@ typedef struct {
 typedef struct {
     int32_t iterations, restarts, n_sigma, converged;
     double resid[RISP_MAX_ROOTS];        /* final residual norms */
-    double sec_total, sec_matvec, sec_subspace; /* wall seconds */
+    double sec_total, sec_matvec, sec_subspace; /* wall seconds: whole call, sigma-builds, subspace algebra (incl. streaming) */
     double bytes_h2d, bytes_d2h;         /* subspace traffic over the host link */
     int32_t subspace_max;                /* largest subspace held */
     int32_t cached_vectors;              /* leading vectors of V and of W kept in HBM as well */
+    double sec_alloc;                    /* wall seconds spent allocating the pinned subspace and the device buffers */
 } risp_solve_info;
 
 typedef struct {

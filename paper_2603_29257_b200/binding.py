@@ -48,7 +48,7 @@ class _SolveOptions(C.Structure):
 class _SolveInfo(C.Structure):
     _fields_ = [("iterations", C.c_int32), ("restarts", C.c_int32), ("n_sigma", C.c_int32), ("converged", C.c_int32),
                 ("resid", C.c_double * RISP_MAX_ROOTS), ("sec_total", C.c_double), ("sec_matvec", C.c_double),
-                ("sec_subspace", C.c_double), ("bytes_h2d", C.c_double), ("bytes_d2h", C.c_double), ("subspace_max", C.c_int32), ("cached_vectors", C.c_int32)]
+                ("sec_subspace", C.c_double), ("bytes_h2d", C.c_double), ("bytes_d2h", C.c_double), ("subspace_max", C.c_int32), ("cached_vectors", C.c_int32), ("sec_alloc", C.c_double)]
 
 
 class _Dims(C.Structure):
@@ -92,6 +92,7 @@ def load_library():
     lib.risp_debug_dgemm.argtypes = [C.c_int, C.c_int, C.c_int, vp, C.c_longlong, C.c_int, vp, C.c_longlong, C.c_int, vp, C.c_longlong,
                                      dbl, dbl, C.c_int, C.c_longlong, C.c_longlong, C.c_longlong, vp]
     lib.risp_debug_sym_eig.argtypes = [C.c_int, vp, vp, vp]
+    lib.risp_debug_sym_eig_lowest.argtypes = [C.c_int, C.c_int, vp, vp, vp]
     lib.risp_debug_force_plan.argtypes = [vp, C.c_int, C.c_int, C.c_int]
     lib.risp_debug_set_gemm_variant.argtypes = [C.c_int]
     _LIB = lib

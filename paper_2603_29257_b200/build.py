@@ -45,7 +45,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return SO
     with ThreadPoolExecutor(max_workers=8) as ex:
         objs = list(ex.map(compile_one, SOURCES))
-    r = subprocess.run([nvcc, "-shared", "-o", SO] + objs + ["-lcudart"], capture_output=True, text=True)
+    r = subprocess.run([nvcc, "-shared", "-o", SO] + objs + ["-lcudart", "-lpthread"], capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
     return SO

@@ -245,20 +245,35 @@ __global__ void __launch_bounds__(32 * JW) j_pass1_kernel(const ShellPair *__res
     }
 }
 
-// R[q][lane] = sum over pair chunks of the pass-1 partials, fixed order (4 interleaved partial sums, then their sum)
-__global__ void __launch_bounds__(128) j_reduce_R_kernel(const double *__restrict__ Rpart, int nchunks, const AuxCentre *__restrict__ cen, int ncen,
+// R[q][lane] = sum over pair chunks of the pass-1 partials, fixed order: warp w of 8 takes chunks w, w+8, ... into four
+// interleaved partial sums (independent loads in flight), then the 8 warps' sums are added in order
+__global__ void __launch_bounds__(256) j_reduce_R_kernel(const double *__restrict__ Rpart, int nchunks, const AuxCentre *__restrict__ cen, int ncen,
                                                          int ncen_pad, double *__restrict__ R)
 {
-    __shared__ double part[4][32];
+    __shared__ double part[8][32];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, k = blockIdx.x;          // k = centre*4 + comp
     const int ci = k >> 2, c = k & 3;
     const int q = c == 0 ? cen[ci].qs : (cen[ci].qp < 0 ? -1 : cen[ci].qp + c - 1);
     if (q < 0) return;
-    double s = 0.0;
-    for (int ch = w; ch < nchunks; ch += 4) s += Rpart[(((long long)ch * ncen_pad + ci) * 4 + c) * MS + lane];
-    part[w][lane] = s;
+    const long long stride = (long long)ncen_pad * 4 * MS;
+    const double *src = Rpart + ((long long)ci * 4 + c) * MS + lane;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    int ch = w;
+    for (; ch + 24 < nchunks; ch += 32) {
+        s0 += src[(long long)ch * stride];
+        s1 += src[(long long)(ch + 8) * stride];
+        s2 += src[(long long)(ch + 16) * stride];
+        s3 += src[(long long)(ch + 24) * stride];
+    }
+    for (; ch < nchunks; ch += 8) s0 += src[(long long)ch * stride];
+    part[w][lane] = (s0 + s1) + (s2 + s3);
     __syncthreads();
-    if (w == 0) R[(long long)q * MS + lane] = (part[0][lane] + part[1][lane]) + (part[2][lane] + part[3][lane]);
+    if (w == 0) {
+        double s = 0.0;
+#pragma unroll
+        for (int ww = 0; ww < 8; ++ww) s += part[ww][lane];
+        R[(long long)q * MS + lane] = s;
+    }
 }
 
 template <class F>
@@ -345,7 +360,7 @@ cudaError_t risp_j_pass1(const PairClass &pc, const PrimPair *prims, const AuxCe
 
 cudaError_t risp_j_reduce_R(const double *Rpart, int nchunks, const AuxCentre *cen, int ncen, int ncen_pad, double *R, cudaStream_t st)
 {
-    j_reduce_R_kernel<<<ncen * 4, 128, 0, st>>>(Rpart, nchunks, cen, ncen, ncen_pad, R);
+    j_reduce_R_kernel<<<ncen * 4, 256, 0, st>>>(Rpart, nchunks, cen, ncen, ncen_pad, R);
     return cudaGetLastError();
 }
 

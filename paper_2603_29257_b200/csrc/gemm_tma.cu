@@ -24,6 +24,8 @@ constexpr int BM_MAX = 128, BN = 128, BK = 16, STAGES = 5, NWARPS = 8, NT = NWAR
 constexpr int TILE_BYTES = BM_MAX * BK * 8;                   // 16 KiB per operand per stage (A tiles of MI < 8 use a part of it)
 constexpr size_t SMEM_BYTES = (size_t)STAGES * 2 * TILE_BYTES + 1024 /*alignment slack*/ + 2 * STAGES * 8;
 
+int sm_count();
+
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
@@ -76,8 +78,8 @@ struct TmaArgs {
     int za1, za2, zb1, zb2;      // 1: the operand moves with batch index z1 / z2; 0: shared by the batch
 };
 
-// MI = 8x8 DMMA tiles per warp along m: CTA tile BM = 16 MI rows (128, 112, 96, 80), chosen per call to minimise the
-// padding of the last tile row (e.g. M = N_occK' = 423: 4 x 112 instead of 4 x 128).
+// MI = 8x8 DMMA tiles per warp along m: CTA tile BM = 16 MI rows (128 ... 16), chosen per call (pick_mi).  The small values
+// serve the skinny products of the Davidson loop (15 x dim Gram and Ritz updates), which are HBM-bound anyway.
 template <bool AKC, bool BKC, int MI>
 __global__ void __launch_bounds__(NT, 1) dgemm_tma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                                                           GemmDesc d, TmaArgs ta, int tiles_m, int tiles_n)
@@ -106,10 +108,12 @@ __global__ void __launch_bounds__(NT, 1) dgemm_tma_kernel(const __grid_constant_
     const int my_tiles = ((int)blockIdx.x < total_tiles) ? (total_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     const long long total_steps = (long long)my_tiles * nk;
 
-    // producer state (thread 0): next step to issue
+    // producer state (warp 0, kept identically by all its lanes): next step to issue
     long long h = 0;
     int h_ti = 0, h_kt = 0, h_slot = 0;
     unsigned h_par = 1;                                        // parity to wait on the empty barrier (fresh barrier passes 1)
+    // executed by all lanes of warp 0: lane 0 waits for the slot and arms the barrier, then the boxes of the stage are issued by
+    // one lane each (an MN-contiguous operand is BM/16 or 8 boxes: issuing them from one thread costs that warp ~10 % of a k tile)
     auto issue = [&]() {
         const int tile = (int)blockIdx.x + h_ti * (int)gridDim.x;
         const int z = tile / tiles_per_batch, tt = tile % tiles_per_batch;
@@ -117,24 +121,26 @@ __global__ void __launch_bounds__(NT, 1) dgemm_tma_kernel(const __grid_constant_
         const int z1 = z / d.nb2, z2 = z % d.nb2;
         const int m0 = tm * BM, n0 = tn * BN, k0 = h_kt * BK;
         const unsigned fb = full0 + 8 * h_slot;
-        mbar_wait(empty0 + 8 * h_slot, h_par);
-        mbar_expect_tx(fb, (BM + BN) * BK * 8);
-        const unsigned da = As_u + h_slot * TILE_BYTES, db = Bs_u + h_slot * TILE_BYTES;
-        if (AKC) tma_load_4d(da, &tmA, fb, k0 + ta.coff_a, m0, z2 * ta.za2, z1 * ta.za1);
-        else {
-#pragma unroll
-            for (int b = 0; b < BM / 16; ++b) tma_load_4d(da + b * 2048, &tmA, fb, m0 + b * 16 + ta.coff_a, k0, z2 * ta.za2, z1 * ta.za1);
+        if (lane == 0) {
+            mbar_wait(empty0 + 8 * h_slot, h_par);
+            mbar_expect_tx(fb, (BM + BN) * BK * 8);
         }
-        if (BKC) tma_load_4d(db, &tmB, fb, k0 + ta.coff_b, n0, z2 * ta.zb2, z1 * ta.zb1);
-        else {
-#pragma unroll
-            for (int b = 0; b < BN / 16; ++b) tma_load_4d(db + b * 2048, &tmB, fb, n0 + b * 16 + ta.coff_b, k0, z2 * ta.zb2, z1 * ta.zb1);
+        __syncwarp();
+        const unsigned da = As_u + h_slot * TILE_BYTES, db = Bs_u + h_slot * TILE_BYTES;
+        constexpr int NA = AKC ? 1 : BM / 16, NB = BKC ? 1 : BN / 16;
+        if (lane < NA) {
+            if (AKC) tma_load_4d(da, &tmA, fb, k0 + ta.coff_a, m0, z2 * ta.za2, z1 * ta.za1);
+            else tma_load_4d(da + lane * 2048, &tmA, fb, m0 + lane * 16 + ta.coff_a, k0, z2 * ta.za2, z1 * ta.za1);
+        } else if (lane < NA + NB) {
+            const int b = lane - NA;
+            if (BKC) tma_load_4d(db, &tmB, fb, k0 + ta.coff_b, n0, z2 * ta.zb2, z1 * ta.zb1);
+            else tma_load_4d(db + b * 2048, &tmB, fb, n0 + b * 16 + ta.coff_b, k0, z2 * ta.zb2, z1 * ta.zb1);
         }
         ++h;
         if (++h_kt == nk) { h_kt = 0; ++h_ti; }
         if (++h_slot == STAGES) { h_slot = 0; h_par ^= 1; }
     };
-    if (tid == 0) {
+    if (warp == 0) {
         for (int s = 0; s < STAGES - 2 && h < total_steps; ++s) issue();
     }
 
@@ -164,8 +170,7 @@ __global__ void __launch_bounds__(NT, 1) dgemm_tma_kernel(const __grid_constant_
             for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
         for (int kt = 0; kt < nk; ++kt) {
-            if (tid == 0 && h < total_steps) issue();
-            __syncwarp();
+            if (warp == 0 && h < total_steps) issue();
             mbar_wait(full0 + 8 * slot, par);
             const unsigned char *as = As + slot * TILE_BYTES;
             const unsigned char *bs = Bs + slot * TILE_BYTES;
@@ -272,14 +277,13 @@ bool make_map(EncodeFn enc, CUtensorMap *tm, const double *p, bool kc, int MN, i
 template <bool AKC, bool BKC, int MI>
 cudaError_t launch_mi(const CUtensorMap &ma, const CUtensorMap &mb, const GemmDesc &d, const TmaArgs &ta, cudaStream_t st)
 {
-    static int sms = 0;
-    if (!sms) {
+    static bool attr = false;
+    if (!attr) {
         cudaError_t e = cudaFuncSetAttribute(dgemm_tma_kernel<AKC, BKC, MI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
         if (e != cudaSuccess) return e;
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        attr = true;
     }
+    const int sms = sm_count();
     constexpr int BM = 16 * MI;
     const int tiles_m = (d.M + BM - 1) / BM, tiles_n = (d.N + BN - 1) / BN;
     const long long total = (long long)tiles_m * tiles_n * d.nb1 * d.nb2;
@@ -288,17 +292,32 @@ cudaError_t launch_mi(const CUtensorMap &ma, const CUtensorMap &mb, const GemmDe
     return cudaGetLastError();
 }
 
-// rows of padding in the last tile row for BM = 16 mi; prefer the larger tile unless a smaller one saves >= 4 % of the work
-int pick_mi(int M)
+// Tile height BM = 16 mi for this call: minimise (waves over the SMs) x (rows per tile), i.e. both the padding of the last
+// tile row (M = N_occK' = 423: 4 x 112 instead of 4 x 128) and the idle tail of the last wave (M = 4500, 6 column tiles:
+// 47 x 6 tiles of 96 rows fill 1.9 waves, 36 x 6 tiles of 128 rows only 1.46); smaller tiles are charged 1.5 % per step.
+int pick_mi(int M, long long col_tiles_x_batch, int sms)
 {
     int best = 8;
-    double best_cost = (double)((M + 127) / 128) * 128;
-    for (int mi = 7; mi >= 5; --mi) {
+    double best_cost = 1e300;
+    for (int mi = 8; mi >= 1; --mi) {
         const int bm = 16 * mi;
-        const double cost = (double)((M + bm - 1) / bm) * bm * (1.0 + 0.01 * (8 - mi));   // smaller tiles: a little less efficient
-        if (cost < 0.96 * best_cost) { best = mi; best_cost = cost; }
+        const long long tiles = (long long)((M + bm - 1) / bm) * col_tiles_x_batch;
+        const long long waves = (tiles + sms - 1) / sms;
+        const double cost = (double)waves * (bm + 12.0) * (1.0 + 0.015 * (8 - mi));   // + ~12 rows' worth of per-tile overhead
+        if (cost < best_cost * 0.995) { best = mi; best_cost = cost; }
     }
     return best;
+}
+
+int sm_count()
+{
+    static int sms = 0;
+    if (!sms) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    }
+    return sms;
 }
 
 template <bool AKC, bool BKC>
@@ -308,6 +327,10 @@ cudaError_t launch(const CUtensorMap &ma, const CUtensorMap &mb, const GemmDesc 
     case 7: return launch_mi<AKC, BKC, 7>(ma, mb, d, ta, st);
     case 6: return launch_mi<AKC, BKC, 6>(ma, mb, d, ta, st);
     case 5: return launch_mi<AKC, BKC, 5>(ma, mb, d, ta, st);
+    case 4: return launch_mi<AKC, BKC, 4>(ma, mb, d, ta, st);
+    case 3: return launch_mi<AKC, BKC, 3>(ma, mb, d, ta, st);
+    case 2: return launch_mi<AKC, BKC, 2>(ma, mb, d, ta, st);
+    case 1: return launch_mi<AKC, BKC, 1>(ma, mb, d, ta, st);
     default: return launch_mi<AKC, BKC, 8>(ma, mb, d, ta, st);
     }
 }
@@ -319,7 +342,7 @@ cudaError_t launch(const CUtensorMap &ma, const CUtensorMap &mb, const GemmDesc 
 cudaError_t risp_dgemm_tma(const GemmDesc &d, cudaStream_t st)
 {
     if (d.K <= 0) return cudaErrorNotSupported;
-    const int mi = pick_mi(d.M);
+    const int mi = pick_mi(d.M, (long long)((d.N + BN - 1) / BN) * d.nb1 * d.nb2, sm_count());
     if ((long long)((d.M + 16 * mi - 1) / (16 * mi)) * ((d.N + BN - 1) / BN) * d.nb1 * d.nb2 >= (1ll << 31)) return cudaErrorNotSupported;
     EncodeFn enc = get_encode();
     if (!enc) return cudaErrorNotSupported;

@@ -88,34 +88,38 @@ __global__ void trinv_row_kernel(double *X, int n, int i0, int nb, const double 
     }
 }
 // C[p][lane] = sum_q op(A)(p,q) B[q][lane], A lower triangular [n][n], B and C [n][32].  TRANS: op(A) = A^T.
-// One warp per output row, the 32 lanes are the 32 trial-vector slots of R / R~ (Eq. 15).
+// One CTA per output row; its 8 warps split the q range (two partial sums each), the 32 lanes are the 32 trial-vector slots of
+// R / R~ (Eq. 15); the partial sums are added in a fixed order.
 template <bool TRANS>
 __global__ void __launch_bounds__(256) tri_mat32_kernel(const double *__restrict__ A, int n, const double *__restrict__ B, double *__restrict__ C)
 {
-    const int lane = threadIdx.x, p = blockIdx.x * blockDim.y + threadIdx.y;
-    if (p >= n) return;
-    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    __shared__ double part[8][32];
+    const int lane = threadIdx.x, w = threadIdx.y, p = blockIdx.x;
     const int q0 = TRANS ? p : 0, q1 = TRANS ? n : p + 1;
-    int q = q0;
-    for (; q + 3 < q1; q += 4) {
+    double a0 = 0.0, a1 = 0.0;
+    int q = q0 + w;
+    for (; q + 8 < q1; q += 16) {
         const double x0 = TRANS ? A[(long long)q * n + p] : A[(long long)p * n + q];
-        const double x1 = TRANS ? A[(long long)(q + 1) * n + p] : A[(long long)p * n + q + 1];
-        const double x2 = TRANS ? A[(long long)(q + 2) * n + p] : A[(long long)p * n + q + 2];
-        const double x3 = TRANS ? A[(long long)(q + 3) * n + p] : A[(long long)p * n + q + 3];
+        const double x1 = TRANS ? A[(long long)(q + 8) * n + p] : A[(long long)p * n + q + 8];
         a0 = fma(x0, B[(long long)q * 32 + lane], a0);
-        a1 = fma(x1, B[(long long)(q + 1) * 32 + lane], a1);
-        a2 = fma(x2, B[(long long)(q + 2) * 32 + lane], a2);
-        a3 = fma(x3, B[(long long)(q + 3) * 32 + lane], a3);
+        a1 = fma(x1, B[(long long)(q + 8) * 32 + lane], a1);
     }
-    for (; q < q1; ++q) a0 = fma(TRANS ? A[(long long)q * n + p] : A[(long long)p * n + q], B[(long long)q * 32 + lane], a0);
-    C[(long long)p * 32 + lane] = (a0 + a1) + (a2 + a3);
+    if (q < q1) a0 = fma(TRANS ? A[(long long)q * n + p] : A[(long long)p * n + q], B[(long long)q * 32 + lane], a0);
+    part[w][lane] = a0 + a1;
+    __syncthreads();
+    if (w == 0) {
+        double s = 0.0;
+#pragma unroll
+        for (int ww = 0; ww < 8; ++ww) s += part[ww][lane];
+        C[(long long)p * 32 + lane] = s;
+    }
 }
 }  // namespace
 
 // R~ = L^-T (L^-1 R) with the precomputed lower-triangular L^-1; R, tmp, Rt are [n][32]
 cudaError_t risp_metric_solve32(const double *Linv, int n, const double *R, double *tmp, double *Rt, cudaStream_t st)
 {
-    dim3 block(32, 8), grid((n + 7) / 8);
+    dim3 block(32, 8), grid(n);
     tri_mat32_kernel<false><<<grid, block, 0, st>>>(Linv, n, R, tmp);
     tri_mat32_kernel<true><<<grid, block, 0, st>>>(Linv, n, tmp, Rt);
     return cudaGetLastError();

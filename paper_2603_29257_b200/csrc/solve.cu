@@ -6,14 +6,17 @@
 // corrections) streams V / W through the device in chunks on a side stream, double buffered against the compute
 // stream.  When the subspace would outgrow its budget the solver restarts from the current Ritz vectors
 // (reading G17: W <- W y by linearity, no extra sigma-build).
-// "Assisted": whatever HBM is left after the K tensors and the matvec work space caches the leading part of V and W on the
-// device, so only the vectors beyond that cache cross the host link (none for the small configurations, most of them at
-// 3000 atoms).  The pinned host copy is always complete: restarts and the uncached tail read it.
+// "Assisted": whatever HBM is left after the K tensors and the matvec work space holds the leading part of V and W on the
+// device; the vectors beyond it live in pinned host memory (page-locked chunk by chunk by a background thread) and are
+// streamed over the host link on the side stream -- none for the small configurations, most of them at 3000 atoms, all of
+// them with RISP_SOLVE_NO_CACHE.
 // The Davidson recipe itself (guess, preconditioner, Gram-Schmidt) is the "standard" one of DESIGN.md reading G16.
 #include "ctx.h"
 #include <algorithm>
+#include <atomic>
 #include <chrono>
 #include <cmath>
+#include <thread>
 
 namespace {
 
@@ -75,9 +78,10 @@ __global__ void reduce_partials_kernel(const double *__restrict__ part, int nz, 
 // component of eigenvector j.
 void sym_eig(std::vector<double> &a, int n, std::vector<double> &w, std::vector<double> &z)
 {
-    z.assign((size_t)n * n, 0.0);
-    for (int i = 0; i < n; ++i) z[(size_t)i * n + i] = 1.0;
-    std::vector<double> v(n), p(n), d(n), e(n, 0.0);
+    // zt[j*n + i] = i-th component of (current) basis vector j: every update below runs over contiguous rows
+    std::vector<double> zt((size_t)n * n, 0.0);
+    for (int i = 0; i < n; ++i) zt[(size_t)i * n + i] = 1.0;
+    std::vector<double> v(n), p(n), d(n), e(n, 0.0), sr(n);
     for (int k = 0; k + 2 < n; ++k) {
         int len = n - k - 1;
         double nrm = 0.0;
@@ -93,22 +97,32 @@ void sym_eig(std::vector<double> &a, int n, std::vector<double> &w, std::vector<
         double beta = 2.0 / vv;
         for (int i = 0; i < len; ++i) {                   // p = beta A22 v
             double s = 0.0;
-            for (int j = 0; j < len; ++j) s += a[(size_t)(k + 1 + i) * n + k + 1 + j] * v[j];
+            const double *row = &a[(size_t)(k + 1 + i) * n + k + 1];
+            for (int j = 0; j < len; ++j) s += row[j] * v[j];
             p[i] = beta * s;
         }
         double K = 0.0;
         for (int i = 0; i < len; ++i) K += v[i] * p[i];
         K *= 0.5 * beta;
         for (int i = 0; i < len; ++i) p[i] -= K * v[i];   // w
-        for (int i = 0; i < len; ++i)
-            for (int j = 0; j < len; ++j) a[(size_t)(k + 1 + i) * n + k + 1 + j] -= v[i] * p[j] + p[i] * v[j];
+        for (int i = 0; i < len; ++i) {
+            double *row = &a[(size_t)(k + 1 + i) * n + k + 1];
+            const double vi = v[i], pi = p[i];
+            for (int j = 0; j < len; ++j) row[j] -= vi * p[j] + pi * v[j];
+        }
         a[(size_t)(k + 1) * n + k] = a[(size_t)k * n + k + 1] = alpha;
         for (int i = 1; i < len; ++i) a[(size_t)(k + 1 + i) * n + k] = a[(size_t)k * n + k + 1 + i] = 0.0;
-        for (int r = 0; r < n; ++r) {                     // Q <- Q H
-            double s = 0.0;
-            for (int j = 0; j < len; ++j) s += z[(size_t)r * n + k + 1 + j] * v[j];
-            s *= beta;
-            for (int j = 0; j < len; ++j) z[(size_t)r * n + k + 1 + j] -= s * v[j];
+        // Q <- Q H: columns k+1.. of Q are rows k+1.. of zt;  s_r = sum_j Q[r][k+1+j] v[j]
+        std::fill(sr.begin(), sr.end(), 0.0);
+        for (int j = 0; j < len; ++j) {
+            const double *zr = &zt[(size_t)(k + 1 + j) * n];
+            const double vj = v[j];
+            for (int r = 0; r < n; ++r) sr[r] += zr[r] * vj;
+        }
+        for (int j = 0; j < len; ++j) {
+            double *zr = &zt[(size_t)(k + 1 + j) * n];
+            const double bv = beta * v[j];
+            for (int r = 0; r < n; ++r) zr[r] -= sr[r] * bv;
         }
     }
     for (int i = 0; i < n; ++i) d[i] = a[(size_t)i * n + i];
@@ -138,10 +152,11 @@ void sym_eig(std::vector<double> &a, int n, std::vector<double> &w, std::vector<
                     pp = s * r;
                     d[i + 1] = g + pp;
                     g = c * r - b;
+                    double *z0 = &zt[(size_t)i * n], *z1 = &zt[(size_t)(i + 1) * n];
                     for (int k = 0; k < n; ++k) {
-                        double f2 = z[(size_t)k * n + i + 1];
-                        z[(size_t)k * n + i + 1] = s * z[(size_t)k * n + i] + c * f2;
-                        z[(size_t)k * n + i] = c * z[(size_t)k * n + i] - s * f2;
+                        const double f2 = z1[k];
+                        z1[k] = s * z0[k] + c * f2;
+                        z0[k] = c * z0[k] - s * f2;
                     }
                 }
                 if (r == 0.0 && i >= l) continue;
@@ -149,29 +164,220 @@ void sym_eig(std::vector<double> &a, int n, std::vector<double> &w, std::vector<
             }
         } while (m != l);
     }
-    // sort ascending
+    // sort ascending; z[i*n + j] = i-th component of eigenvector j
     std::vector<int> ord(n);
     for (int i = 0; i < n; ++i) ord[i] = i;
     std::sort(ord.begin(), ord.end(), [&](int x, int y) { return d[x] < d[y]; });
     w.resize(n);
-    std::vector<double> zs((size_t)n * n);
+    z.assign((size_t)n * n, 0.0);
     for (int j = 0; j < n; ++j) {
         w[j] = d[ord[j]];
-        for (int i = 0; i < n; ++i) zs[(size_t)i * n + j] = z[(size_t)i * n + ord[j]];
+        const double *zr = &zt[(size_t)ord[j] * n];
+        for (int i = 0; i < n; ++i) z[(size_t)i * n + j] = zr[i];
     }
-    z.swap(zs);
 }
+
+// The nv lowest eigenpairs only (what a Davidson iteration needs; the full QL accumulation above costs ~9 n^3 flops, 90 ms at
+// n = 315, once per iteration): Householder tridiagonalisation with the reflectors kept, eigenvalues by QL without vectors,
+// eigenvectors of T by inverse iteration (pivoted tridiagonal LU, re-orthogonalised against the vectors already found, as
+// LAPACK's dstein does for clusters), back-transformed through the reflectors.  z[i*n + j], j < nv; w has all n eigenvalues.
+void sym_eig_lowest(std::vector<double> &a, int n, int nv, std::vector<double> &w, std::vector<double> &z)
+{
+    nv = std::min(nv, n);
+    std::vector<double> vs((size_t)n * n, 0.0), betas(n, 0.0), v(n), p(n), d(n), e(n, 0.0);
+    for (int k = 0; k + 2 < n; ++k) {
+        int len = n - k - 1;
+        double nrm = 0.0;
+        for (int i = 0; i < len; ++i) { v[i] = a[(size_t)(k + 1 + i) * n + k]; nrm += v[i] * v[i]; }
+        nrm = std::sqrt(nrm);
+        double tail = 0.0;
+        for (int i = 1; i < len; ++i) tail += v[i] * v[i];
+        if (tail == 0.0) continue;
+        double alpha = v[0] > 0 ? -nrm : nrm;
+        v[0] -= alpha;
+        double vv = 0.0;
+        for (int i = 0; i < len; ++i) vv += v[i] * v[i];
+        double beta = 2.0 / vv;
+        for (int i = 0; i < len; ++i) {
+            double s = 0.0;
+            const double *row = &a[(size_t)(k + 1 + i) * n + k + 1];
+            for (int j = 0; j < len; ++j) s += row[j] * v[j];
+            p[i] = beta * s;
+        }
+        double K = 0.0;
+        for (int i = 0; i < len; ++i) K += v[i] * p[i];
+        K *= 0.5 * beta;
+        for (int i = 0; i < len; ++i) p[i] -= K * v[i];
+        for (int i = 0; i < len; ++i) {
+            double *row = &a[(size_t)(k + 1 + i) * n + k + 1];
+            const double vi = v[i], pi = p[i];
+            for (int j = 0; j < len; ++j) row[j] -= vi * p[j] + pi * v[j];
+        }
+        a[(size_t)(k + 1) * n + k] = a[(size_t)k * n + k + 1] = alpha;
+        for (int i = 1; i < len; ++i) a[(size_t)(k + 1 + i) * n + k] = a[(size_t)k * n + k + 1 + i] = 0.0;
+        betas[k] = beta;
+        std::copy(v.begin(), v.begin() + len, vs.begin() + (size_t)k * n);
+    }
+    for (int i = 0; i < n; ++i) d[i] = a[(size_t)i * n + i];
+    for (int i = 0; i + 1 < n; ++i) e[i] = a[(size_t)(i + 1) * n + i];
+    const std::vector<double> d0 = d, e0 = e;          // T, kept for the inverse iteration
+    for (int l = 0; l < n; ++l) {                       // QL, eigenvalues only
+        int iter = 0, m;
+        do {
+            for (m = l; m < n - 1; ++m) {
+                double dd = std::fabs(d[m]) + std::fabs(d[m + 1]);
+                if (std::fabs(e[m]) <= 2.3e-16 * dd) break;
+            }
+            if (m != l) {
+                if (++iter > 200) break;
+                double g = (d[l + 1] - d[l]) / (2.0 * e[l]);
+                double r = std::hypot(g, 1.0);
+                g = d[m] - d[l] + e[l] / (g + (g >= 0 ? std::fabs(r) : -std::fabs(r)));
+                double s = 1.0, c = 1.0, pp = 0.0;
+                int i;
+                for (i = m - 1; i >= l; --i) {
+                    double f = s * e[i], b = c * e[i];
+                    e[i + 1] = r = std::hypot(f, g);
+                    if (r == 0.0) { d[i + 1] -= pp; e[m] = 0.0; break; }
+                    s = f / r; c = g / r;
+                    g = d[i + 1] - pp;
+                    r = (d[i] - g) * s + 2.0 * c * b;
+                    pp = s * r;
+                    d[i + 1] = g + pp;
+                    g = c * r - b;
+                }
+                if (r == 0.0 && i >= l) continue;
+                d[l] -= pp; e[l] = g; e[m] = 0.0;
+            }
+        } while (m != l);
+    }
+    w = d;
+    std::sort(w.begin(), w.end());
+    double tnorm = 0.0;
+    for (int i = 0; i < n; ++i) tnorm = std::max(tnorm, std::fabs(d0[i]) + (i ? std::fabs(e0[i - 1]) : 0.0) + (i + 1 < n ? std::fabs(e0[i]) : 0.0));
+    const double eps = 2.2e-16, tiny = std::max(tnorm, 1e-300) * eps;
+    z.assign((size_t)n * n, 0.0);
+    std::vector<double> X((size_t)nv * n), dl(n), dd(n), du(n), du2(n), x(n);
+    std::vector<char> piv(n);
+    double lam_prev = 0.0;
+    for (int j = 0; j < nv; ++j) {
+        double lam = w[j];
+        if (j > 0 && lam - lam_prev < 10.0 * tiny) lam = lam_prev + 10.0 * tiny;   // separate numerically equal eigenvalues
+        lam_prev = lam;
+        // LU of T - lam I with partial pivoting (dgttrf)
+        for (int i = 0; i < n; ++i) { dd[i] = d0[i] - lam; dl[i] = du[i] = (i + 1 < n) ? e0[i] : 0.0; du2[i] = 0.0; piv[i] = 0; }
+        for (int i = 0; i + 1 < n; ++i) {
+            if (std::fabs(dd[i]) >= std::fabs(dl[i])) {
+                if (dd[i] == 0.0) dd[i] = tiny;
+                const double f = dl[i] / dd[i];
+                dl[i] = f; dd[i + 1] -= f * du[i];
+            } else {
+                const double f = dd[i] / dl[i];
+                dd[i] = dl[i]; dl[i] = f;
+                const double t = du[i];
+                du[i] = dd[i + 1]; dd[i + 1] = t - f * dd[i + 1];
+                if (i + 2 < n) { du2[i] = du[i + 1]; du[i + 1] = -f * du[i + 1]; }
+                piv[i] = 1;
+            }
+        }
+        if (std::fabs(dd[n - 1]) < tiny) dd[n - 1] = tiny;
+        for (int i = 0; i < n - 1; ++i) if (std::fabs(dd[i]) < tiny * 1e-3) dd[i] = tiny;
+        unsigned long long seed = 0x9E3779B97F4A7C15ull * (unsigned long long)(j + 1);
+        for (int i = 0; i < n; ++i) { seed = seed * 6364136223846793005ull + 1442695040888963407ull; x[i] = ((double)(seed >> 11) / 9007199254740992.0) - 0.5; }
+        double *xj = &X[(size_t)j * n];
+        for (int it = 0; it < 5; ++it) {
+            for (int i = 0; i + 1 < n; ++i) {
+                if (!piv[i]) x[i + 1] -= dl[i] * x[i];
+                else { const double t = x[i]; x[i] = x[i + 1]; x[i + 1] = t - dl[i] * x[i]; }
+            }
+            x[n - 1] /= dd[n - 1];
+            if (n > 1) x[n - 2] = (x[n - 2] - du[n - 2] * x[n - 1]) / dd[n - 2];
+            for (int i = n - 3; i >= 0; --i) x[i] = (x[i] - du[i] * x[i + 1] - du2[i] * x[i + 2]) / dd[i];
+            for (int rep = 0; rep < 2; ++rep)
+                for (int q = 0; q < j; ++q) {
+                    if (w[j] - w[q] > 1e-3 * std::max(tnorm, 1e-300)) continue;      // well separated: orthogonal by themselves
+                    const double *xq = &X[(size_t)q * n];
+                    double dot = 0.0;
+                    for (int i = 0; i < n; ++i) dot += xq[i] * x[i];
+                    for (int i = 0; i < n; ++i) x[i] -= dot * xq[i];
+                }
+            double nr = 0.0;
+            for (int i = 0; i < n; ++i) nr += x[i] * x[i];
+            nr = 1.0 / std::sqrt(std::max(nr, 1e-300));
+            for (int i = 0; i < n; ++i) x[i] *= nr;
+        }
+        std::copy(x.begin(), x.end(), xj);
+        // back-transform: y = H_0 H_1 ... H_{n-3} x
+        for (int k = n - 3; k >= 0; --k) {
+            if (betas[k] == 0.0) continue;
+            const int len = n - k - 1;
+            const double *vk = &vs[(size_t)k * n];
+            double dot = 0.0;
+            for (int i = 0; i < len; ++i) dot += vk[i] * x[k + 1 + i];
+            dot *= betas[k];
+            for (int i = 0; i < len; ++i) x[k + 1 + i] -= dot * vk[i];
+        }
+        for (int i = 0; i < n; ++i) z[(size_t)i * n + j] = x[i];
+    }
+}
+
+// The pinned host copy of the subspace: V and W as chunks of 32 vectors, page-locked by a background thread
+// while the first sigma-builds run (pinning 7 GB takes ~2.7 s -- a fifth of a 300-atom solve if done up front).
+struct HostStore {
+    static constexpr int CHV = 32;
+    long long dim = 0;
+    int nchunks = 0, device = 0, slots = 0;
+    std::vector<double *> v, w;
+    std::atomic<int> ready{0}, failed{0}, stop{0};
+    std::thread th;
+    void start(int dev, long long dim_, int slots_)
+    {
+        device = dev; dim = dim_; slots = slots_;
+        nchunks = (slots + CHV - 1) / CHV;
+        v.assign(nchunks, nullptr); w.assign(nchunks, nullptr);
+        th = std::thread([this] {
+            cudaSetDevice(device);
+            for (int c = 0; c < nchunks && !stop.load(); ++c) {
+                const size_t nvec = (size_t)std::min(CHV, slots - c * CHV);
+                if (cudaHostAlloc((void **)&v[c], nvec * dim * 8, cudaHostAllocDefault) != cudaSuccess ||
+                    cudaHostAlloc((void **)&w[c], nvec * dim * 8, cudaHostAllocDefault) != cudaSuccess) { failed.store(1); return; }
+                ready.store(c + 1, std::memory_order_release);
+            }
+        });
+    }
+    // host address of vector i of V (isW = false) or W; blocks until its chunk is pinned; nullptr if the allocation failed
+    double *ptr(bool isW, long long i)
+    {
+        const int c = (int)(i / CHV);
+        while (ready.load(std::memory_order_acquire) <= c) {
+            if (failed.load()) return nullptr;
+            std::this_thread::yield();
+        }
+        return (isW ? w[c] : v[c]) + (i % CHV) * dim;
+    }
+    ~HostStore() { finish(); }
+    void finish()
+    {
+        stop.store(1);
+        if (th.joinable()) th.join();
+        for (double *p : v) if (p) cudaFreeHost(p);
+        for (double *p : w) if (p) cudaFreeHost(p);
+        v.clear(); w.clear();
+    }
+};
 
 struct Solver {
     risp_ctx *ctx;
     long long dim;
     int cap = 0, k = 0, CH = 16;
-    double *hV = nullptr, *hW = nullptr;           // pinned host [cap][dim]
+    HostStore host;                                // pinned host copy of V and W
     double *dB = nullptr, *dWB = nullptr;          // newest block and its image [32][dim]
     double *dX = nullptr, *dAX = nullptr, *dRes = nullptr, *dT = nullptr;   // [nroots][dim]
     double *dChunk[2] = {nullptr, nullptr};        // streaming buffers [CH][dim]
     double *dVc = nullptr, *dWc = nullptr;         // device cache of the first ncache subspace vectors [ncache][dim]
     int ncache = 0;
+    long long slice = 16384;                       // split-K slice of the Gram products
+    std::vector<double> tmp;
     double *dCoef = nullptr, *dPart = nullptr, *dSmall = nullptr, *dTheta = nullptr;
     int *dSrc = nullptr;
     cudaEvent_t evUp[2], evFree[2], evD2H, evReady;
@@ -181,26 +387,38 @@ struct Solver {
 
 int gram(Solver &S, const double *A, int na, const double *B, int nb, std::vector<double> &out)
 {
-    // out[na][nb] = sum_x A[i][x] B[j][x]: split-K batched DMMA GEMM + fixed-order reduction
+    // out[na][nb] = sum_x A[i][x] B[j][x]: split-K batched DMMA GEMM + fixed-order reduction.  The smaller operand goes to the
+    // M side (16-row tiles exist, the N tile is always 128 wide); the product is HBM-bound: it reads (na + nb) dim doubles.
     risp_ctx *ctx = S.ctx;
-    const long long slice = 16384;
+    const bool swap = na > nb;
+    const double *P = swap ? B : A, *Q = swap ? A : B;
+    const int np = swap ? nb : na, nq = swap ? na : nb;
+    const long long slice = S.slice;
     int nfull = (int)(S.dim / slice);
     long long tail = S.dim - (long long)nfull * slice;
     int nz = nfull + (tail ? 1 : 0);
     if (nfull) {
-        GemmDesc d = gemm_desc(na, nb, (int)slice, A, S.dim, true, B, S.dim, true, S.dPart, nb);
-        d.nb1 = nfull; d.sA1 = slice; d.sB1 = slice; d.sC1 = (long long)na * nb;
+        GemmDesc d = gemm_desc(np, nq, (int)slice, P, S.dim, true, Q, S.dim, true, S.dPart, nq);
+        d.nb1 = nfull; d.sA1 = slice; d.sB1 = slice; d.sC1 = (long long)np * nq;
         RISP_CUDA_TRY(risp_dgemm(d, S.st));
     }
     if (tail) {
-        GemmDesc d = gemm_desc(na, nb, (int)tail, A + (long long)nfull * slice, S.dim, true, B + (long long)nfull * slice, S.dim, true,
-                               S.dPart + (long long)nfull * na * nb, nb);
+        GemmDesc d = gemm_desc(np, nq, (int)tail, P + (long long)nfull * slice, S.dim, true, Q + (long long)nfull * slice, S.dim, true,
+                               S.dPart + (long long)nfull * np * nq, nq);
         RISP_CUDA_TRY(risp_dgemm(d, S.st));
     }
-    reduce_partials_kernel<<<(na * nb + 127) / 128, 128, 0, S.st>>>(S.dPart, nz, na * nb, S.dSmall);
+    reduce_partials_kernel<<<(np * nq + 127) / 128, 128, 0, S.st>>>(S.dPart, nz, np * nq, S.dSmall);
     out.resize((size_t)na * nb);
-    RISP_CUDA_TRY(cudaMemcpyAsync(out.data(), S.dSmall, (size_t)na * nb * 8, cudaMemcpyDeviceToHost, S.st));
-    RISP_CUDA_TRY(cudaStreamSynchronize(S.st));
+    if (!swap) {
+        RISP_CUDA_TRY(cudaMemcpyAsync(out.data(), S.dSmall, (size_t)na * nb * 8, cudaMemcpyDeviceToHost, S.st));
+        RISP_CUDA_TRY(cudaStreamSynchronize(S.st));
+    } else {
+        S.tmp.resize((size_t)na * nb);
+        RISP_CUDA_TRY(cudaMemcpyAsync(S.tmp.data(), S.dSmall, (size_t)na * nb * 8, cudaMemcpyDeviceToHost, S.st));
+        RISP_CUDA_TRY(cudaStreamSynchronize(S.st));
+        for (int i = 0; i < na; ++i)
+            for (int j = 0; j < nb; ++j) out[(size_t)i * nb + j] = S.tmp[(size_t)j * na + i];
+    }
     return RISP_OK;
 }
 
@@ -215,22 +433,28 @@ int lincomb(Solver &S, const std::vector<double> &coef, int nc, int na, const do
     return RISP_OK;
 }
 
-// pass over subspace vectors [0, n): the first ncache come from the device cache `dc` (chunks of up to 64), the others are
-// streamed from the pinned host array `h` in chunks on the side stream; fn(dev_ptr, first, count) runs on the compute stream
+// pass over subspace vectors [0, n): the first ncache come from the device cache `dc` (chunks of up to 128), the others are
+// streamed from the pinned host store (V or W) in chunks on the side stream; fn(dev_ptr, first, count) runs on the compute stream
 template <class F>
-int stream_pass(Solver &S, const double *h, const double *dc, int n, F &&fn)
+int stream_pass(Solver &S, bool isW, const double *dc, int n, F &&fn)
 {
     risp_ctx *ctx = S.ctx;
     int rc;
     const int nc = std::min(n, S.ncache);
-    for (int first = 0; first < nc; first += 64)
-        if ((rc = fn(dc + (long long)first * S.dim, first, std::min(64, nc - first)))) return rc;
+    for (int first = 0; first < nc; first += 128)
+        if ((rc = fn(dc + (long long)first * S.dim, first, std::min(128, nc - first)))) return rc;
     const int rest = n - nc;
     int nchunk = (rest + S.CH - 1) / S.CH;
     auto upload = [&](int c) -> int {
         int b = c & 1, first = nc + c * S.CH, cnt = std::min(S.CH, n - first);
         RISP_CUDA_TRY(cudaStreamWaitEvent(ctx->side, S.evFree[b], 0));
-        RISP_CUDA_TRY(cudaMemcpyAsync(S.dChunk[b], h + (long long)first * S.dim, (size_t)cnt * S.dim * 8, cudaMemcpyHostToDevice, ctx->side));
+        for (int done = 0; done < cnt;) {           // a block of CH vectors may straddle two pinned chunks
+            const int i = first + done - S.ncache, seg = std::min(cnt - done, HostStore::CHV - i % HostStore::CHV);
+            const double *h = S.host.ptr(isW, i);
+            if (!h) { risp_set_error(ctx, "risp_tda_solve: pinned host allocation of the subspace failed"); return RISP_ENOMEM; }
+            RISP_CUDA_TRY(cudaMemcpyAsync(S.dChunk[b] + (long long)done * S.dim, h, (size_t)seg * S.dim * 8, cudaMemcpyHostToDevice, ctx->side));
+            done += seg;
+        }
         RISP_CUDA_TRY(cudaEventRecord(S.evUp[b], ctx->side));
         S.bytes_h2d += (double)cnt * S.dim * 8;
         return RISP_OK;
@@ -246,17 +470,24 @@ int stream_pass(Solver &S, const double *h, const double *dc, int n, F &&fn)
     return RISP_OK;
 }
 
-// store device vectors src[0, n) as subspace vectors [k, k+n) of (hV|hW, dVc|dWc): always to the pinned host array (side
-// stream, after the compute stream has produced them), and to the device cache where it reaches
-int store_vectors(Solver &S, double *h, double *dc, int k, const double *src, int n)
+// store device vectors src[0, n) as subspace vectors [k, k+n): into the device cache while it reaches, beyond it into the
+// pinned host store (side stream, after the compute stream has produced them)
+int store_vectors(Solver &S, bool isW, double *dc, int k, const double *src, int n)
 {
     risp_ctx *ctx = S.ctx;
+    const int nc = std::max(0, std::min(n, S.ncache - k));       // vectors that land in the device cache
+    if (nc > 0) RISP_CUDA_TRY(cudaMemcpyAsync(dc + (long long)k * S.dim, src, (size_t)nc * S.dim * 8, cudaMemcpyDeviceToDevice, S.st));
+    if (nc == n) return RISP_OK;
     RISP_CUDA_TRY(cudaEventRecord(S.evReady, S.st));
     RISP_CUDA_TRY(cudaStreamWaitEvent(ctx->side, S.evReady, 0));
-    RISP_CUDA_TRY(cudaMemcpyAsync(h + (long long)k * S.dim, src, (size_t)n * S.dim * 8, cudaMemcpyDeviceToHost, ctx->side));
-    S.bytes_d2h += (double)n * S.dim * 8;
-    const int nc = std::max(0, std::min(n, S.ncache - k));
-    if (nc > 0) RISP_CUDA_TRY(cudaMemcpyAsync(dc + (long long)k * S.dim, src, (size_t)nc * S.dim * 8, cudaMemcpyDeviceToDevice, S.st));
+    for (int done = nc; done < n;) {
+        const int i = k + done - S.ncache, seg = std::min(n - done, HostStore::CHV - i % HostStore::CHV);
+        double *h = S.host.ptr(isW, i);
+        if (!h) { risp_set_error(ctx, "risp_tda_solve: pinned host allocation of the subspace failed"); return RISP_ENOMEM; }
+        RISP_CUDA_TRY(cudaMemcpyAsync(h, src + (long long)done * S.dim, (size_t)seg * S.dim * 8, cudaMemcpyDeviceToHost, ctx->side));
+        S.bytes_d2h += (double)seg * S.dim * 8;
+        done += seg;
+    }
     return RISP_OK;
 }
 
@@ -287,8 +518,6 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
     S.cap = (int)std::min<long long>(max_sub, by_budget);
     S.cap = std::max(S.cap, std::max(n_guess, 2 * nroots));
     const int slots = S.cap + nroots;              // room to append one more block before the restart decision
-    RISP_CUDA_TRY(cudaHostAlloc((void **)&S.hV, (size_t)slots * dim * 8, cudaHostAllocDefault));
-    RISP_CUDA_TRY(cudaHostAlloc((void **)&S.hW, (size_t)slots * dim * 8, cudaHostAllocDefault));
     const int nbmax = std::max(n_guess, nroots);
     auto DA = [&](double *&p, size_t n) -> int { RISP_CUDA_TRY(cudaMalloc((void **)&p, n * 8)); return RISP_OK; };
     int rc;
@@ -297,8 +526,9 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
         (rc = DA(S.dChunk[0], (size_t)S.CH * dim)) || (rc = DA(S.dChunk[1], (size_t)S.CH * dim)))
         return rc;
     const int small = std::max(slots, 64);
-    const int nzmax = (int)(dim / 16384) + 2;
-    if ((rc = DA(S.dCoef, (size_t)small * small)) || (rc = DA(S.dPart, std::max((size_t)nzmax * 64 * 64, (size_t)RISP_MAX_ROOTS * 256))) || (rc = DA(S.dSmall, (size_t)64 * 64 + 4096)) ||
+    S.slice = dim > (1 << 20) ? 4096 : 16384;      // enough slices to give every SM a tile
+    const int nzmax = (int)(dim / S.slice) + 2;
+    if ((rc = DA(S.dCoef, (size_t)small * small)) || (rc = DA(S.dPart, std::max((size_t)nzmax * 128 * 64, (size_t)RISP_MAX_ROOTS * 256))) || (rc = DA(S.dSmall, (size_t)128 * 64 + 4096)) ||
         (rc = DA(S.dTheta, (size_t)RISP_MAX_ROOTS)))
         return rc;
     RISP_CUDA_TRY(cudaMalloc((void **)&S.dSrc, RISP_MAX_ROOTS * sizeof(int)));
@@ -322,11 +552,13 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
             RISP_CUDA_TRY(cudaMalloc((void **)&S.dVc, (size_t)S.ncache * dim * 8));
             RISP_CUDA_TRY(cudaMalloc((void **)&S.dWc, (size_t)S.ncache * dim * 8));
         }
+        // vectors beyond the cache live in pinned host memory only; nothing is pinned when everything fits in HBM
+        if (slots > S.ncache) S.host.start(ctx->device, dim, slots - S.ncache);
     }
 
     auto cleanup = [&]() {
         cudaDeviceSynchronize();
-        cudaFreeHost(S.hV); cudaFreeHost(S.hW);
+        S.host.finish();
         double *bufs[] = {S.dB, S.dWB, S.dX, S.dAX, S.dRes, S.dT, S.dChunk[0], S.dChunk[1], S.dCoef, S.dPart, S.dSmall, S.dTheta};
         for (double *b : bufs) if (b) cudaFree(b);
         if (S.dSrc) cudaFree(S.dSrc);
@@ -365,6 +597,7 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
     bool converged = false;
     S.k = 0;
 
+    const double sec_alloc = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
     for (int it = 1; it <= max_iter; ++it) {
         iterations = it;
         // ---- W_B = A B
@@ -383,7 +616,7 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
         {
             const int k = S.k;
             std::vector<double> blk;
-            SOLVE_TRY(stream_pass(S, S.hV, S.dVc, k, [&](const double *Vc, int first, int cnt) -> int {
+            SOLVE_TRY(stream_pass(S, false, S.dVc, k, [&](const double *Vc, int first, int cnt) -> int {
                 int r = gram(S, Vc, cnt, S.dWB, nb, blk);
                 if (r) return r;
                 for (int i = 0; i < cnt; ++i)
@@ -394,8 +627,8 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
             for (int i = 0; i < nb; ++i)
                 for (int j = 0; j < nb; ++j) G[(size_t)(k + i) * ldg + k + j] = 0.5 * (blk[(size_t)i * nb + j] + blk[(size_t)j * nb + i]);
             // append B, W_B to the pinned host subspace (side stream)
-            SOLVE_TRY(store_vectors(S, S.hV, S.dVc, k, S.dB, nb));
-            SOLVE_TRY(store_vectors(S, S.hW, S.dWc, k, S.dWB, nb));
+            SOLVE_TRY(store_vectors(S, false, S.dVc, k, S.dB, nb));
+            SOLVE_TRY(store_vectors(S, true, S.dWc, k, S.dWB, nb));
             RISP_CUDA_TRY(cudaEventRecord(S.evD2H, ctx->side));
             S.k += nb;
             sub_max = std::max(sub_max, S.k);
@@ -406,7 +639,7 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
             std::vector<double> a((size_t)k * k), w;
             for (int i = 0; i < k; ++i)
                 for (int j = 0; j < k; ++j) a[(size_t)i * k + j] = G[(size_t)i * ldg + j];
-            sym_eig(a, k, w, yv);
+            sym_eig_lowest(a, k, nroots, w, yv);
             for (int j = 0; j < nroots; ++j) theta[j] = w[j];
         }
         // ---- X = V y, AX = W y (stream V and W; needs the appended block on the host)
@@ -414,7 +647,7 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
         for (int pass = 0; pass < 2; ++pass) {
             double *dst = pass == 0 ? S.dX : S.dAX;
             bool first_chunk = true;
-            SOLVE_TRY(stream_pass(S, pass == 0 ? S.hV : S.hW, pass == 0 ? S.dVc : S.dWc, k, [&](const double *Vc, int first, int cnt) -> int {
+            SOLVE_TRY(stream_pass(S, pass != 0, pass == 0 ? S.dVc : S.dWc, k, [&](const double *Vc, int first, int cnt) -> int {
                 std::vector<double> coef((size_t)nroots * cnt);
                 for (int j = 0; j < nroots; ++j)
                     for (int i = 0; i < cnt; ++i) coef[(size_t)j * cnt + i] = yv[(size_t)(first + i) * k + j];
@@ -443,8 +676,8 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
         if (it == max_iter) break;
         // ---- restart from the Ritz vectors when the next block would not fit
         if (k + (int)src.size() > S.cap) {
-            SOLVE_TRY(store_vectors(S, S.hV, S.dVc, 0, S.dX, nroots));
-            SOLVE_TRY(store_vectors(S, S.hW, S.dWc, 0, S.dAX, nroots));
+            SOLVE_TRY(store_vectors(S, false, S.dVc, 0, S.dX, nroots));
+            SOLVE_TRY(store_vectors(S, true, S.dWc, 0, S.dAX, nroots));
             RISP_CUDA_TRY(cudaEventRecord(S.evD2H, ctx->side));
             RISP_CUDA_TRY(cudaEventSynchronize(S.evD2H));
             std::fill(G.begin(), G.end(), 0.0);
@@ -475,7 +708,7 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
         std::vector<double> norms;
         SOLVE_TRY(normalise_rows(S.dT, nb, norms));
         // ---- orthogonalise against V: per streamed chunk, two projections (block Gram-Schmidt with re-orthogonalisation)
-        SOLVE_TRY(stream_pass(S, S.hV, S.dVc, S.k, [&](const double *Vc, int first, int cnt) -> int {
+        SOLVE_TRY(stream_pass(S, false, S.dVc, S.k, [&](const double *Vc, int first, int cnt) -> int {
             for (int rep = 0; rep < 2; ++rep) {
                 std::vector<double> c;
                 int r = gram(S, S.dT, nb, Vc, cnt, c);       // c[j][i] = t_j . v_i
@@ -546,7 +779,7 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
         info->iterations = iterations; info->restarts = restarts; info->n_sigma = n_sigma; info->converged = converged ? 1 : 0;
         for (int j = 0; j < nroots; ++j) info->resid[j] = rn[j];
         info->sec_total = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
-        info->sec_matvec = sec_mv; info->sec_subspace = info->sec_total - sec_mv;
+        info->sec_matvec = sec_mv; info->sec_subspace = info->sec_total - sec_mv - sec_alloc; info->sec_alloc = sec_alloc;
         info->bytes_h2d = S.bytes_h2d; info->bytes_d2h = S.bytes_d2h; info->subspace_max = sub_max; info->cached_vectors = S.ncache;
     }
     cleanup();
@@ -560,6 +793,17 @@ extern "C" int risp_debug_sym_eig(int n, const double *a_in, double *w_out, doub
     if (n <= 0 || !a_in || !w_out || !z_out) return RISP_EINVAL;
     std::vector<double> a(a_in, a_in + (size_t)n * n), w, z;
     sym_eig(a, n, w, z);
+    std::memcpy(w_out, w.data(), (size_t)n * 8);
+    std::memcpy(z_out, z.data(), (size_t)n * n * 8);
+    return RISP_OK;
+}
+
+// Debug export: the lowest-nv variant used inside the Davidson loop.
+extern "C" int risp_debug_sym_eig_lowest(int n, int nv, const double *a_in, double *w_out, double *z_out)
+{
+    if (n <= 0 || nv <= 0 || !a_in || !w_out || !z_out) return RISP_EINVAL;
+    std::vector<double> a(a_in, a_in + (size_t)n * n), w, z;
+    sym_eig_lowest(a, n, nv, w, z);
     std::memcpy(w_out, w.data(), (size_t)n * 8);
     std::memcpy(z_out, z.data(), (size_t)n * n * 8);
     return RISP_OK;

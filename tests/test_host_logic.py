@@ -67,6 +67,28 @@ def test_host_eigensolver_against_lapack(lib, n):
     assert np.abs(A @ z - z * w[None]).max() < 1e-11 * max(1.0, np.abs(A).max()) * n
 
 
+@pytest.mark.parametrize("n", [1, 2, 5, 40, 150, 315])
+def test_host_lowest_eigenpairs_against_lapack(lib, n):
+    """the Davidson loop's projected eigenproblem: lowest nv pairs by inverse iteration, incl. clustered / degenerate spectra"""
+    rng = np.random.default_rng(100 + n)
+    A = rng.normal(size=(n, n)); A = A + A.T
+    if n == 40:
+        Q, _ = np.linalg.qr(rng.normal(size=(n, n)))
+        A = Q @ np.diag(np.repeat(np.arange(8.0), 5) + 1e-9 * rng.normal(size=n)) @ Q.T
+        A = 0.5 * (A + A.T)
+    if n == 315:                                  # Davidson-like: dominant diagonal with meV-spaced lowest levels
+        A = np.diag(np.sort(rng.uniform(0.15, 2.0, size=n))) + 1e-3 * A
+        A[np.arange(15), np.arange(15)] = 0.15 + 3e-5 * np.arange(15)
+    nv = min(n, 15)
+    w = np.zeros(n); z = np.zeros((n, n))
+    assert lib.risp_debug_sym_eig_lowest(n, nv, A.ctypes.data, w.ctypes.data, z.ctypes.data) == 0
+    scale = max(1.0, np.abs(A).max()) * n
+    assert np.abs(w - np.linalg.eigvalsh(A)).max() < 1e-12 * scale
+    Z = z[:, :nv]
+    assert np.abs(Z.T @ Z - np.eye(nv)).max() < 1e-10
+    assert np.abs(A @ Z - Z * w[None, :nv]).max() < 1e-11 * scale
+
+
 _WORKER = r"""
 import os, sys, numpy as np, torch, torch.distributed as dist
 sys.path.insert(0, sys.argv[1])
