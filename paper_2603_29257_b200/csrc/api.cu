@@ -16,7 +16,7 @@ extern "C" void risp_destroy(risp_ctx *ctx)
     for (auto b : bufs) if (*b) cudaFree(*b);
     if (ctx->h_TijP) cudaFreeHost(ctx->h_TijP);
     if (ctx->h_TabP) cudaFreeHost(ctx->h_TabP);
-    for (int c = 0; c < 6; ++c) if (ctx->cls[c].d_pairs) cudaFree(ctx->cls[c].d_pairs);
+    for (int c = 0; c < 6; ++c) { if (ctx->cls[c].d_pairs) cudaFree(ctx->cls[c].d_pairs); if (ctx->cls[c].d_permB) cudaFree(ctx->cls[c].d_permB); }
     if (ctx->d_prims) cudaFree(ctx->d_prims);
     if (ctx->d_cenJ) cudaFree(ctx->d_cenJ);
     if (ctx->d_cenK) cudaFree(ctx->d_cenK);
@@ -195,7 +195,7 @@ extern "C" int risp_get_stage(risp_ctx *ctx, int32_t which, const int64_t *sel, 
         RISP_CUDA_TRY(cudaMalloc((void **)&tmp, n * 8));
         RISP_CUDA_TRY(cudaMemset(tmp, 0, n * 8));
         for (int c = 0; c < 6; ++c)
-            RISP_CUDA_TRY(risp_e0_to_U(ctx->cls[c], 0, ctx->cls[c].npairs, 1, (int)sel[0], 0, ctx->ldao, (long long)n, 1, ctx->w_dbar, tmp, 0));
+            RISP_CUDA_TRY(risp_e0_to_U(ctx->cls[c], 0, ctx->cls[c].npairs, 1, (int)sel[0], 0, ctx->ldao, (long long)n, 0, ctx->w_dbar, tmp, 0));
         RISP_CUDA_TRY(cudaMemcpy2D(out, (size_t)ctx->nao * 8, tmp, (size_t)ctx->ldao * 8, (size_t)ctx->nao * 8, ctx->nao, cudaMemcpyDeviceToHost));
         cudaFree(tmp);
         return RISP_OK;

@@ -13,6 +13,8 @@ struct PairClass {                 // kept shell pairs of one (la >= lb) class, 
     long long e_off;               // first e0 row of this class in D-bar / U-bar
     int chunk, nchunks, chunk_base; // pass-1 pair chunking (chunk_base: global index of the class's first chunk)
     std::vector<int> h_aoA;        // host copy of sp.aoA (ascending): row panels of the J transforms are pair ranges
+    int *d_permB = nullptr;        // pair indices sorted by sp.aoB (device), and the sorted aoB values (host)
+    std::vector<int> h_aoB;
 };
 
 // Plan of one risp_matvec (sizes depend on m and on what the HBM budget leaves after the K tensors).
@@ -67,7 +69,7 @@ struct risp_ctx {
     int force_mj = 0, force_prow = 0, force_pc = 0; // debug overrides (risp_debug_force_plan)
     double *w_arena = nullptr;    // J phase: Y [mj][nocc][ldao], D/U panel [mj][prow][ldao];  K phase: X', K', M, expanded T chunk
     double *w_dbar = nullptr;     // [e_rows][MS]     e0-space density, reused for U-bar
-    double *w_Rpart = nullptr, *w_R = nullptr, *w_Rt = nullptr, *w_Rtmp = nullptr;
+    double *w_Rpart = nullptr, *w_R = nullptr, *w_Rt = nullptr, *w_Rtmp = nullptr, *w_RtC = nullptr;
     double *w_J = nullptr;        // [m][nocc][nvir], only with RISP_FLAG_KEEP_STAGES
     double *w_stage[2] = {nullptr, nullptr};      // packed host-resident T chunks in flight
     double *w_Xin = nullptr, *w_Sout = nullptr;   // staging for risp_matvec_host
@@ -87,16 +89,18 @@ struct risp_ctx {
 cudaError_t risp_eri_fill(int la, int lb, bool hasp, bool erf_op, const risp_eri::ShellPair *pairs, int npairs, const risp_eri::PrimPair *prims,
                           const risp_eri::AuxCentre *cen, int ncen, risp_eri::OpParams op, const double *boys_tab, double *out,
                           long long stride_q, long long ld, int mirror, cudaStream_t st);
-// D (rows [r0, ...), leading dimension ld, vector stride mstride) -> e0 space, lanes [lane0, lane0 + mj) of pairs [p0, p1).
-// presym: D already holds D + D^T (diagonal shell pairs are then halved).
-cudaError_t risp_dens_to_e0(const PairClass &pc, int p0, int p1, int mj, int lane0, int r0, long long ld, long long mstride, int presym,
+// D rows [r0, ...) (leading dimension ld, vector stride mstride) -> e0 space, lanes [lane0, lane0 + mj).  mode 0: dense, pairs
+// [p0, p1) of the aoA-sorted list; mode 1: += from the rows of shell A; mode 2: += from the rows of shell B, [p0, p1) of the aoB-sorted list
+cudaError_t risp_dens_to_e0(const PairClass &pc, int p0, int p1, int mj, int lane0, int r0, long long ld, long long mstride, int mode,
                             const double *D, double *dbar, cudaStream_t st);
-// e0 space -> U rows [r0, ...).  mirror: also write the transposed block (dense single panel); else diagonal shell pairs are halved.
-cudaError_t risp_e0_to_U(const PairClass &pc, int p0, int p1, int mj, int lane0, int r0, long long ld, long long mstride, int mirror,
+// e0 space -> U rows [r0, ...), same modes (0: block and mirror image; 1: block at the rows of A; 2: transposed block at the rows of B)
+cudaError_t risp_e0_to_U(const PairClass &pc, int p0, int p1, int mj, int lane0, int r0, long long ld, long long mstride, int mode,
                          const double *ubar, double *U, cudaStream_t st);
 cudaError_t risp_j_pass1(const PairClass &pc, const risp_eri::PrimPair *prims, const risp_eri::AuxCentre *cen, int ncen, int ncen_pad,
                          const double *boys_tab, const double *dbar, double *Rpart, cudaStream_t st);
 cudaError_t risp_j_reduce_R(const double *Rpart, int nchunks, const risp_eri::AuxCentre *cen, int ncen, int ncen_pad, double *R, cudaStream_t st);
+// R~ [nauxJ][MS] -> by centre [ceil32(ncen)*4][MS] (zero padded); pass 2 takes the by-centre array
+cudaError_t risp_rt_by_centre(const double *Rt, const risp_eri::AuxCentre *cen, int ncen, double *RtC, cudaStream_t st);
 cudaError_t risp_j_pass2(const PairClass &pc, const risp_eri::PrimPair *prims, const risp_eri::AuxCentre *cen, int ncen, const double *boys_tab,
                          const double *Rt, double *ubar, cudaStream_t st);
 

@@ -58,91 +58,138 @@ __global__ void __launch_bounds__(128) eri_fill_kernel(const ShellPair *__restri
 }
 
 // ------------------------------------------------------------------------------------------------- density -> e0
-// D: rows [r0, ...) of the AO matrices of mj trial vectors (leading dimension ld, vector stride mstride).
-// presym = 0: D is the plain (unsymmetrised) density with all rows present (r0 = 0); the lower-triangular pair takes
-//             D_ab + D_ba (reading G13).  presym = 1: the panel already holds D + D^T; diagonal shell pairs take half.
+// D: rows [r0, ...) of the plain (unsymmetrised) AO density matrices of mj trial vectors (leading dimension ld, vector stride
+// mstride).  Only sym(D) matters for a lower-triangular pair (reading G13): D-bar(A,B) = adjoint[D_AB + D_BA^T].
+//   mode 0  all rows present (r0 = 0): both blocks read here, D-bar written.
+//   mode 1  panel holds the rows of shell A:  D-bar += adjoint[D_AB]           (pairs [p0, p1) of the aoA-sorted list)
+//   mode 2  panel holds the rows of shell B:  D-bar += adjoint[D_BA^T], A != B (pairs perm[p0 .. p1) of the aoB-sorted list)
+// Modes 1 and 2 visit every pair once each over all panels; D-bar is zeroed before.
 template <int LA, int LB>
-__global__ void __launch_bounds__(128) dens_to_e0_kernel(const ShellPair *__restrict__ pairs, int p0, int p1, long long e_off, int mj, int lane0,
-                                                         int r0, long long ld, long long mstride, int presym,
+__global__ void __launch_bounds__(128) dens_to_e0_kernel(const ShellPair *__restrict__ pairs, const int *__restrict__ perm, int p0, int p1,
+                                                         long long e_off, int mj, int lane0, int r0, long long ld, long long mstride, int mode,
                                                          const double *__restrict__ D, double *__restrict__ dbar)
 {
     constexpr int NE = ne_of(LA, LB);
     const int mi = threadIdx.x;
-    const int pi = p0 + blockIdx.x * blockDim.y + threadIdx.y;
+    int pi = p0 + blockIdx.x * blockDim.y + threadIdx.y;
     if (pi >= p1 || mi >= mj) return;
+    if (mode == 2) pi = perm[pi];
     const ShellPair sp = pairs[pi];
+    const bool diag = sp.shA == sp.shB;
+    if (mode == 2 && diag) return;
     const double *Dm = D + (long long)mi * mstride;
     double d[2 * LA + 1][2 * LB + 1];
-    const bool diag = sp.shA == sp.shB;
 #pragma unroll
     for (int i = 0; i < 2 * LA + 1; ++i)
 #pragma unroll
         for (int j = 0; j < 2 * LB + 1; ++j) {
-            double v = Dm[(long long)(sp.aoA - r0 + i) * ld + sp.aoB + j];
-            if (presym) { if (diag) v *= 0.5; }
-            else if (!diag) v += Dm[(long long)(sp.aoB + j) * ld + sp.aoA + i];
+            double v;
+            if (mode == 2) v = Dm[(long long)(sp.aoB - r0 + j) * ld + sp.aoA + i];
+            else {
+                v = Dm[(long long)(sp.aoA - r0 + i) * ld + sp.aoB + j];
+                if (mode == 0 && !diag) v += Dm[(long long)(sp.aoB + j) * ld + sp.aoA + i];
+            }
             d[i][j] = v;
         }
     double out[NE];
     sph_to_e0_adjoint<LA, LB>(d, sp.ABx, sp.ABy, sp.ABz, out);
+    double *dst = dbar + (e_off + (long long)pi * NE) * MS + lane0 + mi;
 #pragma unroll
-    for (int e = 0; e < NE; ++e) dbar[(e_off + (long long)pi * NE + e) * MS + lane0 + mi] = out[e];
+    for (int e = 0; e < NE; ++e) {
+        if (mode == 0) dst[(long long)e * MS] = out[e];
+        else dst[(long long)e * MS] += out[e];
+    }
 }
 
-// mirror = 1 (single dense panel, r0 = 0): write the block and its transpose.  mirror = 0: write the block at rows aoA - r0 only,
-// diagonal shell pairs halved, so that U = P + P^T.
+// U-bar -> rows [r0, ...) of the symmetric AO matrix U.
+//   mode 0  dense (r0 = 0): the block and its transpose.   mode 1  block at the rows of shell A (aoA-sorted range).
+//   mode 2  transposed block at the rows of shell B, A != B (aoB-sorted range through perm).
 template <int LA, int LB>
-__global__ void __launch_bounds__(128) e0_to_U_kernel(const ShellPair *__restrict__ pairs, int p0, int p1, long long e_off, int mj, int lane0,
-                                                      int r0, long long ld, long long mstride, int mirror,
+__global__ void __launch_bounds__(128) e0_to_U_kernel(const ShellPair *__restrict__ pairs, const int *__restrict__ perm, int p0, int p1,
+                                                      long long e_off, int mj, int lane0, int r0, long long ld, long long mstride, int mode,
                                                       const double *__restrict__ ubar, double *__restrict__ U)
 {
     constexpr int NE = ne_of(LA, LB);
     const int mi = threadIdx.x;
-    const int pi = p0 + blockIdx.x * blockDim.y + threadIdx.y;
+    int pi = p0 + blockIdx.x * blockDim.y + threadIdx.y;
     if (pi >= p1 || mi >= mj) return;
+    if (mode == 2) pi = perm[pi];
     const ShellPair sp = pairs[pi];
+    const bool diag = sp.shA == sp.shB;
+    if (mode == 2 && diag) return;
     double e0[NE];
 #pragma unroll
     for (int e = 0; e < NE; ++e) e0[e] = ubar[(e_off + (long long)pi * NE + e) * MS + lane0 + mi];
     double blk[2 * LA + 1][2 * LB + 1];
     e0_to_sph<LA, LB>(e0, sp.ABx, sp.ABy, sp.ABz, blk);
     double *Um = U + (long long)mi * mstride;
-    const bool diag = sp.shA == sp.shB;
-    const double f = (!mirror && diag) ? 0.5 : 1.0;
 #pragma unroll
     for (int i = 0; i < 2 * LA + 1; ++i)
 #pragma unroll
         for (int j = 0; j < 2 * LB + 1; ++j) {
-            Um[(long long)(sp.aoA - r0 + i) * ld + sp.aoB + j] = f * blk[i][j];
-            if (mirror && !diag) Um[(long long)(sp.aoB + j) * ld + sp.aoA + i] = blk[i][j];
+            if (mode != 2) Um[(long long)(sp.aoA - r0 + i) * ld + sp.aoB + j] = blk[i][j];
+            if (mode == 2 || (mode == 0 && !diag)) Um[(long long)(sp.aoB - r0 + j) * ld + sp.aoA + i] = blk[i][j];
         }
 }
 
 // ------------------------------------------------------------------------------------------------- J passes
 constexpr int JW = 4;   // warps per CTA
 
+// Both passes are bound by FP64 arithmetic only if the global loads (primitive pairs, D-bar, R~) are in flight early: at 8
+// warps per SM nothing else hides their latency (ncu: long-scoreboard stalls on the first use of every such load).  So the
+// next primitive pair is fetched while the current one is processed, and the contraction operands are loaded in batches.
 template <int LA, int LB>
 __device__ __forceinline__ void park_integrals(double *__restrict__ g, int lane, bool valid, const ShellPair &sp,
                                                const PrimPair *__restrict__ prims, const AuxCentre &ax, const double *__restrict__ boys_tab)
 {
     constexpr int NE = ne_of(LA, LB);
+    constexpr bool REG = NE * 4 <= 36;          // small classes accumulate the contraction over primitives in registers
+    if constexpr (REG) {
+        double a[NE * 4];
 #pragma unroll
-    for (int k = 0; k < NE * 4; ++k) g[k * 32 + lane] = 0.0;
-    if (valid) {
-        OpParams op{1.0, 0.0, 0.0};
-        for (int k = 0; k < sp.npp; ++k) {
-            const PrimPair pp = prims[sp.ppoff + k];
-            eri_e0_prim<LA, LB, true, false>(pp, sp.Ax, sp.Ay, sp.Az, ax, op, boys_tab,
-                                             [&](int e, int c, double v) { g[(e * 4 + c) * 32 + lane] += v; });
+        for (int k = 0; k < NE * 4; ++k) a[k] = 0.0;
+        if (valid) {
+            OpParams op{1.0, 0.0, 0.0};
+            PrimPair pp = prims[sp.ppoff];
+            for (int k = 0; k < sp.npp; ++k) {
+                const PrimPair nxt = prims[sp.ppoff + min(k + 1, sp.npp - 1)];
+                eri_e0_prim<LA, LB, true, false>(pp, sp.Ax, sp.Ay, sp.Az, ax, op, boys_tab, [&](int e, int c, double v) { a[e * 4 + c] += v; });
+                pp = nxt;
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < NE * 4; ++k) g[k * 32 + lane] = a[k];
+    } else {
+#pragma unroll
+        for (int k = 0; k < NE * 4; ++k) g[k * 32 + lane] = 0.0;
+        if (valid) {
+            OpParams op{1.0, 0.0, 0.0};
+            PrimPair pp = prims[sp.ppoff];
+            for (int k = 0; k < sp.npp; ++k) {
+                const PrimPair nxt = prims[sp.ppoff + min(k + 1, sp.npp - 1)];
+                eri_e0_prim<LA, LB, true, false>(pp, sp.Ax, sp.Ay, sp.Az, ax, op, boys_tab,
+                                                 [&](int e, int c, double v) { g[(e * 4 + c) * 32 + lane] += v; });
+                pp = nxt;
+            }
         }
     }
+}
+
+// R~ by centre: RtC[(centre*4 + comp)*MS + lane], zero where a centre has no s or no p function and for the padding centres up
+// to a multiple of 32 -- pass 2 then reads its contraction operand without the (qs, qp) indirection
+__global__ void rt_by_centre_kernel(const double *__restrict__ Rt, const AuxCentre *__restrict__ cen, int ncen, double *__restrict__ RtC)
+{
+    const int lane = threadIdx.x, k = blockIdx.x, ci = k >> 2, c = k & 3;
+    int q = -1;
+    if (ci < ncen) q = c == 0 ? cen[ci].qs : (cen[ci].qp < 0 ? -1 : cen[ci].qp + c - 1);
+    RtC[(long long)k * MS + lane] = q >= 0 ? Rt[(long long)q * MS + lane] : 0.0;
 }
 
 // pass 2: one pair per warp, 32 aux centres per step.  ubar[(e_off + pair*NE + e)*MS + mi]
 template <int LA, int LB>
 __global__ void __launch_bounds__(32 * JW) j_pass2_kernel(const ShellPair *__restrict__ pairs, int npairs, const PrimPair *__restrict__ prims,
                                                           const AuxCentre *__restrict__ cen, int ncen, const double *__restrict__ boys_tab,
-                                                          const double *__restrict__ Rt, long long e_off, double *__restrict__ ubar)
+                                                          const double *__restrict__ RtC, long long e_off, double *__restrict__ ubar)
 {
     constexpr int NE = ne_of(LA, LB);
     extern __shared__ double smem[];
@@ -154,29 +201,28 @@ __global__ void __launch_bounds__(32 * JW) j_pass2_kernel(const ShellPair *__res
     double acc[NE];
 #pragma unroll
     for (int e = 0; e < NE; ++e) acc[e] = 0.0;
+    AuxCentre ax = cen[min(lane, ncen - 1)];
     for (int c0 = 0; c0 < ncen; c0 += 32) {
-        const int ci = c0 + lane;
-        const bool valid = ci < ncen;
-        const AuxCentre ax = cen[valid ? ci : 0];
+        const bool valid = c0 + lane < ncen;
+        const AuxCentre ax_next = cen[min(c0 + 32 + lane, ncen - 1)];
         park_integrals<LA, LB>(g, lane, valid, sp, prims, ax, boys_tab);
+        ax = ax_next;
         __syncwarp();
-        const int nc = min(32, ncen - c0);
-        for (int s = 0; s < nc; s += 2) {
-            double rt[2][4];
+        const double *rc = RtC + (long long)c0 * 4 * MS + lane;
+#pragma unroll 2
+        for (int s = 0; s < 32; s += 4) {           // padding centres carry zero integrals and zero R~
+            double rt[4][4];
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const bool ok = s + h < nc;
-                const int qs = ok ? __ldg(&cen[c0 + s + h].qs) : -1, qp = ok ? __ldg(&cen[c0 + s + h].qp) : -1;
-                rt[h][0] = qs >= 0 ? Rt[(long long)qs * MS + lane] : 0.0;
+            for (int h = 0; h < 4; ++h)
 #pragma unroll
-                for (int d = 0; d < 3; ++d) rt[h][1 + d] = qp >= 0 ? Rt[(long long)(qp + d) * MS + lane] : 0.0;
-            }
+                for (int c = 0; c < 4; ++c) rt[h][c] = rc[(long long)((s + h) * 4 + c) * MS];
 #pragma unroll
             for (int e = 0; e < NE; ++e)
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
-                    const double2 gg = *reinterpret_cast<const double2 *>(&g[(e * 4 + c) * 32 + s]);
-                    acc[e] = fma(gg.x, rt[0][c], fma(gg.y, rt[1][c], acc[e]));
+                    const double2 g0 = *reinterpret_cast<const double2 *>(&g[(e * 4 + c) * 32 + s]);
+                    const double2 g1 = *reinterpret_cast<const double2 *>(&g[(e * 4 + c) * 32 + s + 2]);
+                    acc[e] = fma(g0.x, rt[0][c], fma(g0.y, rt[1][c], fma(g1.x, rt[2][c], fma(g1.y, rt[3][c], acc[e]))));
                 }
         }
         __syncwarp();
@@ -194,6 +240,7 @@ __global__ void __launch_bounds__(32 * JW) j_pass1_kernel(const ShellPair *__res
                                                           long long e_off, double *__restrict__ Rpart)
 {
     constexpr int NE = ne_of(LA, LB);
+    constexpr bool PRE = 4 * NE <= 12;      // D-bar of the step's four pairs fetched before the integrals are generated
     extern __shared__ double smem[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     double *g = smem + (size_t)w * NE * 4 * 32;
@@ -204,18 +251,33 @@ __global__ void __launch_bounds__(32 * JW) j_pass1_kernel(const ShellPair *__res
     double acc[32];
 #pragma unroll
     for (int k = 0; k < 32; ++k) acc[k] = 0.0;
+    ShellPair sp = pairs[min(p_begin + w * 4 + slot, p_end - 1)];
     for (int pg = p_begin + w * 4; pg < p_end; pg += JW * 4) {
         const int pi = pg + slot;
         const bool valid = cvalid && pi < p_end;
-        const ShellPair sp = pairs[pi < p_end ? pi : p_begin];
-        park_integrals<LA, LB>(g, lane, valid, sp, prims, ax, boys_tab);
-        __syncwarp();
+        const ShellPair sp_next = pairs[min(pi + JW * 4, p_end - 1)];
+        const double *db = dbar + (e_off + (long long)pg * NE) * MS + lane;
         const int ns = min(4, p_end - pg);
-        for (int s = 0; s < ns; ++s) {
-            const double *db = dbar + (e_off + (long long)(pg + s) * NE) * MS + lane;
+        double dpre[PRE ? 4 * NE : 1];
+        if constexpr (PRE) {
+#pragma unroll
+            for (int k = 0; k < 4 * NE; ++k) dpre[k] = (k / NE < ns) ? db[(long long)k * MS] : 0.0;
+        }
+        park_integrals<LA, LB>(g, lane, valid, sp, prims, ax, boys_tab);
+        sp = sp_next;
+        __syncwarp();
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+            if (s >= ns) break;
+            double dv[NE];
 #pragma unroll
             for (int e = 0; e < NE; ++e) {
-                const double d = db[(long long)e * MS];
+                if constexpr (PRE) dv[e] = dpre[s * NE + e];
+                else dv[e] = db[(long long)(s * NE + e) * MS];
+            }
+#pragma unroll
+            for (int e = 0; e < NE; ++e) {
+                const double d = dv[e];
 #pragma unroll
                 for (int c = 0; c < 4; ++c)
 #pragma unroll
@@ -228,10 +290,9 @@ __global__ void __launch_bounds__(32 * JW) j_pass1_kernel(const ShellPair *__res
         }
         __syncwarp();
     }
-    // cross-warp reduction (fixed order -> deterministic), reuse the parking area
+    // cross-warp reduction (fixed order -> deterministic) in a dedicated region after the parking area
     __syncthreads();
-    double *red = smem;   // [JW][32][32], NE*4*32 >= 32*32 only if NE >= 8, so use a dedicated region after the parking area
-    red = smem + (size_t)JW * NE * 4 * 32;
+    double *red = smem + (size_t)JW * NE * 4 * 32;     // [JW][32][32]
 #pragma unroll
     for (int k = 0; k < 32; ++k) red[(w * 32 + k) * 32 + lane] = acc[k];
     __syncthreads();
@@ -317,26 +378,26 @@ cudaError_t risp_eri_fill(int la, int lb, bool hasp, bool erf_op, const ShellPai
     return cudaGetLastError();
 }
 
-cudaError_t risp_dens_to_e0(const PairClass &pc, int p0, int p1, int mj, int lane0, int r0, long long ld, long long mstride, int presym,
+cudaError_t risp_dens_to_e0(const PairClass &pc, int p0, int p1, int mj, int lane0, int r0, long long ld, long long mstride, int mode,
                             const double *D, double *dbar, cudaStream_t st)
 {
     if (p1 <= p0) return cudaSuccess;
     dim3 block(32, 4), grid((p1 - p0 + 3) / 4);
     dispatch_class(pc.la, pc.lb, [&](auto LA, auto LB) {
-        dens_to_e0_kernel<decltype(LA)::value, decltype(LB)::value><<<grid, block, 0, st>>>(pc.d_pairs, p0, p1, pc.e_off, mj, lane0, r0, ld, mstride,
-                                                                                            presym, D, dbar);
+        dens_to_e0_kernel<decltype(LA)::value, decltype(LB)::value><<<grid, block, 0, st>>>(pc.d_pairs, pc.d_permB, p0, p1, pc.e_off, mj, lane0, r0, ld,
+                                                                                            mstride, mode, D, dbar);
     });
     return cudaGetLastError();
 }
 
-cudaError_t risp_e0_to_U(const PairClass &pc, int p0, int p1, int mj, int lane0, int r0, long long ld, long long mstride, int mirror,
+cudaError_t risp_e0_to_U(const PairClass &pc, int p0, int p1, int mj, int lane0, int r0, long long ld, long long mstride, int mode,
                          const double *ubar, double *U, cudaStream_t st)
 {
     if (p1 <= p0) return cudaSuccess;
     dim3 block(32, 4), grid((p1 - p0 + 3) / 4);
     dispatch_class(pc.la, pc.lb, [&](auto LA, auto LB) {
-        e0_to_U_kernel<decltype(LA)::value, decltype(LB)::value><<<grid, block, 0, st>>>(pc.d_pairs, p0, p1, pc.e_off, mj, lane0, r0, ld, mstride,
-                                                                                         mirror, ubar, U);
+        e0_to_U_kernel<decltype(LA)::value, decltype(LB)::value><<<grid, block, 0, st>>>(pc.d_pairs, pc.d_permB, p0, p1, pc.e_off, mj, lane0, r0, ld,
+                                                                                         mstride, mode, ubar, U);
     });
     return cudaGetLastError();
 }
@@ -361,6 +422,13 @@ cudaError_t risp_j_pass1(const PairClass &pc, const PrimPair *prims, const AuxCe
 cudaError_t risp_j_reduce_R(const double *Rpart, int nchunks, const AuxCentre *cen, int ncen, int ncen_pad, double *R, cudaStream_t st)
 {
     j_reduce_R_kernel<<<ncen * 4, 256, 0, st>>>(Rpart, nchunks, cen, ncen, ncen_pad, R);
+    return cudaGetLastError();
+}
+
+cudaError_t risp_rt_by_centre(const double *Rt, const AuxCentre *cen, int ncen, double *RtC, cudaStream_t st)
+{
+    const int ncen32 = (ncen + 31) / 32 * 32;
+    rt_by_centre_kernel<<<ncen32 * 4, 32, 0, st>>>(Rt, cen, ncen, RtC);
     return cudaGetLastError();
 }
 

@@ -2,7 +2,8 @@
 //
 //   sigma = (eps_a - eps_i) X                                                                         (diagonal)
 //   J (Eq. 11-17), per sub-batch of mj vectors and per panel of AO rows:
-//       Y = X C_vir^T ; D = C_occ Y (Eq. 12) ; D -> e0 space on the kept pairs ;
+//       Y = X C_vir^T ; D = C_occ Y (Eq. 12) ; D -> e0 space on the kept pairs (a pair takes D_AB from the panel that holds
+//       the rows of shell A and D_BA^T from the one that holds the rows of B) ;
 //     then once for all m vectors: pass 1 (Eq. 14) ; R~ = L^-T L^-1 R (Eq. 15) ; pass 2 (Eq. 16) ;
 //     then per sub-batch / panel: e0 space -> U ; Z = C_occ^T U ; sigma += 2 Z C_vir (Eq. 17)
 //   K (Eq. 18-23):  X' = X[window] ; per aux chunk (from HBM, or from pinned host memory through the
@@ -15,7 +16,7 @@
 
 void risp_free_workspace(risp_ctx *ctx)
 {
-    double **bufs[] = {&ctx->w_arena, &ctx->w_dbar, &ctx->w_Rpart, &ctx->w_R, &ctx->w_Rt, &ctx->w_Rtmp, &ctx->w_J,
+    double **bufs[] = {&ctx->w_arena, &ctx->w_dbar, &ctx->w_Rpart, &ctx->w_R, &ctx->w_Rt, &ctx->w_Rtmp, &ctx->w_RtC, &ctx->w_J,
                        &ctx->w_stage[0], &ctx->w_stage[1]};
     for (auto b : bufs) { if (*b) cudaFree(*b); *b = nullptr; }
     ctx->m_cap = 0; ctx->w_bytes = 0;
@@ -117,6 +118,7 @@ int risp_ensure_workspace(risp_ctx *ctx, int m)
     if ((rc = A(ctx->w_R, (size_t)ctx->nauxJ * RISP_MS * 8))) return rc;
     if ((rc = A(ctx->w_Rt, (size_t)ctx->nauxJ * RISP_MS * 8))) return rc;
     if ((rc = A(ctx->w_Rtmp, (size_t)ctx->nauxJ * RISP_MS * 8))) return rc;
+    if ((rc = A(ctx->w_RtC, (size_t)((ctx->ncenJ + 31) / 32 * 32) * 4 * RISP_MS * 8))) return rc;
     if (ctx->flags & RISP_FLAG_KEEP_STAGES) { if ((rc = A(ctx->w_J, (size_t)m * ctx->nocc * ctx->nvir * 8))) return rc; }
     if (spilled)
         for (int b = 0; b < 2; ++b)
@@ -128,11 +130,12 @@ int risp_ensure_workspace(risp_ctx *ctx, int m)
     return RISP_OK;
 }
 
-// pair range of class c whose shell A starts in AO rows [r0, r1)
-static void panel_pairs(const PairClass &pc, int r0, int r1, int &p0, int &p1)
+// index range of an ascending list of first-AO offsets (shell A of the aoA-sorted pairs, or shell B of the aoB-sorted index)
+// that falls into AO rows [r0, r1)
+static void panel_pairs(const std::vector<int> &ao, int r0, int r1, int &p0, int &p1)
 {
-    p0 = (int)(std::lower_bound(pc.h_aoA.begin(), pc.h_aoA.end(), r0) - pc.h_aoA.begin());
-    p1 = (int)(std::lower_bound(pc.h_aoA.begin(), pc.h_aoA.end(), r1) - pc.h_aoA.begin());
+    p0 = (int)(std::lower_bound(ao.begin(), ao.end(), r0) - ao.begin());
+    p1 = (int)(std::lower_bound(ao.begin(), ao.end(), r1) - ao.begin());
 }
 
 // The six pair classes of one J step touch disjoint rows of D-bar / U-bar / R partials and disjoint AO blocks, so their kernels
@@ -170,6 +173,7 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
     double *wY = ctx->w_arena;                                   // [mj][nocc][ldao]
     double *wD = wY + (size_t)pl.mj * nocc * ldao;               // [mj][prow][ldao]
     // ---------------- J: AO transition density (Eq. 12) on the kept pairs, in e0 space
+    if (!dense) RISP_CUDA_TRY(cudaMemsetAsync(ctx->w_dbar, 0, (size_t)ctx->e_rows * RISP_MS * sizeof(double), st));   // panels accumulate
     for (int l0 = 0; l0 < m; l0 += pl.mj) {
         const int mj = std::min(pl.mj, m - l0);
         const double *Xb = X + (size_t)l0 * nocc * nvir;
@@ -182,17 +186,16 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
             GemmDesc e = gemm_desc(pr, nao, nocc, ctx->d_Cocc + (size_t)r0 * ldocc, ldocc, true, wY, ldao, false, wD, ldao);
             e.nb1 = mj; e.sB1 = (long long)nocc * ldao; e.sC1 = mstride;
             RISP_CUDA_TRY(risp_dgemm(e, st)); ++launches;
-            if (!dense) {
-                // + D^T rows: sum_i Y[i][mu] C_occ[nu][i]   (only sym(D) matters, reading G13)
-                GemmDesc f = gemm_desc(pr, nao, nocc, wY + r0, ldao, false, ctx->d_Cocc, ldocc, true, wD, ldao, 1.0, 1.0);
-                f.nb1 = mj; f.sA1 = (long long)nocc * ldao; f.sC1 = mstride;
-                RISP_CUDA_TRY(risp_dgemm(f, st)); ++launches;
-            }
             if ((rc = fork_classes(ctx, st))) return rc;
             for (int c = 0; c < 6; ++c) {
+                const PairClass &pc = ctx->cls[c];
                 int p0, p1;
-                panel_pairs(ctx->cls[c], r0, r1, p0, p1);
-                if (p1 > p0) { RISP_CUDA_TRY(risp_dens_to_e0(ctx->cls[c], p0, p1, mj, l0, r0, ldao, mstride, dense ? 0 : 1, wD, ctx->w_dbar, ctx->cls_st[c])); ++launches; }
+                panel_pairs(pc.h_aoA, r0, r1, p0, p1);
+                if (p1 > p0) { RISP_CUDA_TRY(risp_dens_to_e0(pc, p0, p1, mj, l0, r0, ldao, mstride, dense ? 0 : 1, wD, ctx->w_dbar, ctx->cls_st[c])); ++launches; }
+                if (!dense) {      // the lower-triangular pair also takes D_BA^T (reading G13), found in the panel that holds the rows of B
+                    panel_pairs(pc.h_aoB, r0, r1, p0, p1);
+                    if (p1 > p0) { RISP_CUDA_TRY(risp_dens_to_e0(pc, p0, p1, mj, l0, r0, ldao, mstride, 2, wD, ctx->w_dbar, ctx->cls_st[c])); ++launches; }
+                }
             }
             if ((rc = join_classes(ctx, st))) return rc;
         }
@@ -210,12 +213,13 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
     RISP_CUDA_TRY(cudaEventRecord(ev[2], st));
     // ---------------- R~ = (P|Q)^-1 R = L^-T (L^-1 R)  (Eq. 15)
     RISP_CUDA_TRY(risp_metric_solve32(ctx->d_LinvJ, nJ, ctx->w_R, ctx->w_Rtmp, ctx->w_Rt, st)); launches += 2;
+    RISP_CUDA_TRY(risp_rt_by_centre(ctx->w_Rt, ctx->d_cenJ, ctx->ncenJ, ctx->w_RtC, st)); ++launches;
     RISP_CUDA_TRY(cudaEventRecord(ev[3], st));
     // ---------------- pass 2: U (Eq. 16), into the e0 buffer
     if ((rc = fork_classes(ctx, st))) return rc;
     for (int c = 5; c >= 0; --c)
         if (ctx->cls[c].npairs) {
-            RISP_CUDA_TRY(risp_j_pass2(ctx->cls[c], ctx->d_prims, ctx->d_cenJ, ctx->ncenJ, ctx->d_boys, ctx->w_Rt, ctx->w_dbar, ctx->cls_st[c]));
+            RISP_CUDA_TRY(risp_j_pass2(ctx->cls[c], ctx->d_prims, ctx->d_cenJ, ctx->ncenJ, ctx->d_boys, ctx->w_RtC, ctx->w_dbar, ctx->cls_st[c]));
             ++launches;
         }
     if ((rc = join_classes(ctx, st))) return rc;
@@ -229,21 +233,20 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
             RISP_CUDA_TRY(cudaMemsetAsync(wD, 0, (size_t)mj * mstride * sizeof(double), st));
             if ((rc = fork_classes(ctx, st))) return rc;
             for (int c = 0; c < 6; ++c) {
+                const PairClass &pc = ctx->cls[c];
                 int p0, p1;
-                panel_pairs(ctx->cls[c], r0, r1, p0, p1);
-                if (p1 > p0) { RISP_CUDA_TRY(risp_e0_to_U(ctx->cls[c], p0, p1, mj, l0, r0, ldao, mstride, dense ? 1 : 0, ctx->w_dbar, wD, ctx->cls_st[c])); ++launches; }
+                panel_pairs(pc.h_aoA, r0, r1, p0, p1);
+                if (p1 > p0) { RISP_CUDA_TRY(risp_e0_to_U(pc, p0, p1, mj, l0, r0, ldao, mstride, dense ? 0 : 1, ctx->w_dbar, wD, ctx->cls_st[c])); ++launches; }
+                if (!dense) {      // complete rows of the symmetric U: the transposed blocks of the pairs whose shell B lies in the panel
+                    panel_pairs(pc.h_aoB, r0, r1, p0, p1);
+                    if (p1 > p0) { RISP_CUDA_TRY(risp_e0_to_U(pc, p0, p1, mj, l0, r0, ldao, mstride, 2, ctx->w_dbar, wD, ctx->cls_st[c])); ++launches; }
+                }
             }
             if ((rc = join_classes(ctx, st))) return rc;
-            // Z[i][nu] (+)= sum_{mu in panel} C_occ[mu][i] P[mu][nu]
+            // Z[i][nu] (+)= sum_{mu in panel} C_occ[mu][i] U[mu][nu]
             GemmDesc d = gemm_desc(nocc, nao, pr, ctx->d_Cocc + (size_t)r0 * ldocc, ldocc, false, wD, ldao, false, wY, ldao, 1.0, p == 0 ? 0.0 : 1.0);
             d.nb1 = mj; d.sB1 = mstride; d.sC1 = (long long)nocc * ldao;
             RISP_CUDA_TRY(risp_dgemm(d, st)); ++launches;
-            if (!dense) {
-                // U = P + P^T: Z[i][nu in panel] += sum_mu' P[nu][mu'] C_occ[mu'][i]
-                GemmDesc f = gemm_desc(nocc, pr, nao, ctx->d_Cocc, ldocc, false, wD, ldao, true, wY + r0, ldao, 1.0, 1.0);
-                f.nb1 = mj; f.sB1 = mstride; f.sC1 = (long long)nocc * ldao;
-                RISP_CUDA_TRY(risp_dgemm(f, st)); ++launches;
-            }
         }
         double *Sb = sigma + (size_t)l0 * nocc * nvir;
         if (ctx->w_J) {

@@ -186,7 +186,7 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
     if (!sys) return RISP_EINVAL;
     risp_ctx *ctx = new risp_ctx();
     *out = ctx;   // returned even on failure so that risp_last_error() can be read; caller destroys it
-    for (int c = 0; c < 6; ++c) { ctx->cls[c].npairs = 0; ctx->cls[c].d_pairs = nullptr; }
+    for (int c = 0; c < 6; ++c) { ctx->cls[c].npairs = 0; ctx->cls[c].d_pairs = nullptr; ctx->cls[c].d_permB = nullptr; }
     risp_options opt;
     std::memset(&opt, 0, sizeof(opt));
     if (opt_in) opt = *opt_in;
@@ -335,6 +335,15 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
             pc.la = LA[c]; pc.lb = LB[c]; pc.npairs = (int)pairs[c].size();
             pc.h_aoA.resize(pc.npairs);
             for (int k = 0; k < pc.npairs; ++k) pc.h_aoA[k] = pairs[c][k].aoA;
+            {   // second index of the same pairs, sorted by the first AO of shell B (row panels that hold the rows of B)
+                std::vector<int> perm(pc.npairs);
+                for (int k = 0; k < pc.npairs; ++k) perm[k] = k;
+                std::stable_sort(perm.begin(), perm.end(), [&](int x, int y) { return pairs[c][x].aoB < pairs[c][y].aoB; });
+                pc.h_aoB.resize(pc.npairs);
+                for (int k = 0; k < pc.npairs; ++k) pc.h_aoB[k] = pairs[c][perm[k]].aoB;
+                int rcp;
+                if ((rcp = upload(ctx, pc.d_permB, perm.data(), perm.size()))) return rcp;
+            }
             pc.e_off = e_off; e_off += (long long)pc.npairs * ne_of(pc.la, pc.lb);
             {
                 const int nch = std::max(1, std::min((pc.npairs + 15) / 16, want_chunks));

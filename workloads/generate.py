@@ -376,6 +376,7 @@ def make_system(cfg: int, *, base_seed: int = BASE_SEED, counts=None, check: boo
             St = gpu.from_numpy(S).cuda()
             wt, Ut = gpu.linalg.eigh(St)
             w = wt.cpu().numpy()
+            U = Ut
         else:
             w, U = np.linalg.eigh(S)
         if w[0] > 1e-6 or not check:
