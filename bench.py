@@ -110,6 +110,7 @@ def main():
     ap.add_argument("--ref-vectors", type=int, default=30, help="trial vectors per step of the CPU oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--batch", type=int, default=0, help="trial vectors per step (0: the config's m)")
+    ap.add_argument("--solve-max-iter", type=int, default=100)
     ap.add_argument("--solve", action="store_true", help="also time the 15-root risp_tda_solve (reported under 'solve')")
     args = ap.parse_args()
     # contract: >= 3 warm-up steps; the 1000/3000-atom configs (tens of seconds to minutes per step) are allowed 1 and say so
@@ -259,7 +260,7 @@ def main():
                                         sample=f"one oracle.sigma call on {ms_} of the {m} trial vectors ({dt:.1f} s); tensor build ({tb:.1f} s) excluded like risp_setup",
                                         gpu_vs_oracle_rel_err=err)
         if args.solve:
-            omega, _, info = ctx.tda_solve(s["nroots"], tol=1e-5, allow_unconverged=True)
+            omega, _, info = ctx.tda_solve(s["nroots"], tol=1e-5, max_iter=args.solve_max_iter, allow_unconverged=True)
             line["solve"] = dict(nroots=s["nroots"], tol=1e-5, wall_s=info["sec_total"], matvec_s=info["sec_matvec"], alloc_s=info["sec_alloc"], subspace_s=info["sec_subspace"], cached_vectors=info["cached_vectors"], iterations=info["iterations"],
                                  n_sigma=info["n_sigma"], restarts=info["restarts"], converged=info["converged"], omega_ev=[float(x) * 27.211386245988 for x in omega],
                                  h2d_gb=info["bytes_h2d"] / 1e9, d2h_gb=info["bytes_d2h"] / 1e9)

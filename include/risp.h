@@ -77,7 +77,8 @@ typedef struct {
     double screen_tol;          /* shell-pair screening threshold tau (0 -> default 1e-13; < 0 -> keep every pair) */
     size_t hbm_budget_bytes;    /* device memory the library may use (0 -> 85 % of what is free at setup); K-tensor slices that do
                                    not fit are kept in pinned host memory and streamed per matvec */
-    size_t host_budget_bytes;   /* pinned-host budget of the Davidson subspace; 0 -> 8 GiB */
+    size_t host_budget_bytes;   /* pinned-host budget of the part of the Davidson subspace that does not fit in HBM; 0 -> half of the
+                                   physical host memory */
     int32_t device;             /* CUDA device ordinal */
     int32_t flags;              /* RISP_FLAG_* */
     int32_t max_batch;          /* largest m the caller will pass to risp_matvec (0 -> 32); HBM is reserved for its X, sigma

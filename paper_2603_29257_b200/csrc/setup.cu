@@ -7,6 +7,7 @@
 #include "ctx.h"
 #include <algorithm>
 #include <cmath>
+#include <unistd.h>
 
 using namespace risp_eri;
 
@@ -398,7 +399,11 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
     size_t free_b = 0, total_b = 0;
     RISP_CUDA_TRY(cudaMemGetInfo(&free_b, &total_b));
     ctx->hbm_budget = opt.hbm_budget_bytes ? opt.hbm_budget_bytes : (size_t)(0.85 * (double)free_b) + ctx->setup_bytes;
-    ctx->host_budget = opt.host_budget_bytes ? opt.host_budget_bytes : ((size_t)8 << 30);
+    if (opt.host_budget_bytes) ctx->host_budget = opt.host_budget_bytes;
+    else {   // half of the physical host memory
+        const long pages = sysconf(_SC_PHYS_PAGES), psz = sysconf(_SC_PAGE_SIZE);
+        ctx->host_budget = pages > 0 && psz > 0 ? (size_t)pages * (size_t)psz / 2 : ((size_t)8 << 30);
+    }
 
     // ---------------------------------------------------------------- a3: K tensors, packed lower triangles (Eq. 20-21)
     if (ctx->has_K) {

@@ -513,11 +513,6 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
 
     Solver S;
     S.ctx = ctx; S.dim = dim;
-    // subspace capacity: user limit, and the pinned-host budget (V and W)
-    long long by_budget = (long long)(ctx->host_budget / (2.0 * dim * 8.0));
-    S.cap = (int)std::min<long long>(max_sub, by_budget);
-    S.cap = std::max(S.cap, std::max(n_guess, 2 * nroots));
-    const int slots = S.cap + nroots;              // room to append one more block before the restart decision
     const int nbmax = std::max(n_guess, nroots);
     auto DA = [&](double *&p, size_t n) -> int { RISP_CUDA_TRY(cudaMalloc((void **)&p, n * 8)); return RISP_OK; };
     int rc;
@@ -525,10 +520,9 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
         (rc = DA(S.dAX, (size_t)nroots * dim)) || (rc = DA(S.dRes, (size_t)nroots * dim)) || (rc = DA(S.dT, (size_t)nroots * dim)) ||
         (rc = DA(S.dChunk[0], (size_t)S.CH * dim)) || (rc = DA(S.dChunk[1], (size_t)S.CH * dim)))
         return rc;
-    const int small = std::max(slots, 64);
     S.slice = dim > (1 << 20) ? 4096 : 16384;      // enough slices to give every SM a tile
     const int nzmax = (int)(dim / S.slice) + 2;
-    if ((rc = DA(S.dCoef, (size_t)small * small)) || (rc = DA(S.dPart, std::max((size_t)nzmax * 128 * 64, (size_t)RISP_MAX_ROOTS * 256))) || (rc = DA(S.dSmall, (size_t)128 * 64 + 4096)) ||
+    if ((rc = DA(S.dPart, std::max((size_t)nzmax * 128 * 64, (size_t)RISP_MAX_ROOTS * 256))) || (rc = DA(S.dSmall, (size_t)128 * 64 + 4096)) ||
         (rc = DA(S.dTheta, (size_t)RISP_MAX_ROOTS)))
         return rc;
     RISP_CUDA_TRY(cudaMalloc((void **)&S.dSrc, RISP_MAX_ROOTS * sizeof(int)));
@@ -536,24 +530,31 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
     RISP_CUDA_TRY(cudaEventCreateWithFlags(&S.evD2H, cudaEventDisableTiming));
     RISP_CUDA_TRY(cudaEventCreateWithFlags(&S.evReady, cudaEventDisableTiming));
 
-    // device cache of the subspace: what is left of HBM once the matvec work space for the largest block exists
+    // subspace capacity: the user's max_sub, bounded by what HBM (left once the matvec work space for the largest
+    // block exists) and the pinned-host budget can hold together; vectors [0, ncache) live on the device, the others on the host
+    int slots = 0;
     {
         int rcw = risp_ensure_workspace(ctx, std::min(nbmax, RISP_MS));
         if (rcw) return rcw;
         size_t free_b = 0, total_b = 0;
         RISP_CUDA_TRY(cudaMemGetInfo(&free_b, &total_b));
-        const size_t keep = (size_t)1 << 30;
+        const size_t keep = (size_t)1 << 30, pervec = 2 * (size_t)dim * 8;
         size_t room = free_b > keep ? (size_t)(0.9 * (double)(free_b - keep)) : 0;
-        if (!(opt.flags & 1)) {      // flags bit 0: no device cache (testing the streamed path)
-            S.ncache = (int)std::min<size_t>((size_t)slots, room / (2 * (size_t)dim * 8));
-            if (opt.flags & 2) S.ncache = std::min(S.ncache, nroots + 2);   // flags bit 1: tiny cache (testing the mixed path)
-        }
+        long long dev_vecs = (opt.flags & 1) ? 0 : (long long)(room / pervec);      // flags bit 0: no device cache (testing the streamed path)
+        if (opt.flags & 2) dev_vecs = std::min<long long>(dev_vecs, nroots + 2);     // flags bit 1: tiny cache (testing the mixed path)
+        const long long host_vecs = (long long)(ctx->host_budget / pervec);
+        slots = (int)std::min<long long>((long long)max_sub + nroots, dev_vecs + host_vecs);
+        slots = std::max(slots, std::max(n_guess, 2 * nroots) + nroots);
+        S.cap = slots - nroots;                     // room to append one more block before the restart decision
+        S.ncache = (int)std::min<long long>(slots, dev_vecs);
         if (S.ncache > 0) {
             RISP_CUDA_TRY(cudaMalloc((void **)&S.dVc, (size_t)S.ncache * dim * 8));
             RISP_CUDA_TRY(cudaMalloc((void **)&S.dWc, (size_t)S.ncache * dim * 8));
         }
         // vectors beyond the cache live in pinned host memory only; nothing is pinned when everything fits in HBM
         if (slots > S.ncache) S.host.start(ctx->device, dim, slots - S.ncache);
+        const int small = std::max(slots, 64);
+        if ((rc = DA(S.dCoef, (size_t)small * small))) return rc;
     }
 
     auto cleanup = [&]() {
