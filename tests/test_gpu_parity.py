@@ -205,6 +205,60 @@ def test_no_truncation_and_empty_window(torch_cuda, sys_small_rsh):
         c.close()
 
 
+# ------------------------------------------------------------------------------------------------ edge cases
+@pytest.mark.parametrize("m", [1, 32])
+def test_batch_extremes(m, torch_cuda, sys_small_rsh, ctx_rsh, oracle_small_rsh):
+    """a single trial vector, and the largest batch the ABI takes (32 = one lane per vector in the ERI passes)"""
+    torch = torch_cuda
+    from workloads import trial_vectors
+    X = trial_vectors(sys_small_rsh, m)
+    sig_ref, dg, J_ref, K_ref = oracle_small_rsh.sigma(X, parts=True)
+    sig = ctx_rsh.matvec(torch.from_numpy(X).cuda()).cpu().numpy()
+    assert _rel(ctx_rsh.stage("J", m), J_ref) <= 1e-10
+    assert _rel(ctx_rsh.stage("K", m), K_ref) <= 1e-10
+    assert _rel(sig, sig_ref) <= 1e-10
+
+
+@pytest.mark.parametrize("variant", ["s_only_aux", "p_in_K_aux", "no_exchange", "zero_vector"])
+def test_auxiliary_set_and_operator_variants(variant, torch_cuda, sys_small_rsh):
+    """degenerate / unusual inputs: an s-only auxiliary basis (no p recursion output is used), p functions inside the K auxiliary
+    set (the paper's default is s only), alpha = beta = 0 (no K term at all), and X = 0."""
+    torch = torch_cuda
+    from paper_2603_29257_b200 import setup
+    from oracle.risp_oracle import Oracle
+    from workloads import trial_vectors
+    s = dict(sys_small_rsh)
+    if variant == "s_only_aux":
+        keep = np.nonzero(np.asarray(s["aux_l"]) == 0)[0]
+        for k in ("aux_atom", "aux_l", "aux_exp", "aux_in_K"):
+            s[k] = np.ascontiguousarray(np.asarray(s[k])[keep])
+        s["naux"] = len(keep)
+    if variant == "p_in_K_aux":
+        s["aux_in_K"] = np.ones_like(np.asarray(s["aux_in_K"]))
+    if variant == "no_exchange":
+        s["alpha"], s["beta"] = 0.0, 0.0
+    X = trial_vectors(s, 3)
+    if variant == "zero_vector":
+        X[1] = 0.0
+    o = Oracle(s)
+    sig_ref, dg, J_ref, K_ref = o.sigma(X, parts=True)
+    c = setup(s, flags=1)
+    try:
+        sig = c.matvec(torch.from_numpy(X).cuda()).cpu().numpy()
+        d = c.dims()
+        assert d["nauxJ"] == o.nfun(o.selJ) and d["nauxK"] == (o.nfun(o.selK) if len(o.selK) else 0)
+        assert _rel(c.stage("J", 3), J_ref) <= 1e-10
+        if variant == "no_exchange":
+            assert np.abs(c.stage("K", 3)).max() == 0.0 and np.abs(K_ref).max() == 0.0
+        else:
+            assert _rel(c.stage("K", 3), K_ref) <= 1e-10
+        assert _rel(sig, sig_ref) <= 1e-10
+        if variant == "zero_vector":
+            assert np.abs(sig[1]).max() == 0.0
+    finally:
+        c.close()
+
+
 # ------------------------------------------------------------------------------------------------ memory plans
 @pytest.mark.parametrize("plan", [dict(mj=2, prow=0, pc=0), dict(mj=0, prow=40, pc=1), dict(mj=3, prow=24, pc=2), dict(mj=1, prow=1, pc=5)])
 @pytest.mark.parametrize("which", ["tiny", "rsh"])
