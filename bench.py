@@ -235,6 +235,9 @@ def main():
             roofline=dict(bound="tensor", kernel="dgemm_tma_kernel<KC,KC,MI> (K contraction M^P = X' T_ab^P, Eq. 22)", achieved=achieved, peak=peak,
                           unit="TFLOP/s", frac=achieved / peak, traffic=traffic,
                           peak_source=f"{pk['src']} bf16 burst {pk['bf16']} TFLOP/s x nominal FP64:bf16 ratio 45/2250",
+                          context=dict(dmma_issue_ceiling_tflops=37.2, cublas_dgemm_measured_tflops=36.2,
+                                       note="FP64 tensor op of sm_100a is the warp-level DMMA.8x8x4 (one per 16 clk per sub-partition); the peak "
+                                            "above is the tier rule (other dtype's measured peak x nominal ratio), so frac can slightly exceed 1"),
                           flops_per_launch=flops_launch, launch_ms=1e3 * t_launch),
             phases_ms={k: round(1e3 * v / args.steps, 4) for k, v in phase.items() if k not in ("kernel_launches", "first_chunk_naux")},
             rooflines_other=[
