@@ -163,13 +163,11 @@ __device__ __forceinline__ void park_integrals(double *__restrict__ g, int lane,
 #pragma unroll
         for (int k = 0; k < NE * 4; ++k) g[k * 32 + lane] = 0.0;
         if (valid) {
-            OpParams op{1.0, 0.0, 0.0};
-            PrimPair pp = prims[sp.ppoff];
+            OpParams op{1.0, 0.0, 0.0};      // dp, dd: no prefetch, the recursion needs every register
             for (int k = 0; k < sp.npp; ++k) {
-                const PrimPair nxt = prims[sp.ppoff + min(k + 1, sp.npp - 1)];
+                const PrimPair pp = prims[sp.ppoff + k];
                 eri_e0_prim<LA, LB, true, false>(pp, sp.Ax, sp.Ay, sp.Az, ax, op, boys_tab,
                                                  [&](int e, int c, double v) { g[(e * 4 + c) * 32 + lane] += v; });
-                pp = nxt;
             }
         }
     }
@@ -251,11 +249,14 @@ __global__ void __launch_bounds__(32 * JW) j_pass1_kernel(const ShellPair *__res
     double acc[32];
 #pragma unroll
     for (int k = 0; k < 32; ++k) acc[k] = 0.0;
+    constexpr bool LEAN = NE > 10;          // dp, dd: the recursion already spills; no operand batching, no shell-pair prefetch
     ShellPair sp = pairs[min(p_begin + w * 4 + slot, p_end - 1)];
     for (int pg = p_begin + w * 4; pg < p_end; pg += JW * 4) {
         const int pi = pg + slot;
         const bool valid = cvalid && pi < p_end;
-        const ShellPair sp_next = pairs[min(pi + JW * 4, p_end - 1)];
+        if constexpr (LEAN) sp = pairs[min(pi, p_end - 1)];
+        ShellPair sp_next;
+        if constexpr (!LEAN) sp_next = pairs[min(pi + JW * 4, p_end - 1)];
         const double *db = dbar + (e_off + (long long)pg * NE) * MS + lane;
         const int ns = min(4, p_end - pg);
         double dpre[PRE ? 4 * NE : 1];
@@ -264,20 +265,24 @@ __global__ void __launch_bounds__(32 * JW) j_pass1_kernel(const ShellPair *__res
             for (int k = 0; k < 4 * NE; ++k) dpre[k] = (k / NE < ns) ? db[(long long)k * MS] : 0.0;
         }
         park_integrals<LA, LB>(g, lane, valid, sp, prims, ax, boys_tab);
-        sp = sp_next;
+        if constexpr (!LEAN) sp = sp_next;
         __syncwarp();
-#pragma unroll
+#pragma unroll(LEAN ? 1 : 4)
         for (int s = 0; s < 4; ++s) {
             if (s >= ns) break;
-            double dv[NE];
+            double dv[LEAN ? 1 : NE];
+            if constexpr (!LEAN) {
 #pragma unroll
-            for (int e = 0; e < NE; ++e) {
-                if constexpr (PRE) dv[e] = dpre[s * NE + e];
-                else dv[e] = db[(long long)(s * NE + e) * MS];
+                for (int e = 0; e < NE; ++e) {
+                    if constexpr (PRE) dv[e] = dpre[s * NE + e];
+                    else dv[e] = db[(long long)(s * NE + e) * MS];
+                }
             }
 #pragma unroll
             for (int e = 0; e < NE; ++e) {
-                const double d = dv[e];
+                double d;
+                if constexpr (LEAN) d = db[(long long)(s * NE + e) * MS];
+                else d = dv[e];
 #pragma unroll
                 for (int c = 0; c < 4; ++c)
 #pragma unroll
