@@ -3,40 +3,55 @@
 #include "ctx.h"
 
 namespace {
+// The three streaming kernels work row by row (one (vector, occupied) row of X / sigma per CTA pass): no 64-bit divisions per
+// element, 16-byte accesses where the row start allows, rows strided over the grid.
 // Xk[m][no][ldk] = X[m][o0+i][v0+a]
-__global__ void gather_window_kernel(const double *__restrict__ X, double *__restrict__ Xk, long long total, int nocc, int nvir,
-                                     int o0, int no, int v0, int nv, int ldk)
+__global__ void __launch_bounds__(256) gather_window_kernel(const double *__restrict__ X, double *__restrict__ Xk, long long rows, int nocc, int nvir,
+                                                            int o0, int no, int v0, int nv, int ldk)
 {
-    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
-        int a = (int)(t % nv);
-        long long r = t / nv;
-        int i = (int)(r % no);
-        long long mi = r / no;
-        Xk[r * ldk + a] = X[(mi * nocc + o0 + i) * (long long)nvir + v0 + a];
+    for (long long r = blockIdx.x; r < rows; r += gridDim.x) {
+        const long long mi = r / no;
+        const int i = (int)(r - mi * no);
+        const double *src = X + (mi * nocc + o0 + i) * (long long)nvir + v0;
+        double *dst = Xk + r * ldk;
+        for (int a = threadIdx.x; a < nv; a += blockDim.x) dst[a] = src[a];
     }
 }
 
 // sigma = (eps_a - eps_i) X   (the J and K terms are accumulated onto it afterwards)
-__global__ void diag_sigma_kernel(const double *__restrict__ X, const double *__restrict__ eps, double *__restrict__ sigma, long long total,
-                                  int nocc, int nvir)
+__global__ void __launch_bounds__(256) diag_sigma_kernel(const double *__restrict__ X, const double *__restrict__ eps, double *__restrict__ sigma,
+                                                         long long rows, int nocc, int nvir)
 {
-    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
-        int a = (int)(t % nvir);
-        int i = (int)((t / nvir) % nocc);
-        sigma[t] = (eps[nocc + a] - eps[i]) * X[t];
+    const double *ev = eps + nocc;
+    for (long long r = blockIdx.x; r < rows; r += gridDim.x) {
+        const double ei = eps[(int)(r % nocc)];
+        const double *x = X + r * nvir;
+        double *s = sigma + r * nvir;
+        if ((((size_t)x | (size_t)s) & 15) == 0) {
+            const int n2 = nvir >> 1;
+            for (int a = threadIdx.x; a < n2; a += blockDim.x) {
+                const double2 xv = reinterpret_cast<const double2 *>(x)[a];
+                double2 o;
+                o.x = (ev[2 * a] - ei) * xv.x; o.y = (ev[2 * a + 1] - ei) * xv.y;
+                reinterpret_cast<double2 *>(s)[a] = o;
+            }
+            if ((nvir & 1) && threadIdx.x == 0) s[nvir - 1] = (ev[nvir - 1] - ei) * x[nvir - 1];
+        } else {
+            for (int a = threadIdx.x; a < nvir; a += blockDim.x) s[a] = (ev[a] - ei) * x[a];
+        }
     }
 }
 
 // sigma[m][o0+i][v0+a] -= K'[m][i][a]   (K acts only inside the window; reading G7)
-__global__ void sub_window_kernel(const double *__restrict__ Kk, double *__restrict__ sigma, long long total, int nocc, int nvir, int o0,
-                                  int no, int v0, int nv, int ldk)
+__global__ void __launch_bounds__(256) sub_window_kernel(const double *__restrict__ Kk, double *__restrict__ sigma, long long rows, int nocc, int nvir,
+                                                         int o0, int no, int v0, int nv, int ldk)
 {
-    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
-        int a = (int)(t % nv);
-        long long r = t / nv;
-        int i = (int)(r % no);
-        long long mi = r / no;
-        sigma[(mi * nocc + o0 + i) * (long long)nvir + v0 + a] -= Kk[r * ldk + a];
+    for (long long r = blockIdx.x; r < rows; r += gridDim.x) {
+        const long long mi = r / no;
+        const int i = (int)(r - mi * no);
+        double *dst = sigma + (mi * nocc + o0 + i) * (long long)nvir + v0;
+        const double *src = Kk + r * ldk;
+        for (int a = threadIdx.x; a < nv; a += blockDim.x) dst[a] -= src[a];
     }
 }
 
@@ -90,6 +105,7 @@ __global__ void __launch_bounds__(256) expand_sym_kernel(const double *__restric
     }
 }
 
+inline unsigned rows_grid(long long rows) { return (unsigned)(rows < 148LL * 32 ? rows : 148 * 32); }
 inline unsigned grid_for(long long total)
 {
     long long g = (total + 255) / 256;
@@ -99,23 +115,23 @@ inline unsigned grid_for(long long total)
 
 cudaError_t risp_gather_window(const double *X, double *Xk, int m, int nocc, int nvir, int o0, int no, int v0, int nv, int ldk, cudaStream_t st)
 {
-    long long total = (long long)m * no * nv;
-    if (total == 0) return cudaSuccess;
-    gather_window_kernel<<<grid_for(total), 256, 0, st>>>(X, Xk, total, nocc, nvir, o0, no, v0, nv, ldk);
+    long long rows = (long long)m * no;
+    if (rows == 0 || nv == 0) return cudaSuccess;
+    gather_window_kernel<<<rows_grid(rows), nv >= 256 ? 256 : 128, 0, st>>>(X, Xk, rows, nocc, nvir, o0, no, v0, nv, ldk);
     return cudaGetLastError();
 }
 cudaError_t risp_diag_sigma(const double *X, const double *eps, double *sigma, int m, int nocc, int nvir, cudaStream_t st)
 {
-    long long total = (long long)m * nocc * nvir;
-    if (total == 0) return cudaSuccess;
-    diag_sigma_kernel<<<grid_for(total), 256, 0, st>>>(X, eps, sigma, total, nocc, nvir);
+    long long rows = (long long)m * nocc;
+    if (rows == 0 || nvir == 0) return cudaSuccess;
+    diag_sigma_kernel<<<rows_grid(rows), nvir >= 512 ? 256 : 128, 0, st>>>(X, eps, sigma, rows, nocc, nvir);
     return cudaGetLastError();
 }
 cudaError_t risp_sub_window(const double *Kk, double *sigma, int m, int nocc, int nvir, int o0, int no, int v0, int nv, int ldk, cudaStream_t st)
 {
-    long long total = (long long)m * no * nv;
-    if (total == 0) return cudaSuccess;
-    sub_window_kernel<<<grid_for(total), 256, 0, st>>>(Kk, sigma, total, nocc, nvir, o0, no, v0, nv, ldk);
+    long long rows = (long long)m * no;
+    if (rows == 0 || nv == 0) return cudaSuccess;
+    sub_window_kernel<<<rows_grid(rows), nv >= 256 ? 256 : 128, 0, st>>>(Kk, sigma, rows, nocc, nvir, o0, no, v0, nv, ldk);
     return cudaGetLastError();
 }
 cudaError_t risp_scatter_window(const double *Kk, double *Kf, int m, int nocc, int nvir, int o0, int no, int v0, int nv, int ldk, cudaStream_t st)
