@@ -42,6 +42,39 @@ def test_dgemm_against_torch(torch_cuda, a_kc, b_kc, shape):
     assert float((out - ref).abs().max()) <= 1e-12 * max(1.0, K ** 0.5) * float(ref.abs().max() + 1)
 
 
+@pytest.mark.parametrize("a_kc,b_kc", [(1, 1), (1, 0), (0, 1), (0, 0)])
+@pytest.mark.parametrize("M", [9, 20, 40, 60, 75, 90, 110, 128, 200, 423])
+def test_dgemm_tma_tile_heights(torch_cuda, a_kc, b_kc, M):
+    """The TMA/mbarrier kernel (even leading dimensions, aligned bases) for every tile height 16..128, ragged M, N, K, a batch,
+    alpha/beta, against torch and against the cp.async kernel (variant 0) on the same operands."""
+    torch = torch_cuda
+    from paper_2603_29257_b200 import load_library
+    lib = load_library()
+    N, K, nb = 150, 70, 3
+    lda = (K if a_kc else M) + 2 + ((K if a_kc else M) & 1)           # even, padded
+    ldb = (K if b_kc else N) + 4 + ((K if b_kc else N) & 1)
+    ra, rb = (M if a_kc else K), (N if b_kc else K)
+    g = torch.Generator(device="cuda").manual_seed(1000 * M + 10 * a_kc + b_kc)
+    A = torch.randn((nb, ra, lda), dtype=torch.float64, device="cuda", generator=g)
+    B = torch.randn((nb, rb, ldb), dtype=torch.float64, device="cuda", generator=g)
+    C0 = torch.randn((nb, M, N), dtype=torch.float64, device="cuda", generator=g)
+    Aop = A[:, :, :K] if a_kc else A[:, :, :M].transpose(1, 2)
+    Bop = B[:, :, :K].transpose(1, 2) if b_kc else B[:, :, :N]
+    ref = 1.3 * Aop @ Bop + 0.5 * C0
+    outs = []
+    for variant in (1, 0):
+        lib.risp_debug_set_gemm_variant(variant)
+        out = C0.clone()
+        rc = lib.risp_debug_dgemm(M, N, K, A.data_ptr(), lda, a_kc, B.data_ptr(), ldb, b_kc, out.data_ptr(), N, 1.3, 0.5, nb, ra * lda, rb * ldb, M * N,
+                                  torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        assert rc == 0
+        outs.append(out)
+    lib.risp_debug_set_gemm_variant(1)
+    assert float((outs[0] - ref).abs().max()) <= 1e-12 * float(ref.abs().max() + 1)
+    assert float((outs[0] - outs[1]).abs().max()) <= 1e-12 * float(ref.abs().max() + 1)
+
+
 def test_dgemm_batched(torch_cuda):
     torch = torch_cuda
     from paper_2603_29257_b200 import load_library
