@@ -91,6 +91,8 @@ def load_library():
     lib.risp_get_stage.argtypes = [vp, i32, vp, i64, vp]
     lib.risp_debug_dgemm.argtypes = [C.c_int, C.c_int, C.c_int, vp, C.c_longlong, C.c_int, vp, C.c_longlong, C.c_int, vp, C.c_longlong,
                                      dbl, dbl, C.c_int, C.c_longlong, C.c_longlong, C.c_longlong, vp]
+    lib.risp_debug_dgemm_split.argtypes = [C.c_int, C.c_int, C.c_int, vp, C.c_longlong, vp, C.c_longlong, vp, C.c_longlong,
+                                           C.c_int, C.c_longlong, C.c_int, C.c_longlong, vp]
     lib.risp_debug_sym_eig.argtypes = [C.c_int, vp, vp, vp]
     lib.risp_debug_sym_eig_lowest.argtypes = [C.c_int, C.c_int, vp, vp, vp]
     lib.risp_debug_force_plan.argtypes = [vp, C.c_int, C.c_int, C.c_int]

@@ -221,3 +221,12 @@ extern "C" int risp_debug_set_gemm_variant(int v)
     risp_dgemm_set_variant(v);
     return RISP_OK;
 }
+
+// Debug export: GEMM with the row / column split epilogue (GemmDesc::c_rpg, c_cpg), for the unit test of that addressing.
+extern "C" int risp_debug_dgemm_split(int M, int N, int K, const double *A, long long lda, const double *B, long long ldb, double *C, long long ldc,
+                                      int c_rpg, long long c_gstride, int c_cpg, long long c_cgstride, void *stream)
+{
+    GemmDesc d = gemm_desc(M, N, K, A, lda, true, B, ldb, true, C, ldc);
+    d.c_rpg = c_rpg; d.c_gstride = c_gstride; d.c_cpg = c_cpg; d.c_cgstride = c_cgstride;
+    return risp_dgemm(d, (cudaStream_t)stream) == cudaSuccess ? RISP_OK : RISP_ECUDA;
+}

@@ -165,7 +165,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) dgemm_kernel(GemmDesc d, int t
     }
     cp_async_wait<0>();
     // epilogue: thread holds C(row = q, col = 2r, 2r+1) of each 8x8 tile
-    const bool vecC = ((d.ldc & 1) == 0) && ((d.c_gstride & 1) == 0) && ((((size_t)Cp) & 15) == 0);
+    const bool vecC = ((d.ldc & 1) == 0) && ((d.c_gstride & 1) == 0) && ((d.c_cgstride & 1) == 0) && ((((size_t)Cp) & 15) == 0);
 #pragma unroll
     for (int i = 0; i < MI; ++i) {
         int row = m0 + wm * (MI * 8) + i * 8 + q;
@@ -175,18 +175,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) dgemm_kernel(GemmDesc d, int t
 #pragma unroll
         for (int j = 0; j < NI; ++j) {
             int col = n0 + wn * (NI * 8) + j * 8 + 2 * r;
-            double *c = Cp + row_off + col;
-            if (vecC && col + 1 < d.N) {
-                double2 v;
-                if (d.beta != 0.0) {
-                    v = *reinterpret_cast<double2 *>(c);
-                    v.x = d.alpha * acc[i][j][0] + d.beta * v.x; v.y = d.alpha * acc[i][j][1] + d.beta * v.y;
-                } else { v.x = d.alpha * acc[i][j][0]; v.y = d.alpha * acc[i][j][1]; }
-                *reinterpret_cast<double2 *>(c) = v;
-            } else {
-                if (col < d.N) c[0] = d.alpha * acc[i][j][0] + (d.beta != 0.0 ? d.beta * c[0] : 0.0);
-                if (col + 1 < d.N) c[1] = d.alpha * acc[i][j][1] + (d.beta != 0.0 ? d.beta * c[1] : 0.0);
-            }
+            risp_store_c_pair(d, Cp, row_off, col, acc[i][j][0], acc[i][j][1], vecC);
         }
     }
 }

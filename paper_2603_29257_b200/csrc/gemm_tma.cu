@@ -160,7 +160,7 @@ __global__ void __launch_bounds__(NT, 1) dgemm_tma_kernel(const __grid_constant_
     auto offA_mc = [&](int s, int i) { return frag_off<false>(wm * WMROWS + i * 8 + q, kstep[s]); };
     int slot = 0;
     unsigned par = 0;
-    const bool vecC = ((d.ldc & 1) == 0) && ((d.c_gstride & 1) == 0) && ((d.sC1 & 1) == 0) && ((d.sC2 & 1) == 0) && ((((size_t)d.C) & 15) == 0);
+    const bool vecC = ((d.ldc & 1) == 0) && ((d.c_gstride & 1) == 0) && ((d.c_cgstride & 1) == 0) && ((d.sC1 & 1) == 0) && ((d.sC2 & 1) == 0) && ((((size_t)d.C) & 15) == 0);
 
     for (int ti = 0; ti < my_tiles; ++ti) {
         double acc[MI][4][2];
@@ -212,18 +212,7 @@ __global__ void __launch_bounds__(NT, 1) dgemm_tma_kernel(const __grid_constant_
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const int col = n0 + wn * 32 + j * 8 + 2 * r;
-                double *c = Cp + row_off + col;
-                if (vecC && col + 1 < d.N) {
-                    double2 v;
-                    if (d.beta != 0.0) {
-                        v = *reinterpret_cast<double2 *>(c);
-                        v.x = d.alpha * acc[i][j][0] + d.beta * v.x; v.y = d.alpha * acc[i][j][1] + d.beta * v.y;
-                    } else { v.x = d.alpha * acc[i][j][0]; v.y = d.alpha * acc[i][j][1]; }
-                    *reinterpret_cast<double2 *>(c) = v;
-                } else {
-                    if (col < d.N) c[0] = d.alpha * acc[i][j][0] + (d.beta != 0.0 ? d.beta * c[0] : 0.0);
-                    if (col + 1 < d.N) c[1] = d.alpha * acc[i][j][1] + (d.beta != 0.0 ? d.beta * c[1] : 0.0);
-                }
+                risp_store_c_pair(d, Cp, row_off, col, acc[i][j][0], acc[i][j][1], vecC);
             }
         }
     }

@@ -319,7 +319,8 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
             RISP_CUDA_TRY(risp_expand_sym(pij, ctx->tri_o, no, c.np, wTij, (long long)pc * no_p, no_p, st)); ++launches;
             if (c.host) RISP_CUDA_TRY(cudaEventRecord(ctx->evStageFree[buf], st));
             if (ci == 0) RISP_CUDA_TRY(cudaEventRecord(ev[11], st));
-            // M[mi][P][j][a] = sum_b X'[mi][j][b] T_ab^P[a][b]; rows (mi,j) of one P are split by mi
+            // M[mi][P][j][a] = sum_b X'[mi][j][b] T_ab^P[a][b]; rows (mi,j) of one P are split by mi.  (One product over N = (P, a)
+            // with the column-split epilogue of GemmDesc was measured too: fewer padded tiles, same time -- the batched form stays.)
             GemmDesc d = gemm_desc(m * no, nv, nv, wXk, nv_p, true, wTab, nv_p, true, wM, nv_p);
             d.nb1 = c.np; d.sB1 = (long long)nv * nv_p; d.sC1 = (long long)no_p * nv_p;
             d.c_rpg = no; d.c_gstride = (long long)pc * no_p * nv_p;

@@ -75,6 +75,32 @@ def test_dgemm_tma_tile_heights(torch_cuda, a_kc, b_kc, M):
     assert float((outs[0] - outs[1]).abs().max()) <= 1e-12 * float(ref.abs().max() + 1)
 
 
+@pytest.mark.parametrize("no,nv", [(7, 10), (6, 9), (11, 33)])
+@pytest.mark.parametrize("variant", [1, 0])
+def test_dgemm_row_and_column_split_epilogue(torch_cuda, no, nv, variant):
+    """Eq. 22 as one product over N = (P, a): rows (mi, j) split by mi, columns (P, a) split by P, into M[mi][P][j][a] with padded
+    leading dimensions (odd and even block widths: a column pair may straddle two P blocks)."""
+    torch = torch_cuda
+    from paper_2603_29257_b200 import load_library
+    lib = load_library()
+    m, npc, pc = 5, 4, 6
+    no_p, nv_p = no + (no & 1), nv + (nv & 1)
+    X = torch.randn((m * no, nv_p), dtype=torch.float64, device="cuda")
+    T = torch.randn((npc * nv, nv_p), dtype=torch.float64, device="cuda")
+    Mout = torch.full((m, pc, no_p, nv_p), -7.0, dtype=torch.float64, device="cuda")
+    lib.risp_debug_set_gemm_variant(variant)
+    rc = lib.risp_debug_dgemm_split(m * no, npc * nv, nv, X.data_ptr(), nv_p, T.data_ptr(), nv_p, Mout.data_ptr(), nv_p,
+                                    no, pc * no_p * nv_p, nv, no_p * nv_p, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    lib.risp_debug_set_gemm_variant(1)
+    assert rc == 0
+    ref = torch.einsum('mjb,pab->mpja', X[:, :nv].reshape(m, no, nv), T[:, :nv].reshape(npc, nv, nv))
+    got = Mout[:, :npc, :no, :nv]
+    assert float((got - ref).abs().max()) <= 1e-12 * float(ref.abs().max() + 1)
+    untouched = Mout.clone(); untouched[:, :npc, :no, :nv] = -7.0
+    assert bool((untouched == -7.0).all())                       # padding rows / columns / unused P slots are never written
+
+
 def test_dgemm_batched(torch_cuda):
     torch = torch_cuda
     from paper_2603_29257_b200 import load_library
