@@ -262,11 +262,18 @@ def main():
             line["cpu_baseline"] = dict(value=ms_ / dt, unit=UNIT, cores=os.cpu_count(), kind="oracle",
                                         sample=f"one oracle.sigma call on {ms_} of the {m} trial vectors ({dt:.1f} s); tensor build ({tb:.1f} s) excluded like risp_setup",
                                         gpu_vs_oracle_rel_err=err)
+        oracle_for_solve = o if (not args.no_cpu_baseline and world == 1 and not big and args.config <= 2) else None
         if args.solve:
             omega, _, info = ctx.tda_solve(s["nroots"], tol=1e-5, max_iter=args.solve_max_iter, allow_unconverged=True)
             line["solve"] = dict(nroots=s["nroots"], tol=1e-5, wall_s=info["sec_total"], matvec_s=info["sec_matvec"], alloc_s=info["sec_alloc"], subspace_s=info["sec_subspace"], cached_vectors=info["cached_vectors"], iterations=info["iterations"],
                                  n_sigma=info["n_sigma"], restarts=info["restarts"], converged=info["converged"], omega_ev=[float(x) * 27.211386245988 for x in omega],
                                  h2d_gb=info["bytes_h2d"] / 1e9, d2h_gb=info["bytes_d2h"] / 1e9)
+            if oracle_for_solve is not None:      # the CPU oracle's own Davidson on the same problem (reported baseline; same tolerance)
+                t0 = time.time()
+                th_ref, _, iref = oracle_for_solve.davidson(s["nroots"], tol=1e-5)
+                line["solve"]["cpu_oracle"] = dict(wall_s=time.time() - t0, iterations=int(iref["iterations"]), n_sigma=int(iref["n_sigma"]),
+                                                   converged=bool(iref["converged"]), cores=os.cpu_count(),
+                                                   max_abs_diff_ev=float(np.abs(np.asarray(omega) - th_ref).max() * 27.211386245988))
         print(json.dumps(line))
     ctx.close()
     if world > 1:
