@@ -95,6 +95,7 @@ extern "C" int risp_eri3c_shell(risp_ctx *ctx, int32_t shl_i, int32_t shl_j, int
     c.g = ctx->h_aux_exp[aux_k];
     c.ns = std::pow(2.0 * c.g / 3.14159265358979323846, 0.75);
     c.np = c.ns * 2.0 * std::sqrt(c.g);
+    c.ig = 1.0 / c.g;
     c.qs = lk == 0 ? 0 : -1; c.qp = lk == 1 ? 0 : -1;
     ShellPair *d_sp = nullptr; PrimPair *d_pp = nullptr; AuxCentre *d_c = nullptr; double *d_out = nullptr;
     RISP_CUDA_TRY(cudaMalloc((void **)&d_sp, sizeof(sp)));

@@ -69,6 +69,7 @@ struct PrimPair {        // one primitive pair of a shell pair
     double p;            // a + b
     double Px, Py, Pz;   // (a A + b B)/p
     double cc;           // d_a d_b exp(-a b/p |AB|^2) * 2 pi^{5/2} / p   (d = contraction coef * radial norm)
+    double hp;           // 1 / (2p), precomputed: the recursion then needs no FP64 division
 };
 struct ShellPair {       // l(A) >= l(B)
     double Ax, Ay, Az;
@@ -82,6 +83,7 @@ struct AuxCentre {       // s and p functions sharing one exponent on one atom
     double x, y, z, g;
     double ns, np;       // normalisation of the s and of the p functions
     int qs, qp;          // function index of s (or -1) and of p_x (or -1) in the target aux set
+    double ig;           // 1 / g
 };
 struct OpParams { double ca, cb, w2; };   // operator (ca + cb erf(w r))/r, w2 = w*w
 
@@ -93,12 +95,12 @@ __device__ __forceinline__ void vrr(const PrimPair &pp, double Ax, double Ay, do
                                     double &WCx, double &WCy, double &WCz, double &c3)
 {
     const double p = pp.p, g = ax.g;
-    const double q = p + g, iq = 1.0 / q;
+    const double q = p + g, rsq = rsqrt(q), iq = rsq * rsq;     // 1/(p+g) from the reciprocal square root the prefactor needs anyway
     const double rho = p * g * iq;
     const double PCx = pp.Px - ax.x, PCy = pp.Py - ax.y, PCz = pp.Pz - ax.z;
     const double r2 = PCx * PCx + PCy * PCy + PCz * PCz;
     const double T = rho * r2;
-    const double pref = pp.cc * rsqrt(q) / g;               // cc carries 2 pi^{5/2}/p
+    const double pref = pp.cc * rsq * ax.ig;                // cc carries 2 pi^{5/2}/p
     double F[MTOP + 1];
     boys<MTOP>(T, boys_tab, F);
     if (ERF) {
@@ -118,7 +120,7 @@ __device__ __forceinline__ void vrr(const PrimPair &pp, double Ax, double Ay, do
     const double PA[3] = {pp.Px - Ax, pp.Py - Ay, pp.Pz - Az};
     const double c2 = g * iq;                                // rho / p
     const double WP[3] = {-c2 * PCx, -c2 * PCy, -c2 * PCz};  // W - P
-    const double c1 = 0.5 / p;
+    const double c1 = pp.hp;
 #pragma unroll
     for (int n = 1; n <= L; ++n) {
 #pragma unroll

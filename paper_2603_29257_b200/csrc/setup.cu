@@ -88,6 +88,7 @@ void build_centres(const risp_ctx *ctx, const std::vector<int> &fn_of_shell, std
         c.g = ctx->h_aux_exp[s];
         c.ns = std::pow(2.0 * c.g / PI, 0.75);
         c.np = c.ns * 2.0 * std::sqrt(c.g);
+        c.ig = 1.0 / c.g;
         c.qs = c.qp = -1;
         for (int t = s; t < naux; ++t) {
             if (used[t] || fn_of_shell[t] < 0 || ctx->h_aux_atom[t] != at || ctx->h_aux_exp[t] != c.g) continue;
@@ -119,6 +120,7 @@ int build_metric(risp_ctx *ctx, const std::vector<int> &fn_of_shell, int nfn, co
             PrimPair p;
             p.p = g; p.Px = r.Ax; p.Py = r.Ay; p.Pz = r.Az;
             p.cc = radial_norm(g, l) * std::sqrt(4.0 * PI) * 2.0 * std::pow(PI, 2.5) / g;
+            p.hp = 0.5 / g;
             sp.push_back(r); pp.push_back(p);
         }
         if (sp.empty()) continue;
@@ -168,6 +170,7 @@ static double pair_estimate_and_build(const risp_ctx *ctx, int shA, int shB, She
             q.p = p;
             q.Px = (a * A[0] + b * B[0]) / p; q.Py = (a * A[1] + b * B[1]) / p; q.Pz = (a * A[2] + b * B[2]) / p;
             q.cc = da * db * kab * 2.0 * std::pow(PI, 2.5) / p;
+            q.hp = 0.5 / p;
             pp.push_back(q);
         }
     sp.npp = (int)pp.size() - sp.ppoff;
