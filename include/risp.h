@@ -25,7 +25,7 @@
  *     function) or l = 1 (x, y, z).  Function index = running index over `aux_*` shells in the given order.
  *     The caller supplies the exponents theta/R_A^2 and omits hydrogens.
  *   - pointers in risp_system are HOST pointers, read during risp_setup only and never retained.
- *   - one context per host thread at a time; no global state.
+ *   - one context per host thread at a time; no global state.  Test and tuning exports are declared in risp_debug.h.
  */
 #ifndef RISP_H
 #define RISP_H
@@ -88,6 +88,7 @@ typedef struct {
 
 #define RISP_FLAG_KEEP_STAGES 1   /* keep J_mia of the last risp_matvec for risp_get_stage (costs one more [m][nocc][nvir] buffer) */
 #define RISP_FLAG_SPILL_HALF 2    /* testing: place the upper half of the K-tensor slices in pinned host memory regardless of the budget */
+#define RISP_FLAG_SMALL_KBUILD 4  /* testing: build the K tensors in runs of at most 5 auxiliary functions (the large-system code path) */
 
 typedef struct {
     double tol;                 /* residual 2-norm threshold (0 -> 1e-5) */
@@ -95,10 +96,21 @@ typedef struct {
     int32_t n_guess;            /* initial unit vectors on the smallest e_a - e_i (0 -> 2*nroots) */
     int32_t max_sub;            /* restart when the subspace would exceed this (0 -> 20*nroots) */
     int32_t flags;              /* RISP_SOLVE_* */
+    int32_t max_block;          /* trial vectors per sigma-build inside the solver (0 -> min(32, max_batch of risp_setup, n_guess)); the
+                                   solver holds two blocks of this many vectors on the device, everything else of the subspace is
+                                   cached in what HBM is left or streamed from pinned host memory */
+    int32_t reserved;
+    size_t device_budget_bytes; /* device memory the solver may allocate (0 -> what is free after the matvec work space); if two
+                                   blocks and the streaming buffers do not fit: RISP_ENOMEM, nothing stays allocated */
 } risp_solve_options;
 
-#define RISP_SOLVE_NO_CACHE 1     /* every pass over V, W streams from pinned host memory (no device cache) */
-#define RISP_SOLVE_TINY_CACHE 2   /* testing: cache only nroots + 2 vectors, the rest is streamed */
+#define RISP_SOLVE_NO_CACHE 1        /* every pass over V, W streams from pinned host memory (no device cache) */
+#define RISP_SOLVE_TINY_CACHE 2      /* testing: cache only nroots + 2 vectors, the rest is streamed */
+#define RISP_SOLVE_PERTURBED_GUESS 4 /* guess = unit vectors + seeded dense noise (relative norm 0.3), orthonormalised: a second,
+                                        different start to check that no lower root was missed */
+#define RISP_SOLVE_HOST_FP32 8       /* host-resident part of V, W stored in single precision (the paper's storage precision,
+                                        PAPER.md:201); every product still accumulates in FP64.  Trial vectors are rounded to
+                                        FP32-representable values before their sigma-build, so V is stored exactly */
 
 #define RISP_MAX_ROOTS 64
 typedef struct {
@@ -109,6 +121,9 @@ typedef struct {
     int32_t subspace_max;                /* largest subspace held */
     int32_t cached_vectors;              /* leading vectors of V and of W kept in HBM as well */
     double sec_alloc;                    /* wall seconds spent allocating the pinned subspace and the device buffers */
+    int32_t block;                       /* trial vectors per sigma-build the solver used */
+    int32_t capacity;                    /* subspace vectors the device cache and the pinned-host budget hold together */
+    double bytes_host_subspace;          /* pinned host bytes reserved for V and W */
 } risp_solve_info;
 
 typedef struct {
@@ -138,7 +153,9 @@ int risp_setup(const risp_system *sys, const risp_options *opt, risp_ctx **out);
 
 /* sigma = A X for a batch of m trial vectors.  X_dev, sigma_dev: DEVICE pointers, [m][nocc][nvir] row-major,
  * sigma overwritten, X not modified, the two must not overlap.  Asynchronous on `cuda_stream` (a cudaStream_t;
- * NULL = default stream). */
+ * NULL = default stream).  Any m >= 1 is accepted: the call works through sub-batches of at most 32 vectors (one lane per
+ * trial vector in the integral passes); the work space grows to min(m, 32) vectors if `max_batch` of risp_setup was smaller
+ * (RISP_ENOMEM if that no longer fits beside the K tensors).  risp_get_timings / risp_get_stage refer to the last sub-batch. */
 int risp_matvec(risp_ctx *ctx, int32_t m, const double *X_dev, double *sigma_dev, void *cuda_stream);
 
 /* Same with HOST buffers: copies X in, runs risp_matvec, copies sigma out, synchronises. */

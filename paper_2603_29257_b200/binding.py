@@ -14,6 +14,7 @@ EXPORTED_SYMBOLS = ["risp_setup", "risp_matvec", "risp_matvec_host", "risp_tda_s
 
 RISP_MAX_ROOTS = 64
 FLAG_KEEP_STAGES, FLAG_SPILL_HALF = 1, 2
+SOLVE_NO_CACHE, SOLVE_TINY_CACHE, SOLVE_PERTURBED_GUESS, SOLVE_HOST_FP32 = 1, 2, 4, 8
 STAGE = dict(R=1, RTILDE=2, J=3, K=4, TIJ=5, TAB=6, PAIRS=7, METRIC_J=8, METRIC_K=9, U=10)
 _ERR = {-1: "RISP_EINVAL", -2: "RISP_ENOMEM", -3: "RISP_ECUDA", -4: "RISP_ENOTPD", -5: "RISP_ENOTCONV"}
 
@@ -42,13 +43,15 @@ class _Options(C.Structure):
 
 
 class _SolveOptions(C.Structure):
-    _fields_ = [("tol", C.c_double), ("max_iter", C.c_int32), ("n_guess", C.c_int32), ("max_sub", C.c_int32), ("flags", C.c_int32)]
+    _fields_ = [("tol", C.c_double), ("max_iter", C.c_int32), ("n_guess", C.c_int32), ("max_sub", C.c_int32), ("flags", C.c_int32),
+                ("max_block", C.c_int32), ("reserved", C.c_int32), ("device_budget_bytes", C.c_size_t)]
 
 
 class _SolveInfo(C.Structure):
     _fields_ = [("iterations", C.c_int32), ("restarts", C.c_int32), ("n_sigma", C.c_int32), ("converged", C.c_int32),
                 ("resid", C.c_double * RISP_MAX_ROOTS), ("sec_total", C.c_double), ("sec_matvec", C.c_double),
-                ("sec_subspace", C.c_double), ("bytes_h2d", C.c_double), ("bytes_d2h", C.c_double), ("subspace_max", C.c_int32), ("cached_vectors", C.c_int32), ("sec_alloc", C.c_double)]
+                ("sec_subspace", C.c_double), ("bytes_h2d", C.c_double), ("bytes_d2h", C.c_double), ("subspace_max", C.c_int32), ("cached_vectors", C.c_int32), ("sec_alloc", C.c_double),
+                ("block", C.c_int32), ("capacity", C.c_int32), ("bytes_host_subspace", C.c_double)]
 
 
 class _Dims(C.Structure):
@@ -89,14 +92,12 @@ def load_library():
     lib.risp_get_timings.argtypes = [vp, C.POINTER(_Timings)]
     lib.risp_eri3c_shell.argtypes = [vp, i32, i32, i32, i32, vp]
     lib.risp_get_stage.argtypes = [vp, i32, vp, i64, vp]
+    # include/risp_debug.h
     lib.risp_debug_dgemm.argtypes = [C.c_int, C.c_int, C.c_int, vp, C.c_longlong, C.c_int, vp, C.c_longlong, C.c_int, vp, C.c_longlong,
-                                     dbl, dbl, C.c_int, C.c_longlong, C.c_longlong, C.c_longlong, vp]
-    lib.risp_debug_dgemm_split.argtypes = [C.c_int, C.c_int, C.c_int, vp, C.c_longlong, vp, C.c_longlong, vp, C.c_longlong,
-                                           C.c_int, C.c_longlong, C.c_int, C.c_longlong, vp]
-    lib.risp_debug_sym_eig.argtypes = [C.c_int, vp, vp, vp]
+                                     dbl, dbl, C.c_int, C.c_longlong, C.c_longlong, C.c_longlong, C.c_int, C.c_int, C.c_longlong, vp]
     lib.risp_debug_sym_eig_lowest.argtypes = [C.c_int, C.c_int, vp, vp, vp]
     lib.risp_debug_force_plan.argtypes = [vp, C.c_int, C.c_int, C.c_int]
-    lib.risp_debug_set_gemm_variant.argtypes = [C.c_int]
+    lib.risp_debug_yardstick.argtypes = [vp, C.c_int, C.c_size_t, C.c_int, C.POINTER(dbl)]
     _LIB = lib
     return lib
 
@@ -181,11 +182,12 @@ class RispContext:
         """Host buffers given as raw addresses (e.g. pinned torch tensors)."""
         self._check(self.lib.risp_matvec_host(self.handle, m, x_ptr, s_ptr))
 
-    def tda_solve(self, nroots, tol=1e-5, max_iter=100, n_guess=0, max_sub=0, want_vectors=False, allow_unconverged=False, flags=0):
+    def tda_solve(self, nroots, tol=1e-5, max_iter=100, n_guess=0, max_sub=0, want_vectors=False, allow_unconverged=False, flags=0,
+                  max_block=0, device_budget_bytes=0):
         import torch
         omega = np.zeros(nroots)
         info = _SolveInfo()
-        opt = _SolveOptions(float(tol), int(max_iter), int(n_guess), int(max_sub), int(flags))
+        opt = _SolveOptions(float(tol), int(max_iter), int(n_guess), int(max_sub), int(flags), int(max_block), 0, int(device_budget_bytes))
         X = torch.empty((nroots, self.nocc, self.nvir), dtype=torch.float64, device=f"cuda:{self.device}") if want_vectors else None
         rc = self.lib.risp_tda_solve(self.handle, nroots, C.byref(opt), omega.ctypes.data_as(C.POINTER(C.c_double)),
                                      X.data_ptr() if X is not None else None, C.byref(info))
@@ -198,6 +200,12 @@ class RispContext:
     def force_plan(self, mj: int = 0, prow: int = 0, pc: int = 0):
         """Testing: override the work-space plan (J sub-batch, AO rows per panel, K aux chunk); 0 keeps the automatic choice."""
         self._check(self.lib.risp_debug_force_plan(self.handle, mj, prow, pc))
+
+    def yardstick(self, which: int, nbytes: int = 0, reps: int = 5) -> float:
+        """risp_debug_yardstick: 0 DFMA flop/s, 1 DMMA flop/s, 2 device copy bytes/s (read + write)."""
+        out = C.c_double(0.0)
+        self._check(self.lib.risp_debug_yardstick(self.handle, which, nbytes, reps, C.byref(out)))
+        return out.value
 
     # ---- getters
     def dims(self) -> dict:

@@ -9,13 +9,13 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "librisp.so")
-SOURCES = ["gemm.cu", "gemm_tma.cu", "eri_kernels.cu", "linalg.cu", "elementwise.cu", "setup.cu", "matvec.cu", "solve.cu", "api.cu"]
+SOURCES = ["gemm.cu", "gemm_tma.cu", "eri_kernels.cu", "linalg.cu", "elementwise.cu", "setup.cu", "matvec.cu", "solve.cu", "host_eig.cu", "yardstick.cu", "api.cu"]
 NVCC_FLAGS = ["-std=c++17", "--extended-lambda", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo",
               "-Xcompiler", "-fPIC"]
 
 
 def _newest_source() -> float:
-    t = os.path.getmtime(os.path.join(HERE, "..", "include", "risp.h"))
+    t = max(os.path.getmtime(os.path.join(HERE, "..", "include", f)) for f in ("risp.h", "risp_debug.h"))
     for f in os.listdir(CSRC):
         t = max(t, os.path.getmtime(os.path.join(CSRC, f)))
     return t

@@ -97,11 +97,12 @@ extern "C" int risp_eri3c_shell(risp_ctx *ctx, int32_t shl_i, int32_t shl_j, int
     c.np = c.ns * 2.0 * std::sqrt(c.g);
     c.ig = 1.0 / c.g;
     c.qs = lk == 0 ? 0 : -1; c.qp = lk == 1 ? 0 : -1;
+    DevScratch scr;
     ShellPair *d_sp = nullptr; PrimPair *d_pp = nullptr; AuxCentre *d_c = nullptr; double *d_out = nullptr;
-    RISP_CUDA_TRY(cudaMalloc((void **)&d_sp, sizeof(sp)));
-    RISP_CUDA_TRY(cudaMalloc((void **)&d_pp, pp.size() * sizeof(PrimPair)));
-    RISP_CUDA_TRY(cudaMalloc((void **)&d_c, sizeof(c)));
-    RISP_CUDA_TRY(cudaMalloc((void **)&d_out, (size_t)nk * nfa * nfb * sizeof(double)));
+    RISP_CUDA_TRY(scr.alloc(d_sp, 1));
+    RISP_CUDA_TRY(scr.alloc(d_pp, pp.size()));
+    RISP_CUDA_TRY(scr.alloc(d_c, 1));
+    RISP_CUDA_TRY(scr.alloc(d_out, (size_t)nk * nfa * nfb));
     RISP_CUDA_TRY(cudaMemcpy(d_sp, &sp, sizeof(sp), cudaMemcpyHostToDevice));
     RISP_CUDA_TRY(cudaMemcpy(d_pp, pp.data(), pp.size() * sizeof(PrimPair), cudaMemcpyHostToDevice));
     RISP_CUDA_TRY(cudaMemcpy(d_c, &c, sizeof(c), cudaMemcpyHostToDevice));
@@ -110,7 +111,6 @@ extern "C" int risp_eri3c_shell(risp_ctx *ctx, int32_t shl_i, int32_t shl_j, int
     RISP_CUDA_TRY(risp_eri_fill(la, lb, lk == 1, op == 1, d_sp, 1, d_pp, d_c, 1, o, ctx->d_boys, d_out, (long long)nfa * nfb, nfb, 0, 0));
     std::vector<double> h((size_t)nk * nfa * nfb);
     RISP_CUDA_TRY(cudaMemcpy(h.data(), d_out, h.size() * sizeof(double), cudaMemcpyDeviceToHost));
-    cudaFree(d_sp); cudaFree(d_pp); cudaFree(d_c); cudaFree(d_out);
     // h[k][a][b] -> out[i][j][k]
     const int nfi = swapped ? nfb : nfa, nfj = swapped ? nfa : nfb;
     for (int i = 0; i < nfi; ++i)
@@ -129,6 +129,7 @@ extern "C" int risp_get_stage(risp_ctx *ctx, int32_t which, const int64_t *sel, 
     RISP_CUDA_TRY(cudaDeviceSynchronize());
     const int m = ctx->last_m;
     double *out = (double *)out_host;
+    DevScratch scr;
     auto need_mv = [&]() { if (!m) { risp_set_error(ctx, "risp_get_stage: no risp_matvec has run"); return true; } return false; };
     switch (which) {
     case RISP_STAGE_R:
@@ -148,11 +149,10 @@ extern "C" int risp_get_stage(risp_ctx *ctx, int32_t which, const int64_t *sel, 
         size_t n = (size_t)m * ctx->nocc * ctx->nvir;
         if (!ctx->has_K) { std::memset(out, 0, n * 8); return RISP_OK; }
         double *tmp = nullptr;
-        RISP_CUDA_TRY(cudaMalloc((void **)&tmp, n * 8));
+        RISP_CUDA_TRY(scr.alloc(tmp, n));
         const double *wKk = ctx->w_arena + (size_t)m * ctx->noccK * ctx->nv_p;     // K' of the last matvec (matvec.cu arena layout)
         RISP_CUDA_TRY(risp_scatter_window(wKk, tmp, m, ctx->nocc, ctx->nvir, ctx->occK0, ctx->noccK, ctx->virK0, ctx->nvirK, ctx->nv_p, 0));
         RISP_CUDA_TRY(cudaMemcpy(out, tmp, n * 8, cudaMemcpyDeviceToHost));
-        cudaFree(tmp);
         return RISP_OK;
     }
     case RISP_STAGE_TIJ:
@@ -162,10 +162,10 @@ extern "C" int risp_get_stage(risp_ctx *ctx, int32_t which, const int64_t *sel, 
         const size_t n = ij ? ctx->noccK : ctx->nvirK, nK = ctx->nauxK;
         const long long tri = ij ? ctx->tri_o : ctx->tri_v;
         double *full = nullptr, *pk = nullptr;
-        RISP_CUDA_TRY(cudaMalloc((void **)&full, n * n * 8));
-        RISP_CUDA_TRY(cudaMalloc((void **)&pk, (size_t)tri * 8));
+        RISP_CUDA_TRY(scr.alloc(full, n * n));
+        RISP_CUDA_TRY(scr.alloc(pk, (size_t)tri));
         for (int64_t s = 0; s < nsel; ++s) {
-            if (sel[s] < 0 || sel[s] >= (int64_t)nK) { risp_set_error(ctx, "risp_get_stage: aux index out of range"); cudaFree(full); cudaFree(pk); return RISP_EINVAL; }
+            if (sel[s] < 0 || sel[s] >= (int64_t)nK) { risp_set_error(ctx, "risp_get_stage: aux index out of range"); return RISP_EINVAL; }
             const double *src;
             if (sel[s] < ctx->nK_dev) src = (ij ? ctx->d_TijP : ctx->d_TabP) + (size_t)sel[s] * tri;
             else {
@@ -175,7 +175,6 @@ extern "C" int risp_get_stage(risp_ctx *ctx, int32_t which, const int64_t *sel, 
             RISP_CUDA_TRY(risp_expand_sym(src, tri, (int)n, 1, full, (long long)n, 0, 0));
             RISP_CUDA_TRY(cudaMemcpy(out + s * n * n, full, n * n * 8, cudaMemcpyDeviceToHost));
         }
-        cudaFree(full); cudaFree(pk);
         return RISP_OK;
     }
     case RISP_STAGE_PAIRS:
@@ -193,12 +192,11 @@ extern "C" int risp_get_stage(risp_ctx *ctx, int32_t which, const int64_t *sel, 
         if (need_mv() || !sel || sel[0] < 0 || sel[0] >= m) return RISP_EINVAL;
         double *tmp = nullptr;
         const size_t n = (size_t)ctx->nao * ctx->ldao;
-        RISP_CUDA_TRY(cudaMalloc((void **)&tmp, n * 8));
+        RISP_CUDA_TRY(scr.alloc(tmp, n));
         RISP_CUDA_TRY(cudaMemset(tmp, 0, n * 8));
         for (int c = 0; c < 6; ++c)
             RISP_CUDA_TRY(risp_e0_to_U(ctx->cls[c], 0, ctx->cls[c].npairs, 1, (int)sel[0], 0, ctx->ldao, (long long)n, 0, ctx->w_dbar, tmp, 0));
         RISP_CUDA_TRY(cudaMemcpy2D(out, (size_t)ctx->nao * 8, tmp, (size_t)ctx->ldao * 8, (size_t)ctx->nao * 8, ctx->nao, cudaMemcpyDeviceToHost));
-        cudaFree(tmp);
         return RISP_OK;
     }
     default:
@@ -207,27 +205,16 @@ extern "C" int risp_get_stage(risp_ctx *ctx, int32_t which, const int64_t *sel, 
     }
 }
 
-// Debug export (not part of the method): the DMMA GEMM on caller-provided DEVICE buffers, used by the GEMM unit test and
-// the FP64 tensor-rate measurement of bench.py.  C = alpha op(A) op(B) + beta C, see GemmDesc in common.cuh.
+// ---- debug exports (include/risp_debug.h; not part of the method)
+// The DMMA GEMM on caller-provided DEVICE buffers: GEMM unit tests and the FP64 tensor-rate yardstick of bench.py.
+// C = alpha op(A) op(B) + beta C, see GemmDesc in common.cuh.  variant 1: TMA kernel when the operands allow it, 0: cp.async kernel.
+// c_rpg > 0: row r of C lives at (r / c_rpg) * c_gstride + (r % c_rpg) * ldc (the split-row epilogue of Eq. 22).
 extern "C" int risp_debug_dgemm(int M, int N, int K, const double *A, long long lda, int a_kc, const double *B, long long ldb, int b_kc, double *C,
-                                long long ldc, double alpha, double beta, int nbatch, long long sA, long long sB, long long sC, void *stream)
+                                long long ldc, double alpha, double beta, int nbatch, long long sA, long long sB, long long sC, int variant,
+                                int c_rpg, long long c_gstride, void *stream)
 {
     GemmDesc d = gemm_desc(M, N, K, A, lda, a_kc != 0, B, ldb, b_kc != 0, C, ldc, alpha, beta);
     d.nb1 = nbatch; d.sA1 = sA; d.sB1 = sB; d.sC1 = sC;
-    return risp_dgemm(d, (cudaStream_t)stream) == cudaSuccess ? RISP_OK : RISP_ECUDA;
-}
-
-extern "C" int risp_debug_set_gemm_variant(int v)
-{
-    risp_dgemm_set_variant(v);
-    return RISP_OK;
-}
-
-// Debug export: GEMM with the row / column split epilogue (GemmDesc::c_rpg, c_cpg), for the unit test of that addressing.
-extern "C" int risp_debug_dgemm_split(int M, int N, int K, const double *A, long long lda, const double *B, long long ldb, double *C, long long ldc,
-                                      int c_rpg, long long c_gstride, int c_cpg, long long c_cgstride, void *stream)
-{
-    GemmDesc d = gemm_desc(M, N, K, A, lda, true, B, ldb, true, C, ldc);
-    d.c_rpg = c_rpg; d.c_gstride = c_gstride; d.c_cpg = c_cpg; d.c_cgstride = c_cgstride;
+    d.variant = variant; d.c_rpg = c_rpg; d.c_gstride = c_gstride;
     return risp_dgemm(d, (cudaStream_t)stream) == cudaSuccess ? RISP_OK : RISP_ECUDA;
 }

@@ -7,6 +7,27 @@
 #define RISP_MS 32   // padded trial-vector stride of R, R~, D-bar, U-bar (one lane per trial vector)
 #define RISP_NEV 16
 
+// Temporaries of one call: everything allocated through it is released when it goes out of scope (any early return included).
+struct DevScratch {
+    std::vector<void *> v;
+    template <class T>
+    cudaError_t alloc(T *&p, size_t count)
+    {
+        p = nullptr;
+        if (count == 0) return cudaSuccess;
+        cudaError_t e = cudaMalloc((void **)&p, count * sizeof(T));
+        if (e == cudaSuccess) v.push_back(p);
+        return e;
+    }
+    template <class T>
+    void release(T *&p)
+    {
+        for (auto &q : v) if (q == (void *)p) { cudaFree(q); q = nullptr; }
+        p = nullptr;
+    }
+    ~DevScratch() { for (void *q : v) if (q) cudaFree(q); }
+};
+
 struct PairClass {                 // kept shell pairs of one (la >= lb) class, sorted by the first AO of shell A
     int la, lb, npairs;
     risp_eri::ShellPair *d_pairs;  // device
@@ -91,7 +112,8 @@ cudaError_t risp_eri_fill(int la, int lb, bool hasp, bool erf_op, const risp_eri
                           long long stride_q, long long ld, int mirror, cudaStream_t st);
 // D rows [r0, ...) (leading dimension ld, vector stride mstride) -> e0 space, lanes [lane0, lane0 + mj).  mode 0: dense, pairs
 // [p0, p1) of the aoA-sorted list; mode 1: += from the rows of shell A; mode 2: += from the rows of shell B, [p0, p1) of the aoB-sorted list
-cudaError_t risp_dens_to_e0(const PairClass &pc, int p0, int p1, int mj, int lane0, int r0, long long ld, long long mstride, int mode,
+// (mode 0 also zeroes the lanes >= m_total, so that the unused lanes of the passes never carry stale data)
+cudaError_t risp_dens_to_e0(const PairClass &pc, int p0, int p1, int mj, int lane0, int m_total, int r0, long long ld, long long mstride, int mode,
                             const double *D, double *dbar, cudaStream_t st);
 // e0 space -> U rows [r0, ...), same modes (0: block and mirror image; 1: block at the rows of A; 2: transposed block at the rows of B)
 cudaError_t risp_e0_to_U(const PairClass &pc, int p0, int p1, int mj, int lane0, int r0, long long ld, long long mstride, int mode,

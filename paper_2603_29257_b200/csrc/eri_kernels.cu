@@ -66,13 +66,23 @@ __global__ void __launch_bounds__(128) eri_fill_kernel(const ShellPair *__restri
 // Modes 1 and 2 visit every pair once each over all panels; D-bar is zeroed before.
 template <int LA, int LB>
 __global__ void __launch_bounds__(128) dens_to_e0_kernel(const ShellPair *__restrict__ pairs, const int *__restrict__ perm, int p0, int p1,
-                                                         long long e_off, int mj, int lane0, int r0, long long ld, long long mstride, int mode,
+                                                         long long e_off, int mj, int lane0, int m_total, int r0, long long ld, long long mstride, int mode,
                                                          const double *__restrict__ D, double *__restrict__ dbar)
 {
     constexpr int NE = ne_of(LA, LB);
     const int mi = threadIdx.x;
     int pi = p0 + blockIdx.x * blockDim.y + threadIdx.y;
-    if (pi >= p1 || mi >= mj) return;
+    if (pi >= p1) return;
+    if (mi >= mj) {
+        // dense mode overwrites D-bar lane by lane: the lanes beyond the batch are cleared here, so that neither pass ever works on
+        // what an earlier, larger batch left there
+        if (mode == 0 && lane0 + mi >= m_total && lane0 + mi < MS) {
+            double *z = dbar + (e_off + (long long)pi * NE) * MS + lane0 + mi;
+#pragma unroll
+            for (int e = 0; e < NE; ++e) z[(long long)e * MS] = 0.0;
+        }
+        return;
+    }
     if (mode == 2) pi = perm[pi];
     const ShellPair sp = pairs[pi];
     const bool diag = sp.shA == sp.shB;
@@ -383,14 +393,14 @@ cudaError_t risp_eri_fill(int la, int lb, bool hasp, bool erf_op, const ShellPai
     return cudaGetLastError();
 }
 
-cudaError_t risp_dens_to_e0(const PairClass &pc, int p0, int p1, int mj, int lane0, int r0, long long ld, long long mstride, int mode,
+cudaError_t risp_dens_to_e0(const PairClass &pc, int p0, int p1, int mj, int lane0, int m_total, int r0, long long ld, long long mstride, int mode,
                             const double *D, double *dbar, cudaStream_t st)
 {
     if (p1 <= p0) return cudaSuccess;
     dim3 block(32, 4), grid((p1 - p0 + 3) / 4);
     dispatch_class(pc.la, pc.lb, [&](auto LA, auto LB) {
-        dens_to_e0_kernel<decltype(LA)::value, decltype(LB)::value><<<grid, block, 0, st>>>(pc.d_pairs, pc.d_permB, p0, p1, pc.e_off, mj, lane0, r0, ld,
-                                                                                            mstride, mode, D, dbar);
+        dens_to_e0_kernel<decltype(LA)::value, decltype(LB)::value><<<grid, block, 0, st>>>(pc.d_pairs, pc.d_permB, p0, p1, pc.e_off, mj, lane0, m_total, r0,
+                                                                                            ld, mstride, mode, D, dbar);
     });
     return cudaGetLastError();
 }

@@ -165,7 +165,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) dgemm_kernel(GemmDesc d, int t
     }
     cp_async_wait<0>();
     // epilogue: thread holds C(row = q, col = 2r, 2r+1) of each 8x8 tile
-    const bool vecC = ((d.ldc & 1) == 0) && ((d.c_gstride & 1) == 0) && ((d.c_cgstride & 1) == 0) && ((((size_t)Cp) & 15) == 0);
+    const bool vecC = ((d.ldc & 1) == 0) && ((d.c_gstride & 1) == 0) && ((((size_t)Cp) & 15) == 0);
 #pragma unroll
     for (int i = 0; i < MI; ++i) {
         int row = m0 + wm * (MI * 8) + i * 8 + q;
@@ -183,11 +183,13 @@ __global__ void __launch_bounds__(C::NT, C::MINB) dgemm_kernel(GemmDesc d, int t
 template <class C, bool AKC, bool BKC, bool VECA, bool VECB>
 cudaError_t launch3(const GemmDesc &d, cudaStream_t st)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static bool attr_set[64] = {};          // per device: the attribute belongs to the function as loaded on that device
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (!attr_set[dev & 63]) {
         cudaError_t e = cudaFuncSetAttribute(dgemm_kernel<C, AKC, BKC, VECA, VECB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        attr_set[dev & 63] = true;
     }
     int tiles_m = (d.M + C::BM - 1) / C::BM, tiles_n = (d.N + C::BN - 1) / C::BN;
     dim3 grid(tiles_m * tiles_n, 1, d.nb1 * d.nb2);
@@ -217,18 +219,14 @@ cudaError_t launch1(const GemmDesc &d, cudaStream_t st)
 
 using Cfg0 = Cfg<128, 128, 16, 4, 2, 4, 1>;    // 8 warps, 1 CTA/SM, warp tile 64x32
 
-int g_variant = 1;   // 1: TMA kernel (gemm_tma.cu) whenever the operands allow it; 0: always the cp.async kernel
-
 }  // namespace
 
 cudaError_t risp_dgemm_tma(const GemmDesc &d, cudaStream_t st);   // gemm_tma.cu
 
-void risp_dgemm_set_variant(int v) { g_variant = v; }
-
 cudaError_t risp_dgemm(const GemmDesc &d, cudaStream_t st)
 {
     if (d.M <= 0 || d.N <= 0 || d.nb1 * d.nb2 <= 0) return cudaSuccess;
-    if (g_variant != 0) {
+    if (d.variant != 0) {
         cudaError_t e = risp_dgemm_tma(d, st);
         if (e != cudaErrorNotSupported) return e;
     }

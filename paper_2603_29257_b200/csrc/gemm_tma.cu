@@ -160,7 +160,7 @@ __global__ void __launch_bounds__(NT, 1) dgemm_tma_kernel(const __grid_constant_
     auto offA_mc = [&](int s, int i) { return frag_off<false>(wm * WMROWS + i * 8 + q, kstep[s]); };
     int slot = 0;
     unsigned par = 0;
-    const bool vecC = ((d.ldc & 1) == 0) && ((d.c_gstride & 1) == 0) && ((d.c_cgstride & 1) == 0) && ((d.sC1 & 1) == 0) && ((d.sC2 & 1) == 0) && ((((size_t)d.C) & 15) == 0);
+    const bool vecC = ((d.ldc & 1) == 0) && ((d.c_gstride & 1) == 0) && ((d.sC1 & 1) == 0) && ((d.sC2 & 1) == 0) && ((((size_t)d.C) & 15) == 0);
 
     for (int ti = 0; ti < my_tiles; ++ti) {
         double acc[MI][4][2];
@@ -266,11 +266,13 @@ bool make_map(EncodeFn enc, CUtensorMap *tm, const double *p, bool kc, int MN, i
 template <bool AKC, bool BKC, int MI>
 cudaError_t launch_mi(const CUtensorMap &ma, const CUtensorMap &mb, const GemmDesc &d, const TmaArgs &ta, cudaStream_t st)
 {
-    static bool attr = false;
-    if (!attr) {
+    static bool attr[64] = {};              // per device
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (!attr[dev & 63]) {
         cudaError_t e = cudaFuncSetAttribute(dgemm_tma_kernel<AKC, BKC, MI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
         if (e != cudaSuccess) return e;
-        attr = true;
+        attr[dev & 63] = true;
     }
     const int sms = sm_count();
     constexpr int BM = 16 * MI;
@@ -300,13 +302,11 @@ int pick_mi(int M, long long col_tiles_x_batch, int sms)
 
 int sm_count()
 {
-    static int sms = 0;
-    if (!sms) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    }
-    return sms;
+    static int sms[64] = {};                // per device
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (!sms[dev & 63]) cudaDeviceGetAttribute(&sms[dev & 63], cudaDevAttrMultiProcessorCount, dev);
+    return sms[dev & 63];
 }
 
 template <bool AKC, bool BKC>

@@ -191,10 +191,10 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
                 const PairClass &pc = ctx->cls[c];
                 int p0, p1;
                 panel_pairs(pc.h_aoA, r0, r1, p0, p1);
-                if (p1 > p0) { RISP_CUDA_TRY(risp_dens_to_e0(pc, p0, p1, mj, l0, r0, ldao, mstride, dense ? 0 : 1, wD, ctx->w_dbar, ctx->cls_st[c])); ++launches; }
+                if (p1 > p0) { RISP_CUDA_TRY(risp_dens_to_e0(pc, p0, p1, mj, l0, m, r0, ldao, mstride, dense ? 0 : 1, wD, ctx->w_dbar, ctx->cls_st[c])); ++launches; }
                 if (!dense) {      // the lower-triangular pair also takes D_BA^T (reading G13), found in the panel that holds the rows of B
                     panel_pairs(pc.h_aoB, r0, r1, p0, p1);
-                    if (p1 > p0) { RISP_CUDA_TRY(risp_dens_to_e0(pc, p0, p1, mj, l0, r0, ldao, mstride, 2, wD, ctx->w_dbar, ctx->cls_st[c])); ++launches; }
+                    if (p1 > p0) { RISP_CUDA_TRY(risp_dens_to_e0(pc, p0, p1, mj, l0, m, r0, ldao, mstride, 2, wD, ctx->w_dbar, ctx->cls_st[c])); ++launches; }
                 }
             }
             if ((rc = join_classes(ctx, st))) return rc;
@@ -319,8 +319,7 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
             RISP_CUDA_TRY(risp_expand_sym(pij, ctx->tri_o, no, c.np, wTij, (long long)pc * no_p, no_p, st)); ++launches;
             if (c.host) RISP_CUDA_TRY(cudaEventRecord(ctx->evStageFree[buf], st));
             if (ci == 0) RISP_CUDA_TRY(cudaEventRecord(ev[11], st));
-            // M[mi][P][j][a] = sum_b X'[mi][j][b] T_ab^P[a][b]; rows (mi,j) of one P are split by mi.  (One product over N = (P, a)
-            // with the column-split epilogue of GemmDesc was measured too: fewer padded tiles, same time -- the batched form stays.)
+            // M[mi][P][j][a] = sum_b X'[mi][j][b] T_ab^P[a][b]; rows (mi,j) of one P are split by mi
             GemmDesc d = gemm_desc(m * no, nv, nv, wXk, nv_p, true, wTab, nv_p, true, wM, nv_p);
             d.nb1 = c.np; d.sB1 = (long long)nv * nv_p; d.sC1 = (long long)no_p * nv_p;
             d.c_rpg = no; d.c_gstride = (long long)pc * no_p * nv_p;
@@ -344,39 +343,48 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
     return RISP_OK;
 }
 
+// m > 32 is worked through in sub-batches of 32 (one lane per trial vector in the integral passes)
 extern "C" int risp_matvec(risp_ctx *ctx, int32_t m, const double *X_dev, double *sigma_dev, void *cuda_stream)
 {
     if (!ctx) return RISP_EINVAL;
-    if (m <= 0 || m > RISP_MS || !X_dev || !sigma_dev) { risp_set_error(ctx, "risp_matvec: need 1 <= m <= 32 and non-NULL device pointers"); return RISP_EINVAL; }
-    size_t bytes = (size_t)m * ctx->nocc * ctx->nvir * sizeof(double);
+    if (m <= 0 || !X_dev || !sigma_dev) { risp_set_error(ctx, "risp_matvec: need m >= 1 and non-NULL device pointers"); return RISP_EINVAL; }
+    const size_t vec = (size_t)ctx->nocc * ctx->nvir, bytes = (size_t)m * vec * sizeof(double);
     const char *x = (const char *)X_dev, *s = (const char *)sigma_dev;
     if (x < s + bytes && s < x + bytes) { risp_set_error(ctx, "risp_matvec: X and sigma overlap"); return RISP_EINVAL; }
     RISP_CUDA_TRY(cudaSetDevice(ctx->device));
-    int rc = risp_ensure_workspace(ctx, m);
+    int rc = risp_ensure_workspace(ctx, std::min<int>(m, RISP_MS));
     if (rc) return rc;
-    return risp_matvec_impl(ctx, m, X_dev, sigma_dev, (cudaStream_t)cuda_stream);
+    for (int m0 = 0; m0 < m; m0 += RISP_MS)
+        if ((rc = risp_matvec_impl(ctx, std::min<int>(RISP_MS, m - m0), X_dev + (size_t)m0 * vec, sigma_dev + (size_t)m0 * vec, (cudaStream_t)cuda_stream))) return rc;
+    return RISP_OK;
 }
 
 extern "C" int risp_matvec_host(risp_ctx *ctx, int32_t m, const double *X_host, double *sigma_host)
 {
     if (!ctx) return RISP_EINVAL;
-    if (m <= 0 || m > RISP_MS || !X_host || !sigma_host) { risp_set_error(ctx, "risp_matvec_host: need 1 <= m <= 32 and non-NULL host pointers"); return RISP_EINVAL; }
+    if (m <= 0 || !X_host || !sigma_host) { risp_set_error(ctx, "risp_matvec_host: need m >= 1 and non-NULL host pointers"); return RISP_EINVAL; }
     RISP_CUDA_TRY(cudaSetDevice(ctx->device));
-    const size_t bytes = (size_t)m * ctx->nocc * ctx->nvir * sizeof(double);
-    if (m > ctx->xin_cap) {
+    const size_t vec = (size_t)ctx->nocc * ctx->nvir;
+    const int mb = std::min<int>(m, RISP_MS);
+    if (mb > ctx->xin_cap) {
         // the staging copies of X and sigma are the caller's share of HBM in this entry point: allocate them before the work space is planned
         risp_free_workspace(ctx);
-        if (ctx->w_Xin) { cudaFree(ctx->w_Xin); cudaFree(ctx->w_Sout); ctx->w_Xin = ctx->w_Sout = nullptr; ctx->xin_cap = 0; }
-        RISP_CUDA_TRY(cudaMalloc((void **)&ctx->w_Xin, bytes));
-        RISP_CUDA_TRY(cudaMalloc((void **)&ctx->w_Sout, bytes));
-        ctx->xin_cap = m;
+        if (ctx->w_Xin) { cudaFree(ctx->w_Xin); ctx->w_Xin = nullptr; }
+        if (ctx->w_Sout) { cudaFree(ctx->w_Sout); ctx->w_Sout = nullptr; }
+        ctx->xin_cap = 0;
+        RISP_CUDA_TRY(cudaMalloc((void **)&ctx->w_Xin, (size_t)mb * vec * sizeof(double)));
+        RISP_CUDA_TRY(cudaMalloc((void **)&ctx->w_Sout, (size_t)mb * vec * sizeof(double)));
+        ctx->xin_cap = mb;
     }
-    int rc = risp_ensure_workspace(ctx, m);
+    int rc = risp_ensure_workspace(ctx, mb);
     if (rc) return rc;
-    RISP_CUDA_TRY(cudaMemcpyAsync(ctx->w_Xin, X_host, bytes, cudaMemcpyHostToDevice, 0));
-    rc = risp_matvec_impl(ctx, m, ctx->w_Xin, ctx->w_Sout, 0);
-    if (rc) return rc;
-    RISP_CUDA_TRY(cudaMemcpyAsync(sigma_host, ctx->w_Sout, bytes, cudaMemcpyDeviceToHost, 0));
+    for (int m0 = 0; m0 < m; m0 += RISP_MS) {
+        const int mc = std::min<int>(RISP_MS, m - m0);
+        const size_t bytes = (size_t)mc * vec * sizeof(double);
+        RISP_CUDA_TRY(cudaMemcpyAsync(ctx->w_Xin, X_host + (size_t)m0 * vec, bytes, cudaMemcpyHostToDevice, 0));
+        if ((rc = risp_matvec_impl(ctx, mc, ctx->w_Xin, ctx->w_Sout, 0))) return rc;
+        RISP_CUDA_TRY(cudaMemcpyAsync(sigma_host + (size_t)m0 * vec, ctx->w_Sout, bytes, cudaMemcpyDeviceToHost, 0));
+    }
     RISP_CUDA_TRY(cudaStreamSynchronize(0));
     return RISP_OK;
 }

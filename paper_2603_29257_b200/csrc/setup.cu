@@ -124,15 +124,15 @@ int build_metric(risp_ctx *ctx, const std::vector<int> &fn_of_shell, int nfn, co
             sp.push_back(r); pp.push_back(p);
         }
         if (sp.empty()) continue;
+        DevScratch scr;
         ShellPair *d_sp = nullptr; PrimPair *d_pp = nullptr;
-        RISP_CUDA_TRY(cudaMalloc((void **)&d_sp, sp.size() * sizeof(ShellPair)));
-        RISP_CUDA_TRY(cudaMalloc((void **)&d_pp, pp.size() * sizeof(PrimPair)));
+        RISP_CUDA_TRY(scr.alloc(d_sp, sp.size()));
+        RISP_CUDA_TRY(scr.alloc(d_pp, pp.size()));
         RISP_CUDA_TRY(cudaMemcpy(d_sp, sp.data(), sp.size() * sizeof(ShellPair), cudaMemcpyHostToDevice));
         RISP_CUDA_TRY(cudaMemcpy(d_pp, pp.data(), pp.size() * sizeof(PrimPair), cudaMemcpyHostToDevice));
         // out[q*nfn + (aoA + i)*1 + 0]
         RISP_CUDA_TRY(risp_eri_fill(l, 0, hasp, erf_op, d_sp, (int)sp.size(), d_pp, d_cen, ncen, op, ctx->d_boys, d_M, nfn, 1, 0, 0));
         RISP_CUDA_TRY(cudaDeviceSynchronize());
-        cudaFree(d_sp); cudaFree(d_pp);
     }
     return RISP_OK;
 }
@@ -370,11 +370,12 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
         if ((rc = dalloc(ctx, ctx->d_MJ, nJ * nJ))) return rc;
         if ((rc = dalloc(ctx, ctx->d_LinvJ, nJ * nJ))) return rc;
         if ((rc = build_metric(ctx, ctx->h_aux_fn, ctx->nauxJ, ctx->d_cenJ, ctx->ncenJ, OpParams{1.0, 0.0, 0.0}, false, ctx->d_MJ))) return rc;
+        DevScratch scr;
         double *tmp = nullptr;
-        RISP_CUDA_TRY(cudaMalloc((void **)&tmp, nJ * nJ * sizeof(double)));
+        RISP_CUDA_TRY(scr.alloc(tmp, nJ * nJ));
         RISP_CUDA_TRY(cudaMemcpy(tmp, ctx->d_MJ, nJ * nJ * sizeof(double), cudaMemcpyDeviceToDevice));
         RISP_CUDA_TRY(risp_cholesky_inverse(tmp, ctx->d_LinvJ, ctx->nauxJ, &info, 0));
-        cudaFree(tmp);
+        scr.release(tmp);
         if (info) { risp_set_error(ctx, "risp_setup: Coulomb metric (P|Q)_J not positive definite at pivot " + std::to_string(info)); return RISP_ENOTPD; }
         if (ctx->has_K) {
             size_t nK = (size_t)ctx->nauxK;
@@ -383,8 +384,8 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
             OpParams opK{sys->alpha, sys->beta, sys->omega * sys->omega};
             if ((rc = build_metric(ctx, ctx->h_aux_fnK, ctx->nauxK, ctx->d_cenK, ctx->ncenK, opK, true, ctx->d_MK))) return rc;
             double *tmpL = nullptr, *tmpI = nullptr;
-            RISP_CUDA_TRY(cudaMalloc((void **)&tmpL, nK * nK * sizeof(double)));
-            RISP_CUDA_TRY(cudaMalloc((void **)&tmpI, nK * nK * sizeof(double)));
+            RISP_CUDA_TRY(scr.alloc(tmpL, nK * nK));
+            RISP_CUDA_TRY(scr.alloc(tmpI, nK * nK));
             RISP_CUDA_TRY(cudaMemcpy(tmpL, ctx->d_MK, nK * nK * sizeof(double), cudaMemcpyDeviceToDevice));
             RISP_CUDA_TRY(risp_cholesky_inverse(tmpL, tmpI, ctx->nauxK, &info, 0));
             if (!info) {
@@ -393,7 +394,6 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
                 RISP_CUDA_TRY(risp_dgemm(d, 0));
                 RISP_CUDA_TRY(cudaDeviceSynchronize());
             }
-            cudaFree(tmpL); cudaFree(tmpI);
             if (info) { risp_set_error(ctx, "risp_setup: exchange metric (P|J^|Q)_K not positive definite at pivot " + std::to_string(info)); return RISP_ENOTPD; }
         }
     }
@@ -439,24 +439,27 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
         const size_t per_fn = ((size_t)nao * ldao + (size_t)nao * nmax_p + sq + (size_t)std::max(tri_o, tri_v)) * sizeof(double);
         bool haspK = false;
         for (auto &c : cenK) if (c.qp >= 0) haspK = true;
-        const int max_fn = (int)std::max<size_t>(haspK ? 4 : 1, std::min<size_t>((size_t)nK, ((size_t)3 << 30) / per_fn));
-        double *G = nullptr, *H = nullptr, *F = nullptr, *Pk = nullptr, *CoK = nullptr, *CvK = nullptr, *BP = nullptr;
-        RISP_CUDA_TRY(cudaMalloc((void **)&G, (size_t)max_fn * nao * ldao * sizeof(double)));
-        RISP_CUDA_TRY(cudaMalloc((void **)&H, (size_t)max_fn * nao * nmax_p * sizeof(double)));
-        RISP_CUDA_TRY(cudaMalloc((void **)&F, (size_t)max_fn * sq * sizeof(double)));
-        RISP_CUDA_TRY(cudaMalloc((void **)&Pk, (size_t)max_fn * std::max(tri_o, tri_v) * sizeof(double)));
+        int max_fn = (int)std::max<size_t>(haspK ? 4 : 1, std::min<size_t>((size_t)nK, ((size_t)3 << 30) / per_fn));
+        if (ctx->flags & RISP_FLAG_SMALL_KBUILD) max_fn = std::min(max_fn, 5);
+        DevScratch scr;                                  // every temporary of the build: released on any return
+        double *G = nullptr, *H = nullptr, *F = nullptr, *Pk = nullptr, *CoK = nullptr, *CvK = nullptr, *BP = nullptr, *BPr = nullptr, *tmpc = nullptr;
+        AuxCentre *d_cenRun = nullptr;
+        RISP_CUDA_TRY(scr.alloc(G, (size_t)max_fn * nao * ldao));
+        RISP_CUDA_TRY(scr.alloc(H, (size_t)max_fn * nao * nmax_p));
+        RISP_CUDA_TRY(scr.alloc(F, (size_t)max_fn * sq));
+        RISP_CUDA_TRY(scr.alloc(Pk, (size_t)max_fn * std::max(tri_o, tri_v)));
+        RISP_CUDA_TRY(scr.alloc(d_cenRun, (size_t)ctx->ncenK));
         // window blocks of C with even leading dimensions and aligned bases
-        RISP_CUDA_TRY(cudaMalloc((void **)&CoK, (size_t)nao * no_p * sizeof(double)));
-        RISP_CUDA_TRY(cudaMalloc((void **)&CvK, (size_t)nao * nv_p * sizeof(double)));
+        RISP_CUDA_TRY(scr.alloc(CoK, (size_t)nao * no_p));
+        RISP_CUDA_TRY(scr.alloc(CvK, (size_t)nao * nv_p));
         RISP_CUDA_TRY(cudaMemset(CoK, 0, (size_t)nao * no_p * sizeof(double)));
         RISP_CUDA_TRY(cudaMemset(CvK, 0, (size_t)nao * nv_p * sizeof(double)));
         RISP_CUDA_TRY(cudaMemcpy2D(CoK, (size_t)no_p * 8, ctx->d_Cocc + ctx->occK0, (size_t)ctx->ldocc * 8, (size_t)no * 8, nao, cudaMemcpyDeviceToDevice));
         RISP_CUDA_TRY(cudaMemcpy2D(CvK, (size_t)nv_p * 8, ctx->d_Cvir + ctx->virK0, (size_t)ctx->ldvir * 8, (size_t)nv * 8, nao, cudaMemcpyDeviceToDevice));
         // all (ij|Q) slices, packed, in HBM until the metric has been applied (Eq. 20 mixes every Q): the first nK_dev of them
         // in their final place, the others in a block that is copied to the host and freed afterwards
-        double *BPr = nullptr;
         if (ctx->nK_dev > 0) { if ((rc = dalloc(ctx, ctx->d_TijP, (size_t)ctx->nK_dev * tri_o))) return rc; }
-        if (nK_host > 0) RISP_CUDA_TRY(cudaMalloc((void **)&BPr, (size_t)nK_host * tri_o * sizeof(double)));
+        if (nK_host > 0) RISP_CUDA_TRY(scr.alloc(BPr, (size_t)nK_host * tri_o));
         BP = ctx->d_TijP;
         auto bp_slice = [&](int f) { return f < ctx->nK_dev ? BP + (size_t)f * tri_o : BPr + (size_t)(f - ctx->nK_dev) * tri_o; };
         if (nK_host > 0) {
@@ -471,23 +474,28 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
             const double *Cw = pass == 0 ? CoK : CvK;
             int c0 = 0;
             while (c0 < ctx->ncenK) {
-                // centres are created in function order: a run of centres covers the contiguous function range [f0, f1)
-                int c1 = c0, f0 = 1 << 30, f1 = -1;
+                // a run of centres with at most max_fn functions; inside the run the functions get compact indices 0 .. nf-1, so the
+                // order of the caller's aux shells (grouped by atom, or all s shells first) does not matter: fn_of[j] is the
+                // function's index in the K auxiliary set
+                std::vector<AuxCentre> run;
+                std::vector<int> fn_of;
+                int c1 = c0;
                 while (c1 < ctx->ncenK) {
-                    int lo = 1 << 30, hi = -1;
-                    if (cenK[c1].qs >= 0) { lo = std::min(lo, cenK[c1].qs); hi = std::max(hi, cenK[c1].qs + 1); }
-                    if (cenK[c1].qp >= 0) { lo = std::min(lo, cenK[c1].qp); hi = std::max(hi, cenK[c1].qp + 3); }
-                    int nf0 = std::min(f0, lo), nf1 = std::max(f1, hi);
-                    if (c1 > c0 && nf1 - nf0 > max_fn) break;
-                    f0 = nf0; f1 = nf1; ++c1;
+                    const int add = (cenK[c1].qs >= 0 ? 1 : 0) + (cenK[c1].qp >= 0 ? 3 : 0);
+                    if (c1 > c0 && (int)fn_of.size() + add > max_fn) break;
+                    AuxCentre cc = cenK[c1];
+                    if (cc.qs >= 0) { fn_of.push_back(cc.qs); cc.qs = (int)fn_of.size() - 1; }
+                    if (cc.qp >= 0) { for (int t = 0; t < 3; ++t) fn_of.push_back(cenK[c1].qp + t); cc.qp = (int)fn_of.size() - 3; }
+                    run.push_back(cc);
+                    ++c1;
                 }
-                const int nf = f1 - f0;
-                if (nf > max_fn) { risp_set_error(ctx, "risp_setup: K aux functions of one centre are not contiguous"); return RISP_EINVAL; }
+                const int nf = (int)fn_of.size();
+                RISP_CUDA_TRY(cudaMemcpy(d_cenRun, run.data(), run.size() * sizeof(AuxCentre), cudaMemcpyHostToDevice));
                 RISP_CUDA_TRY(cudaMemsetAsync(G, 0, (size_t)nf * nao * ldao * sizeof(double), 0));
                 for (int c = 0; c < 6; ++c) {
                     const PairClass &pc = ctx->cls[c];
-                    RISP_CUDA_TRY(risp_eri_fill(pc.la, pc.lb, haspK, true, pc.d_pairs, pc.npairs, ctx->d_prims, ctx->d_cenK + c0, c1 - c0, opK, ctx->d_boys,
-                                                G - (long long)f0 * nao * ldao, (long long)nao * ldao, ldao, 1, 0));
+                    RISP_CUDA_TRY(risp_eri_fill(pc.la, pc.lb, haspK, true, pc.d_pairs, pc.npairs, ctx->d_prims, d_cenRun, (int)run.size(), opK, ctx->d_boys, G,
+                                                (long long)nao * ldao, ldao, 1, 0));
                 }
                 // H[P] = (mu nu|P) C_w ; F[P] = C_w^T H[P]      (Eq. 20-21 before the metric)
                 GemmDesc d1 = gemm_desc(nao, n, nao, G, ldao, true, Cw, n_p, false, H, n_p);
@@ -497,25 +505,25 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
                 d2.nb1 = nf; d2.sB1 = (long long)nao * n_p; d2.sC1 = (long long)n * n_p;
                 RISP_CUDA_TRY(risp_dgemm(d2, 0));
                 if (pass == 0) {
-                    for (int f = f0; f < f1; ++f)
-                        RISP_CUDA_TRY(risp_pack_sym(F + (size_t)(f - f0) * n * n_p, (long long)n * n_p, n_p, n, 1, bp_slice(f), tri, 0));
+                    for (int j = 0; j < nf; ++j)
+                        RISP_CUDA_TRY(risp_pack_sym(F + (size_t)j * n * n_p, (long long)n * n_p, n_p, n, 1, bp_slice(fn_of[j]), tri, 0));
                 } else {
                     RISP_CUDA_TRY(risp_pack_sym(F, (long long)n * n_p, n_p, n, nf, Pk, tri, 0));
-                    for (int f = f0; f < f1; ++f) {
-                        const double *src = Pk + (size_t)(f - f0) * tri;
+                    for (int j = 0; j < nf; ++j) {
+                        const int f = fn_of[j];
+                        const double *src = Pk + (size_t)j * tri;
                         if (f < ctx->nK_dev) RISP_CUDA_TRY(cudaMemcpyAsync(ctx->d_TabP + (size_t)f * tri, src, (size_t)tri * 8, cudaMemcpyDeviceToDevice, 0));
                         else RISP_CUDA_TRY(cudaMemcpyAsync(ctx->h_TabP + (size_t)(f - ctx->nK_dev) * tri, src, (size_t)tri * 8, cudaMemcpyDeviceToHost, 0));
                     }
-                    RISP_CUDA_TRY(cudaStreamSynchronize(0));
                 }
+                RISP_CUDA_TRY(cudaStreamSynchronize(0));      // d_cenRun and the scratch are reused by the next run
                 c0 = c1;
             }
             if (pass == 0) {
                 // T_ij^P = sum_Q (P|Q)^-1 (ij|Q)   (Eq. 20): [BP; BPr] <- MKinv [BP; BPr], in column panels, in place
                 const int nKd = ctx->nK_dev;
                 long long w = std::min<long long>(tri_o, std::max<long long>(2, (((long long)1 << 30) / ((long long)nK * 8)) & ~1LL));
-                double *tmpc = nullptr;
-                RISP_CUDA_TRY(cudaMalloc((void **)&tmpc, (size_t)nK * w * sizeof(double)));
+                RISP_CUDA_TRY(scr.alloc(tmpc, (size_t)nK * w));
                 for (long long col = 0; col < tri_o; col += w) {
                     const int wc = (int)std::min<long long>(w, tri_o - col);
                     if (nKd > 0) {
@@ -533,15 +541,14 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
                                                         cudaMemcpyDeviceToDevice, 0));
                 }
                 RISP_CUDA_TRY(cudaDeviceSynchronize());
-                cudaFree(tmpc);
+                scr.release(tmpc);
                 if (nK_host > 0) {
                     RISP_CUDA_TRY(cudaMemcpy(ctx->h_TijP, BPr, (size_t)nK_host * tri_o * 8, cudaMemcpyDeviceToHost));
-                    cudaFree(BPr); BPr = nullptr;
+                    scr.release(BPr);
                 }
             }
         }
         RISP_CUDA_TRY(cudaDeviceSynchronize());
-        cudaFree(G); cudaFree(H); cudaFree(F); cudaFree(Pk); cudaFree(CoK); cudaFree(CvK);
     }
     RISP_CUDA_TRY(cudaDeviceSynchronize());
     RISP_CUDA_TRY(cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking));

@@ -13,8 +13,10 @@ checked one by one against quantities the oracle CAN compute at full size:
   (viii) sigma: symmetry <x, A y> = <y, A x>, and independence of the memory plan (dense vs sub-batched / panelled / small
         aux chunks), which together with (vi)-(vii) and the element-wise K parity of the small configs covers Eq. 22-23.
 
-Slow (minutes) and memory hungry: runs only with RISP_LARGE=<comma separated configs>, e.g. RISP_LARGE=3,4.  The log of the
-last run is kept under profiles/.
+The 300- and 1000-atom configurations always run (about 2.5 minutes together on a B200 box); the 3000-atom one needs ~25
+minutes (11 of them risp_setup) and more than the 1200 s the driver gives `pytest -m gpu`, so it runs only with RISP_LARGE=5
+and its log is kept under profiles/.  The element-by-element comparison against the FULL oracle at 300 atoms is
+tests/test_gpu_cfg3.py.
 """
 import os
 
@@ -23,7 +25,7 @@ import pytest
 
 pytestmark = pytest.mark.gpu
 HARTREE_EV = 27.211386245988
-_CFGS = [int(c) for c in os.environ.get("RISP_LARGE", "").split(",") if c.strip()]
+_CFGS = sorted({3, 4} | {int(c) for c in os.environ.get("RISP_LARGE", "").split(",") if c.strip()})
 
 
 def _rel(a, b):
@@ -49,8 +51,7 @@ def _sub_oracle(s, shells, auxs):
     return Oracle(sub)
 
 
-@pytest.mark.skipif(not _CFGS, reason="set RISP_LARGE=3,4 to run the large-configuration parity checks")
-@pytest.mark.parametrize("cfg", _CFGS or [0])
+@pytest.mark.parametrize("cfg", _CFGS)
 def test_large_configuration_compositional_parity(cfg):
     import time
     import torch
@@ -132,8 +133,16 @@ def test_large_configuration_compositional_parity(cfg):
         assert e <= 1e-10
         U = c.stage("U", m, sel=[1])
         kept = c.stage("PAIRS")
-        worstU = 0.0
-        for idx in rng.choice(len(kept), size=12, replace=False):
+        # half of the sample from same-atom / neighbouring-atom pairs (large blocks), half uniformly from the kept list (mostly far
+        # pairs, tiny blocks); error measured PER BLOCK against the block's own norm, with the absolute floor the integral
+        # tolerance implies: |dU| <= 1e-12 * sum_P |R~_P|
+        at_of = np.asarray(s["shl_atom"])
+        dist_at = np.linalg.norm(s["xyz_bohr"][at_of[kept[:, 0]]] - s["xyz_bohr"][at_of[kept[:, 1]]], axis=1)
+        near = np.nonzero((dist_at < 3.0) & (kept[:, 0] != kept[:, 1]))[0]
+        sample = list(rng.choice(near, size=8, replace=False)) + list(rng.choice(len(kept), size=8, replace=False))
+        floor = 1e-12 * float(np.abs(Rt[:, 1]).sum())
+        worstU, worst_rel = 0.0, 0.0
+        for idx in sample:
             si, sj = int(kept[idx][0]), int(kept[idx][1])
             if si == sj:
                 continue
@@ -142,9 +151,12 @@ def test_large_configuration_compositional_parity(cfg):
             n_i = 2 * int(s["shl_l"][si]) + 1
             ref = np.einsum('pij,p->ij', I3[:, :n_i, n_i:], Rt[:, 1])
             got = U[soff[si]:soff[si + 1], soff[sj]:soff[sj + 1]]
-            worstU = max(worstU, float(np.abs(got - ref).max()) / max(float(np.abs(U).max()), 1e-300))
-        print(f"[cfg{cfg}] (iv) U on sampled kept shell pairs: max err / max|U| = {worstU:.2e}", flush=True)
-        assert worstU <= 1e-10
+            err, nrm = float(np.abs(got - ref).max()), float(np.linalg.norm(ref))
+            worstU = max(worstU, err / (1e-10 * nrm + floor))
+            worst_rel = max(worst_rel, err / max(nrm, 1e-300))
+        print(f"[cfg{cfg}] (iv) U on {len(sample)} kept shell pairs (8 near, 8 random): worst err / (1e-10 |block| + {floor:.1e}) = {worstU:.2e}; "
+              f"worst err / |block| = {worst_rel:.2e}", flush=True)
+        assert worstU <= 1.0
         assert np.abs(U - U.T).max() <= 1e-12 * np.abs(U).max()
         # ---- (v) J on sampled (i, a)
         J = c.stage("J", m)
