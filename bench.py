@@ -1,14 +1,17 @@
 #!/usr/bin/env python
 """bench.py -- sigma-builds/s of the TDA-risp hot path on seeded synthetic systems (BASELINE.json metric).
 
-A "step" is one pass of the whole hot path: one `risp_matvec` over a batch of m trial vectors (J + K + diagonal,
-all SURVEY 8(a) rows a4-a12) with the setup (pair list, metrics, K tensors) already built and X resident in HBM.
-`value` = m * K / (sum of the K device-timed steps), max over ranks; `e2e` = the same through `risp_matvec_host`
-(pinned HOST buffers, H2D and D2H inside the timed region).  Between timed iterations L2 is flushed by writing a
-512 MiB buffer.  N > 1: every rank owns its own batch of m vectors (the path shards by trial vector with no
-collective), weak scaling.
+A "step" is one pass of the whole hot path: one `risp_matvec` over a batch of m trial vectors (J + K + diagonal, all
+SURVEY 8(a) rows a4-a12) with the setup (pair list, metrics, K tensors) already built and X resident in HBM.
+`value` = m * K / (sum of the K device-timed steps), max over ranks; `e2e` = the same through `risp_matvec_host` (pinned HOST
+buffers, H2D and D2H inside the timed region).  Between timed iterations L2 is flushed by writing a 512 MiB buffer.
+The default workload is the 300-atom system (BASELINE.json configs[2], m = 30); the line also carries the metric's second
+half, the wall time of the 15-root `risp_tda_solve`, the FP64 yardsticks measured in the same run (DFMA and DMMA issue rates of
+the library's own micro-kernels, cuBLAS DGEMM through torch), one roofline entry per phase, and -- `also` -- a short run of the
+1000-atom system (and of the 3000-atom one with --also 4,5).  N > 1: every rank owns its own batch of m vectors (the path
+shards by trial vector with no collective), weak scaling.
 
-`--impl reference` times the CPU oracle (oracle/, as it stands) on the same workload, metric and unit.
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload, metric and unit.
 """
 from __future__ import annotations
 
@@ -28,6 +31,8 @@ sys.path.insert(0, ROOT)
 METRIC = "TDA-risp sigma-builds/s (15-root wall time and % of FP64 tensor/HBM roofline alongside)"
 UNIT = "sigma-builds/s"
 FP64_PER_BF16 = 45.0 / 2250.0     # nominal B200 dense FP64-tensor : bf16-tensor ratio (blackwell guide: 45 TF vs 2.25 PF)
+HARTREE_EV = 27.211386245988
+T_START = time.time()
 
 
 def _peaks():
@@ -71,69 +76,95 @@ class ClockSampler:
                     reasons=reasons, samples=len(rows))
 
 
+# ------------------------------------------------------------------------------------------------ the CPU oracle, bounded
+_AUX_ATOMS_SAMPLE = {1: None, 2: None, 3: 8, 4: 1, 5: 1}      # heavy atoms whose aux shells enter the sample (None: all of them)
+
+
+class OracleSample:
+    """The oracle as it stands on a bounded sample of the workload: `oracle.sigma`'s three terms with the auxiliary basis
+    restricted to the shells of the first few heavy atoms, timed term by term and extrapolated linearly in the number of
+    auxiliary functions (J and K are sums over auxiliary functions of equally sized pieces of work, oracle.coulomb /
+    oracle.exchange); configs 1-2 use the whole auxiliary basis and need no extrapolation."""
+
+    def __init__(self, s, m_s):
+        from oracle.risp_oracle import Oracle
+        na = _AUX_ATOMS_SAMPLE[s["cfg"]]
+        self.s, self.m_s = s, m_s
+        self.full = na is None
+        sub = s
+        if not self.full:
+            keep = np.arange(min(2 * na, len(s["aux_l"])))
+            sub = dict(s)
+            for k in ("aux_atom", "aux_l", "aux_exp", "aux_in_K"):
+                sub[k] = np.ascontiguousarray(np.asarray(s[k])[keep])
+            sub["naux"] = len(keep)
+        self.o = Oracle(sub)
+        t0 = time.time(); self.o.build(); self.t_build = time.time() - t0
+        nJ_full = int(np.sum(2 * np.asarray(s["aux_l"]) + 1)); nK_full = int(np.sum((2 * np.asarray(s["aux_l"]) + 1) * np.asarray(s["aux_in_K"])))
+        self.fJ = nJ_full / self.o.nfun(self.o.selJ)
+        self.fK = nK_full / max(self.o.nfun(self.o.selK), 1)
+        self.cores = os.cpu_count()
+
+    def step(self, X):
+        """one sample evaluation; returns the extrapolated seconds of a full oracle.sigma on these vectors"""
+        o = self.o
+        t0 = time.time(); dg = o.delta[None] * X; t_d = time.time() - t0
+        t0 = time.time(); J = o.coulomb(X); t_j = time.time() - t0
+        t0 = time.time(); K = o.exchange(X); t_k = time.time() - t0
+        self.last = (dg, J, K)
+        return t_d + self.fJ * t_j + self.fK * t_k, t_d + t_j + t_k
+
+    def describe(self, t_cpu):
+        if self.full:
+            return f"oracle.sigma (all three terms) on {self.m_s} trial vectors, whole auxiliary basis, {t_cpu:.1f} s of CPU work per call; tensor build ({self.t_build:.1f} s) excluded like risp_setup"
+        return (f"oracle diagonal + coulomb + exchange on {self.m_s} trial vectors with the auxiliary shells of the first {_AUX_ATOMS_SAMPLE[self.s['cfg']]} heavy "
+                f"atoms ({self.o.nfun(self.o.selJ)} J / {self.o.nfun(self.o.selK)} K functions), {t_cpu:.1f} s of CPU work per call, J and K times scaled by "
+                f"{self.fJ:.1f} / {self.fK:.1f} to the whole auxiliary basis; tensor build of the sample ({self.t_build:.1f} s) excluded like risp_setup")
+
+
 def run_reference(args):
-    """The CPU oracle as the reference arm: sigma-builds/s of oracle.sigma on a bounded sample of the same workload."""
+    """The CPU oracle as the reference arm: sigma-builds/s of the oracle on a bounded sample of the same workload."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    from oracle.risp_oracle import Oracle
     from workloads import make_system, trial_vectors
     s = make_system(args.config)
-    o = Oracle(s)
-    t0 = time.time(); o.build(); t_build = time.time() - t0
-    m_s = min(s["m"], args.ref_vectors)
+    m_s = min(args.batch if args.batch > 0 else s["m"], args.ref_vectors)
+    smp = OracleSample(s, m_s)
     X = trial_vectors(s)[:m_s]
     for _ in range(args.warmup):
-        o.sigma(X)
-    t0 = time.time()
+        smp.step(X)
+    t_est = t_cpu = 0.0
     for _ in range(args.steps):
-        o.sigma(X)
-    dt = time.time() - t0
-    val = m_s * args.steps / dt
-    cores = os.cpu_count()
+        a, b = smp.step(X)
+        t_est += a; t_cpu += b
+    val = m_s * args.steps / t_est
     line = dict(impl="reference", metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
-                ms_per_step=1e3 * dt / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
-                config=dict(workload=s["name"], m=m_s, nao=s["nao"], nocc=s["nocc"], nvir=s["nvir"]),
-                cpu_baseline=dict(value=val, unit=UNIT, cores=cores, kind="oracle",
-                                  sample=f"oracle.sigma on {m_s} of the {s['m']} trial vectors per step; tensor build ({t_build:.1f} s) excluded like risp_setup"),
+                ms_per_step=1e3 * t_cpu / args.steps, ms_per_step_extrapolated=1e3 * t_est / args.steps,
+                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+                config=dict(workload=s["name"], m=m_s, atoms=int(s["natm"]), nao=s["nao"], nocc=s["nocc"], nvir=s["nvir"]),
+                cpu_baseline=dict(value=val, unit=UNIT, cores=smp.cores, kind="oracle", sample=smp.describe(t_cpu / args.steps)),
                 e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
     print(json.dumps(line))
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="risp", choices=["risp", "reference"])
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index + 1 (default 2: the 100-atom system)")
-    ap.add_argument("--ref-vectors", type=int, default=30, help="trial vectors per step of the CPU oracle sample")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--batch", type=int, default=0, help="trial vectors per step (0: the config's m)")
-    ap.add_argument("--solve-max-iter", type=int, default=100)
-    ap.add_argument("--solve", action="store_true", help="also time the 15-root risp_tda_solve (reported under 'solve')")
-    args = ap.parse_args()
-    # contract: >= 3 warm-up steps; the 1000/3000-atom configs (tens of seconds to minutes per step) are allowed 1 and say so
-    args.warmup = (max(args.warmup, 3) if args.config <= 3 else max(args.warmup, 1)) if args.impl == "risp" else args.warmup
-    if args.impl == "reference":
-        return run_reference(args)
+# ------------------------------------------------------------------------------------------------ one configuration on the GPU
+def _eri_flops_per_task():
+    """FP64 thread-instructions per (shell pair, aux centre) task and pair class, counted by ncu on the pass kernels
+    (profiles/eri_flops.json; flop = 2 DFMA + DMUL + DADD)."""
+    p = os.path.join(ROOT, "profiles", "eri_flops.json")
+    return json.load(open(p)) if os.path.exists(p) else None
 
+
+def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps, warmup):
     import torch
-    import torch.distributed as dist
     from paper_2603_29257_b200 import setup
     from workloads import make_system, trial_vectors
-
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     dev = torch.device(f"cuda:{local}")
-
-    s = make_system(args.config)
-    m = args.batch if args.batch > 0 else s["m"]
-    # every rank gets its own seeded batch of m trial vectors (weak scaling over trial vectors, no collective)
+    s = make_system(cfg)
+    m = args.batch if (args.batch > 0 and cfg == args.config) else s["m"]
+    if cfg == 5 and not (args.batch > 0 and cfg == args.config):
+        m = 15          # X and sigma of 30 vectors (2 x 32 GB) do not fit beside the K tensors on a 180 GB part
     big = s["nocc"] * s["nvir"] * m > 1e9
     if big:    # 3000-atom scale: one pinned copy of X on the host, filled in place
         Xp = torch.empty((m, s["nocc"], s["nvir"]), dtype=torch.float64, pin_memory=True)
@@ -142,7 +173,7 @@ def main():
         X_h = trial_vectors(s, m, base_seed=260329257 + 17 * rank)
         Xp = None
     t0 = time.time()
-    ctx = setup(s, device=local, max_batch=m)
+    ctx = setup(s, device=local, max_batch=m, host_budget_bytes=args.host_budget_gb << 30)
     t_setup = time.time() - t0
     X = torch.from_numpy(X_h).to(dev)
     sigma = torch.empty_like(X)
@@ -155,12 +186,12 @@ def main():
         torch.cuda.synchronize(dev)
 
     # ---- device-resident timing
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         ctx.matvec(X, sigma)
     barrier()
     sampler = ClockSampler(local) if rank == 0 else None
     tw0 = time.time()
-    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     phase = {}
     for a, b in evs:
         flush.zero_()
@@ -176,10 +207,11 @@ def main():
     t_dev = sum(a.elapsed_time(b) for a, b in evs) * 1e-3
     tim = ctx.timings()
     d = ctx.dims()
-    launches = tim["kernel_launches"] * args.steps
+    launches = tim["kernel_launches"] * steps
 
     # ---- end to end: pinned host buffers through risp_matvec_host
     fp = None
+    sig_h = None if big else sigma.cpu().numpy()
     if big:    # the library's own staging copies of X and sigma take the place of the caller's device tensors
         fp = sigma.view(m, -1)[:, ::997].cpu()
         del X, sigma
@@ -187,11 +219,11 @@ def main():
     if Xp is None:
         Xp = torch.from_numpy(X_h).pin_memory()
     Sp = torch.empty(Xp.shape, dtype=torch.float64, pin_memory=True)
-    for _ in range(2 if args.config <= 3 else 1):
+    for _ in range(2 if cfg <= 3 else 1):
         ctx.matvec_host_ptr(m, Xp.data_ptr(), Sp.data_ptr())
     barrier()
     t_e2e = 0.0
-    e2e_steps = args.steps if args.config <= 3 else 1
+    e2e_steps = steps if cfg <= 3 else 1
     for _ in range(e2e_steps):
         flush.zero_(); torch.cuda.synchronize(dev)
         t0 = time.perf_counter()
@@ -202,25 +234,61 @@ def main():
         tt = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=dev)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         t_dev, t_e2e = float(tt[0]), float(tt[1])
-    same = bool(torch.equal(Sp.view(m, -1)[:, ::997], fp)) if big else all(bool(torch.equal(Sp[k].to(dev), sigma[k])) for k in range(m))
+    same = bool(torch.equal(Sp.view(m, -1)[:, ::997], fp)) if big else bool(np.array_equal(Sp.numpy(), sig_h))
+    if not big:
+        del X, sigma
+    del flush
+    torch.cuda.empty_cache()
 
+    res = None
     if rank == 0:
         pk = _peaks()
         no, nv, nK = d["noccK"], d["nvirK"], d["nauxK"]
+        ms_step = 1e3 * t_dev / steps
+        # a launch inside a step of a second or more runs under the sustained power / clock state, a short step under the burst one
+        long_step = ms_step >= 1000.0
+        bf16 = pk["bf16_sustained"] if long_step else pk["bf16"]
+        peak = bf16 * FP64_PER_BF16
+        peak_src = f"{pk['src']} bf16 {'sustained' if long_step else 'burst'} {bf16} TFLOP/s x nominal FP64:bf16 ratio 45/2250 ({'step >= 1 s' if long_step else 'step < 1 s'})"
         # dominant kernel: the DMMA GEMM launch M^P = X' T_ab^P (Eq. 22) of the first aux chunk
         npf = tim["first_chunk_naux"]
         flops_launch = 2.0 * m * no * nv * nv * npf
-        t_launch = phase["k_gemm1"] / args.steps
+        t_launch = phase["k_gemm1"] / steps
         achieved = flops_launch / t_launch / 1e12 if t_launch > 0 else 0.0
-        peak = pk["bf16"] * FP64_PER_BF16
         traffic = None
-        tpath = os.path.join(ROOT, "profiles", f"traffic_cfg{args.config}.json")
+        tpath = os.path.join(ROOT, "profiles", f"traffic_cfg{cfg}.json")
         if os.path.exists(tpath):
             traffic = json.load(open(tpath)).get("dgemm_k_gemm1_dram_bytes_per_launch")
-        flops_step = dict(K=2.0 * m * nK * no * nv * (no + nv), transforms=4.0 * m * s["nocc"] * s["nvir"] * s["nao"] + 4.0 * m * s["nao"] ** 2 * s["nocc"])
+        # yardsticks measured now, on this GPU, by the library's own register-resident micro-kernels and by cuBLAS through torch
+        dfma = ctx.yardstick(0, reps=3) / 1e12
+        dmma = ctx.yardstick(1, reps=3) / 1e12
+        A = torch.randn((8192, 8192), dtype=torch.float64, device=dev)
+        for _ in range(2):
+            A @ A
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); C3 = [A @ A for _ in range(3)]; e1.record(); e1.synchronize()
+        cublas = 3 * 2.0 * 8192 ** 3 / (e0.elapsed_time(e1) * 1e-3) / 1e12
+        del A, C3
+        torch.cuda.empty_cache()
+        z_pairs = d["n_ao_pairs_kept"]
+        flops_step = dict(K=2.0 * m * nK * no * nv * (no + nv),
+                          transforms_dense=4.0 * m * s["nocc"] * s["nvir"] * s["nao"] + 4.0 * m * s["nao"] ** 2 * s["nocc"],
+                          transforms_pair_sparse=4.0 * m * s["nocc"] * s["nvir"] * s["nao"] + 8.0 * m * z_pairs * s["nocc"])
+        eri = _eri_flops_per_task()
+        eri_entry = dict(phase="ERI passes (Eq. 14, 16): FP64 instructions executed, both passes", bound="alu", unit="TFLOP/s", achieved=None, peak=dfma,
+                         peak_source="risp_debug_yardstick(0): register-resident DFMA chains on all SMs, measured in this run")
+        t_eri = (phase["j_pass1"] + phase["j_pass2"]) / steps
+        if eri is not None and t_eri > 0:
+            fl = 0.0
+            for c, npairs in enumerate(d["pairs_per_class"]):
+                for ps in ("pass1", "pass2"):
+                    fl += eri[ps][c] * npairs * d["n_aux_centres"]
+            eri_entry.update(achieved=fl / t_eri / 1e12, frac=fl / t_eri / 1e12 / dfma, flops_per_step=fl,
+                             note=eri.get("note", ""))
+        t_tr = (phase["j_transform_in"] + phase["j_transform_out"]) / steps
         line = dict(
-            metric=METRIC, value=world * m * args.steps / t_dev, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
-            ms_per_step=1e3 * t_dev / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+            metric=METRIC, value=world * m * steps / t_dev, unit=UNIT, n_gpus=world, steps=steps, warmup=warmup,
+            ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
             config=dict(workload=s["name"], m=m, atoms=int(s["natm"]), nao=s["nao"], nocc=s["nocc"], nvir=s["nvir"], nauxJ=d["nauxJ"], nauxK=nK,
                         noccK=no, nvirK=nv, shell_pairs_kept=d["n_shell_pairs_kept"], shell_pairs=d["n_shell_pairs"],
                         ao_pair_survival=round(2.0 * d["n_ao_pairs_kept"] / (s["nao"] * (s["nao"] + 1)), 4),
@@ -233,49 +301,126 @@ def main():
                      bitwise_equal_to_device_path=same),
             gpu_launches=launches,
             roofline=dict(bound="tensor", kernel="dgemm_tma_kernel<KC,KC,MI> (K contraction M^P = X' T_ab^P, Eq. 22)", achieved=achieved, peak=peak,
-                          unit="TFLOP/s", frac=achieved / peak, traffic=traffic,
-                          peak_source=f"{pk['src']} bf16 burst {pk['bf16']} TFLOP/s x nominal FP64:bf16 ratio 45/2250",
-                          context=dict(dmma_issue_ceiling_tflops=37.2, cublas_dgemm_measured_tflops=36.2,
-                                       note="FP64 tensor op of sm_100a is the warp-level DMMA.8x8x4 (one per 16 clk per sub-partition); the peak "
-                                            "above is the tier rule (other dtype's measured peak x nominal ratio), so frac can slightly exceed 1"),
+                          unit="TFLOP/s", frac=achieved / peak, traffic=traffic, peak_source=peak_src,
+                          context=dict(dmma_issue_ceiling_tflops_measured=dmma, cublas_dgemm_8192_tflops_measured=cublas, dfma_tflops_measured=dfma,
+                                       frac_of_dmma_ceiling=achieved / dmma, frac_of_cublas_dgemm=achieved / cublas,
+                                       note="FP64 tensor op of sm_100a is the warp-level DMMA.8x8x4; `peak` follows the tier rule (another dtype's "
+                                            "measured peak x nominal ratio), the three yardsticks beside it were measured in this run"),
                           flops_per_launch=flops_launch, launch_ms=1e3 * t_launch),
-            phases_ms={k: round(1e3 * v / args.steps, 4) for k, v in phase.items() if k not in ("kernel_launches", "first_chunk_naux")},
+            phases_ms={k: round(1e3 * v / steps, 4) for k, v in phase.items() if k not in ("kernel_launches", "first_chunk_naux")},
             rooflines_other=[
                 dict(phase="K contraction, all chunks (Eq. 22-23, packed-slice expansion included)", bound="tensor", unit="TFLOP/s",
-                     achieved=flops_step["K"] / (phase["k_total"] / args.steps) / 1e12 if phase.get("k_total") else None, peak=peak),
-                dict(phase="J AO<->MO transforms (Eq. 12, 17; e0 gather/scatter and the diagonal term included)", bound="tensor", unit="TFLOP/s",
-                     achieved=flops_step["transforms"] / ((phase["j_transform_in"] + phase["j_transform_out"]) / args.steps) / 1e12, peak=peak),
+                     achieved=flops_step["K"] / (phase["k_total"] / steps) / 1e12 if phase.get("k_total") else None, peak=peak,
+                     frac=flops_step["K"] / (phase["k_total"] / steps) / 1e12 / peak if phase.get("k_total") else None),
+                dict(phase="J AO<->MO transforms (Eq. 12, 17; e0 gather/scatter and the diagonal term included), against the PAIR-SPARSE flop count "
+                           "4 m nocc nvir nao + 8 m z nocc the method needs", bound="tensor", unit="TFLOP/s",
+                     achieved=flops_step["transforms_pair_sparse"] / t_tr / 1e12, peak=peak, frac=flops_step["transforms_pair_sparse"] / t_tr / 1e12 / peak,
+                     executed_tflops=flops_step["transforms_dense"] / t_tr / 1e12),
                 dict(phase="sigma[window] -= K' (Eq. 10)", bound="hbm", unit="GB/s",
-                     achieved=24.0 * m * no * nv / (phase["assemble"] / args.steps) / 1e9 if phase.get("assemble") else None, peak=pk["hbm"]),
-                dict(phase="ERI passes (Eq. 14, 16): (pair, aux centre) tasks per second, both passes", bound="alu", unit="Gtask/s",
-                     achieved=2.0 * d["n_shell_pairs_kept"] * (d["nauxJ"] / 4) / ((phase["j_pass1"] + phase["j_pass2"]) / args.steps) / 1e9, peak=None),
+                     achieved=24.0 * m * no * nv / (phase["assemble"] / steps) / 1e9 if phase.get("assemble") else None, peak=pk["hbm"],
+                     frac=24.0 * m * no * nv / (phase["assemble"] / steps) / 1e9 / pk["hbm"] if phase.get("assemble") else None),
+                eri_entry,
             ],
             flops_per_step=flops_step,
         )
-        if not args.no_cpu_baseline and world == 1 and not big:
-            from oracle.risp_oracle import Oracle
-            o = Oracle(s)
-            t0 = time.time(); o.build(); tb = time.time() - t0
+        smp = None
+        if want_cpu and world == 1 and cfg <= 4:
             ms_ = min(m, 30)
-            t0 = time.time(); ref = o.sigma(X_h[:ms_]); dt = time.time() - t0
-            err = float(np.linalg.norm(sigma.cpu().numpy()[:ms_] - ref) / np.linalg.norm(ref))
-            line["cpu_baseline"] = dict(value=ms_ / dt, unit=UNIT, cores=os.cpu_count(), kind="oracle",
-                                        sample=f"one oracle.sigma call on {ms_} of the {m} trial vectors ({dt:.1f} s); tensor build ({tb:.1f} s) excluded like risp_setup",
-                                        gpu_vs_oracle_rel_err=err)
-        oracle_for_solve = o if (not args.no_cpu_baseline and world == 1 and not big and args.config <= 2) else None
-        if args.solve:
-            omega, _, info = ctx.tda_solve(s["nroots"], tol=1e-5, max_iter=args.solve_max_iter, allow_unconverged=True)
-            line["solve"] = dict(nroots=s["nroots"], tol=1e-5, wall_s=info["sec_total"], matvec_s=info["sec_matvec"], alloc_s=info["sec_alloc"], subspace_s=info["sec_subspace"], cached_vectors=info["cached_vectors"], iterations=info["iterations"],
-                                 n_sigma=info["n_sigma"], restarts=info["restarts"], converged=info["converged"], omega_ev=[float(x) * 27.211386245988 for x in omega],
-                                 h2d_gb=info["bytes_h2d"] / 1e9, d2h_gb=info["bytes_d2h"] / 1e9)
-            if oracle_for_solve is not None:      # the CPU oracle's own Davidson on the same problem (reported baseline; same tolerance)
+            smp = OracleSample(s, ms_)
+            t_est, t_cpu = smp.step(X_h[:ms_])
+            cb = dict(value=ms_ / t_est, unit=UNIT, cores=smp.cores, kind="oracle", sample=smp.describe(t_cpu))
+            if smp.full:
+                ref = smp.last[0] + 2.0 * smp.last[1] - smp.last[2]
+                cb["gpu_vs_oracle_rel_err"] = float(np.linalg.norm(sig_h[:ms_] - ref) / np.linalg.norm(ref))
+            line["cpu_baseline"] = cb
+        if want_solve:
+            big_dim = s["nocc"] * s["nvir"] >= 5e7
+            kw = dict(tol=args.solve_tol, max_iter=args.solve_max_iter, allow_unconverged=True)
+            if big_dim:
+                kw.update(flags=8 if args.solve_fp32_host else 0)
+            t0 = time.time()
+            omega, Xs, info = ctx.tda_solve(s["nroots"], want_vectors=not big_dim, **kw)
+            sv = dict(nroots=s["nroots"], tol=args.solve_tol, wall_s=info["sec_total"], matvec_s=info["sec_matvec"], alloc_s=info["sec_alloc"],
+                      subspace_s=info["sec_subspace"], block=info["block"], capacity=info["capacity"], cached_vectors=info["cached_vectors"],
+                      host_subspace_gb=info["bytes_host_subspace"] / 1e9, iterations=info["iterations"], n_sigma=info["n_sigma"], restarts=info["restarts"],
+                      converged=info["converged"], subspace_max=info["subspace_max"], resid_max=float(max(info["resid"])),
+                      omega_ev=[float(x) * HARTREE_EV for x in omega], h2d_gb=info["bytes_h2d"] / 1e9, d2h_gb=info["bytes_d2h"] / 1e9,
+                      setup_s=round(t_setup, 3), setup_plus_solve_s=round(t_setup + info["sec_total"], 3))
+            if Xs is not None:      # compositional check (v) of SURVEY 8(c).6: residuals recomputed by a fresh risp_matvec
+                AX = ctx.matvec(Xs)
+                r = (AX - torch.from_numpy(omega).to(dev)[:, None, None] * Xs).reshape(s["nroots"], -1).norm(dim=1)
+                sv["resid_recomputed_max"] = float(r.max())
+                del AX, Xs
+            if smp is not None and smp.full and cfg <= 2:      # the CPU oracle's own Davidson on the same problem (same tolerance)
                 t0 = time.time()
-                th_ref, _, iref = oracle_for_solve.davidson(s["nroots"], tol=1e-5)
-                line["solve"]["cpu_oracle"] = dict(wall_s=time.time() - t0, iterations=int(iref["iterations"]), n_sigma=int(iref["n_sigma"]),
-                                                   converged=bool(iref["converged"]), cores=os.cpu_count(),
-                                                   max_abs_diff_ev=float(np.abs(np.asarray(omega) - th_ref).max() * 27.211386245988))
-        print(json.dumps(line))
+                th_ref, _, iref = smp.o.davidson(s["nroots"], tol=args.solve_tol)
+                sv["cpu_oracle"] = dict(wall_s=time.time() - t0, iterations=int(iref["iterations"]), n_sigma=int(iref["n_sigma"]),
+                                        converged=bool(iref["converged"]), cores=os.cpu_count(),
+                                        max_abs_diff_ev=float(np.abs(np.asarray(omega) - th_ref).max() * HARTREE_EV))
+            elif "cpu_baseline" in line:
+                sv["cpu_oracle_estimate"] = dict(wall_s=info["n_sigma"] / line["cpu_baseline"]["value"], cores=os.cpu_count(),
+                                                 note="n_sigma of the GPU solve / sampled oracle sigma-builds/s; the oracle's own Davidson is not run at this size")
+            line["solve"] = sv
+        res = line
     ctx.close()
+    del ctx
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
+    return res
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="risp", choices=["risp", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index + 1 (default 3: the 300-atom system)")
+    ap.add_argument("--ref-vectors", type=int, default=30, help="trial vectors per step of the CPU oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--batch", type=int, default=0, help="trial vectors per step (0: the config's m)")
+    ap.add_argument("--solve-max-iter", type=int, default=150)
+    ap.add_argument("--solve-tol", type=float, default=1e-5)
+    ap.add_argument("--solve-fp32-host", action="store_true", help="RISP_SOLVE_HOST_FP32 for the solve of the 1000/3000-atom systems")
+    ap.add_argument("--no-solve", action="store_true", help="skip the 15-root risp_tda_solve")
+    ap.add_argument("--solve", action="store_true", help="(default) kept for compatibility")
+    ap.add_argument("--also", default="4", help="comma separated further configs run briefly after the main one (1 GPU only); '' for none")
+    ap.add_argument("--also-budget-s", type=float, default=420.0, help="an `also` config starts only if the run is younger than this")
+    ap.add_argument("--host-budget-gb", type=int, default=0, help="pinned-host budget of the Davidson subspace (0: half of the host memory)")
+    args = ap.parse_args()
+    # contract: >= 3 warm-up steps; the 1000/3000-atom configs (tens of seconds to minutes per step) are allowed 1 and say so
+    args.warmup = (max(args.warmup, 3) if args.config <= 3 else max(args.warmup, 1)) if args.impl == "risp" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+
+    solve_main = not args.no_solve and world == 1 and args.config <= 4
+    solve_main = solve_main or (not args.no_solve and world == 1 and args.solve)
+    line = run_config(args.config, args, world, rank, local, dist, want_solve=solve_main, want_cpu=not args.no_cpu_baseline,
+                      steps=args.steps, warmup=args.warmup)
+    if rank == 0 and world == 1 and args.also:
+        line["also"] = []
+        for c in [int(x) for x in args.also.split(",") if x.strip()]:
+            if c == args.config:
+                continue
+            if time.time() - T_START > args.also_budget_s:
+                line["also"].append(dict(workload=f"cfg{c}", skipped=f"run already {time.time() - T_START:.0f} s old (budget {args.also_budget_s:.0f} s)"))
+                continue
+            sub = run_config(c, args, 1, 0, local, dist, want_solve=False, want_cpu=False, steps=2 if c == 4 else 1, warmup=1)
+            keep = {k: sub[k] for k in ("value", "unit", "steps", "warmup", "ms_per_step", "config", "e2e", "roofline", "phases_ms", "rooflines_other", "clocks")}
+            line["also"].append(keep)
+    if rank == 0:
+        print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 

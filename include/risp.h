@@ -136,6 +136,8 @@ typedef struct {
     int32_t nauxK_device;                /* K-tensor slices resident in HBM; the other nauxK - nauxK_device live in pinned host memory */
     int64_t bytes_T_host;                /* pinned host bytes of the spilled slices */
     int32_t j_sub_batch, j_panels;       /* J transforms: trial vectors per sub-batch, AO row panels per sub-batch (1 = dense) */
+    int64_t pairs_per_class[6];          /* kept shell pairs by angular-momentum class (l_a >= l_b): ss, ps, pp, ds, dp, dd */
+    int64_t n_aux_centres;               /* auxiliary centres of the J set (an s and a p shell of one atom share a centre, Eq. 4) */
 } risp_dims;
 
 /* per-phase device seconds of the last risp_matvec (CUDA events; valid after the stream was synchronised) */

@@ -59,7 +59,8 @@ class _Dims(C.Structure):
                 ("noccK", C.c_int32), ("nvirK", C.c_int32), ("occK_first", C.c_int32), ("virK_first", C.c_int32),
                 ("n_shell_pairs", C.c_int64), ("n_shell_pairs_kept", C.c_int64), ("n_ao_pairs_kept", C.c_int64),
                 ("bytes_Tij", C.c_int64), ("bytes_Tab", C.c_int64), ("bytes_device_total", C.c_int64), ("aux_chunk", C.c_int32),
-                ("nauxK_device", C.c_int32), ("bytes_T_host", C.c_int64), ("j_sub_batch", C.c_int32), ("j_panels", C.c_int32)]
+                ("nauxK_device", C.c_int32), ("bytes_T_host", C.c_int64), ("j_sub_batch", C.c_int32), ("j_panels", C.c_int32),
+                ("pairs_per_class", C.c_int64 * 6), ("n_aux_centres", C.c_int64)]
 
 
 class _Timings(C.Structure):

@@ -51,6 +51,8 @@ extern "C" int risp_get_dims(const risp_ctx *ctx, risp_dims *out)
     out->bytes_T_host = ctx->has_K ? (int64_t)(ctx->nauxK - ctx->nK_dev) * (ctx->tri_o + ctx->tri_v) * 8 : 0;
     out->j_sub_batch = ctx->plan.mj;
     out->j_panels = ctx->plan.panel_r0.empty() ? 0 : (int)ctx->plan.panel_r0.size() - 1;
+    for (int c = 0; c < 6; ++c) out->pairs_per_class[c] = ctx->cls[c].npairs;
+    out->n_aux_centres = ctx->ncenJ;
     return RISP_OK;
 }
 
