@@ -325,7 +325,7 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
         )
         smp = None
         if want_cpu and world == 1 and cfg <= 4:
-            ms_ = min(m, 30)
+            ms_ = min(m, 30 if cfg <= 2 else args.ref_vectors)
             smp = OracleSample(s, ms_)
             t_est, t_cpu = smp.step(X_h[:ms_])
             cb = dict(value=ms_ / t_est, unit=UNIT, cores=smp.cores, kind="oracle", sample=smp.describe(t_cpu))
@@ -377,7 +377,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="risp", choices=["risp", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index + 1 (default 3: the 300-atom system)")
-    ap.add_argument("--ref-vectors", type=int, default=30, help="trial vectors per step of the CPU oracle sample")
+    ap.add_argument("--ref-vectors", type=int, default=10, help="trial vectors per step of the CPU oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--batch", type=int, default=0, help="trial vectors per step (0: the config's m)")
     ap.add_argument("--solve-max-iter", type=int, default=150)
