@@ -335,22 +335,26 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
             line["cpu_baseline"] = cb
         if want_solve:
             big_dim = s["nocc"] * s["nvir"] >= 5e7
-            kw = dict(tol=args.solve_tol, max_iter=args.solve_max_iter, allow_unconverged=True)
-            if big_dim:
-                kw.update(flags=8 if args.solve_fp32_host else 0)
-            t0 = time.time()
-            omega, Xs, info = ctx.tda_solve(s["nroots"], want_vectors=not big_dim, **kw)
-            sv = dict(nroots=s["nroots"], tol=args.solve_tol, wall_s=info["sec_total"], matvec_s=info["sec_matvec"], alloc_s=info["sec_alloc"],
-                      subspace_s=info["sec_subspace"], block=info["block"], capacity=info["capacity"], cached_vectors=info["cached_vectors"],
-                      host_subspace_gb=info["bytes_host_subspace"] / 1e9, iterations=info["iterations"], n_sigma=info["n_sigma"], restarts=info["restarts"],
-                      converged=info["converged"], subspace_max=info["subspace_max"], resid_max=float(max(info["resid"])),
+            kw = dict(tol=args.solve_tol, max_iter=args.solve_max_iter, allow_unconverged=True, n_guess=args.solve_n_guess)
+            flags = (8 if args.solve_fp32_host else 0) | (16 if big_dim else 0)
+            omega, Xs, info = ctx.tda_solve(s["nroots"], want_vectors=True, flags=flags, **kw)
+            sv = dict(nroots=s["nroots"], tol=args.solve_tol, n_guess=args.solve_n_guess or 2 * s["nroots"], wall_s=info["sec_total"], matvec_s=info["sec_matvec"],
+                      alloc_s=info["sec_alloc"], subspace_s=info["sec_subspace"], block=info["block"], capacity=info["capacity"],
+                      cached_vectors=info["cached_vectors"], host_subspace_gb=info["bytes_host_subspace"] / 1e9,
+                      host_store="fp32" if args.solve_fp32_host else "fp64", iterations=info["iterations"], n_sigma=info["n_sigma"],
+                      restarts=info["restarts"], converged=info["converged"], subspace_max=info["subspace_max"], resid_max=float(max(info["resid"])),
                       omega_ev=[float(x) * HARTREE_EV for x in omega], h2d_gb=info["bytes_h2d"] / 1e9, d2h_gb=info["bytes_d2h"] / 1e9,
                       setup_s=round(t_setup, 3), setup_plus_solve_s=round(t_setup + info["sec_total"], 3))
-            if Xs is not None:      # compositional check (v) of SURVEY 8(c).6: residuals recomputed by a fresh risp_matvec
-                AX = ctx.matvec(Xs)
-                r = (AX - torch.from_numpy(omega).to(dev)[:, None, None] * Xs).reshape(s["nroots"], -1).norm(dim=1)
-                sv["resid_recomputed_max"] = float(r.max())
-                del AX, Xs
+            # compositional check (v) of SURVEY 8(c).6: residuals ||A x_k - omega_k x_k|| recomputed by fresh risp_matvec calls
+            rmax, blk = 0.0, info["block"]
+            for c0 in range(0, s["nroots"], blk):
+                Xc = (torch.from_numpy(Xs[c0:c0 + blk]).to(dev) if big_dim else Xs[c0:c0 + blk].contiguous())
+                AX = ctx.matvec(Xc)
+                r = (AX - torch.from_numpy(omega[c0:c0 + blk]).to(dev)[:, None, None] * Xc).reshape(Xc.shape[0], -1).norm(dim=1)
+                rmax = max(rmax, float(r.max()))
+                del AX, Xc
+            sv["resid_recomputed_max"] = rmax
+            del Xs
             if smp is not None and smp.full and cfg <= 2:      # the CPU oracle's own Davidson on the same problem (same tolerance)
                 t0 = time.time()
                 th_ref, _, iref = smp.o.davidson(s["nroots"], tol=args.solve_tol)
@@ -382,6 +386,7 @@ def main():
     ap.add_argument("--batch", type=int, default=0, help="trial vectors per step (0: the config's m)")
     ap.add_argument("--solve-max-iter", type=int, default=150)
     ap.add_argument("--solve-tol", type=float, default=1e-5)
+    ap.add_argument("--solve-n-guess", type=int, default=0, help="initial unit vectors of the solve (0: 2 * nroots, the config's batch of 30)")
     ap.add_argument("--solve-fp32-host", action="store_true", help="RISP_SOLVE_HOST_FP32 for the solve of the 1000/3000-atom systems")
     ap.add_argument("--no-solve", action="store_true", help="skip the 15-root risp_tda_solve")
     ap.add_argument("--solve", action="store_true", help="(default) kept for compatibility")

@@ -112,6 +112,9 @@ typedef struct {
                                         PAPER.md:201); every product still accumulates in FP64.  Trial vectors are rounded to
                                         FP32-representable values before their sigma-build, so V is stored exactly */
 
+#define RISP_SOLVE_X_OUT_HOST 16      /* X_out is a HOST pointer: the Ritz vectors are written there chunk by chunk (3000 atoms: 15 vectors
+                                        are 16 GB, more than is left on the device beside the K tensors) */
+
 #define RISP_MAX_ROOTS 64
 typedef struct {
     int32_t iterations, restarts, n_sigma, converged;
@@ -165,9 +168,20 @@ int risp_matvec_host(risp_ctx *ctx, int32_t m, const double *X_host, double *sig
 
 /* Lowest `nroots` eigenpairs of A by a Davidson iteration whose subspace (V, W = A V) lives in pinned host
  * memory and is streamed through the device on a side stream.  omega_hartree: HOST [nroots]
- * ascending.  X_out: DEVICE [nroots][nocc][nvir] or NULL.  info may be NULL. */
+ * ascending.  X_out: DEVICE [nroots][nocc][nvir] (HOST with RISP_SOLVE_X_OUT_HOST) or NULL.  info may be NULL. */
 int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_options *opt, double *omega_hartree, double *X_out,
                    risp_solve_info *info);
+
+/* Transition properties of n TDA states (Eq. 5-8; TDA: Y = 0):
+ *     mu_0n = scale sum_ia r_ia X_nia (Eq. 7),   m_0n = scale sum_ia (r x nabla)_ia X_nia (Eq. 8),
+ *     f_0n = 2/3 Omega_n mu_0n . mu_0n (Eq. 5),  R_0n = 1/2 mu_0n . m_0n (Eq. 6),    atomic units, dipole-length form.
+ * X_dev: DEVICE [n][nocc][nvir] (e.g. X_out of risp_tda_solve, <X|X> = 1); omega_hartree: HOST [n] (needed for f_out only);
+ * origin_bohr: HOST [3] gauge origin of r and r x nabla, NULL = (0,0,0); scale: factor on both moments, <= 0 selects sqrt(2), the
+ * closed-shell singlet factor for unit-normalised X (the paper prints none: DESIGN.md reading G24).  Outputs are HOST arrays,
+ * mu_out[n][3], m_out[n][3], f_out[n], R_out[n]; any of them may be NULL.  Synchronous; allocates and frees its own scratch
+ * (one AO matrix, one half-transformed matrix, six [nocc][nvir] blocks). */
+int risp_transition_properties(risp_ctx *ctx, int32_t n, const double *X_dev, const double *omega_hartree, const double *origin_bohr,
+                               double scale, double *mu_out, double *m_out, double *f_out, double *R_out);
 
 void risp_destroy(risp_ctx *ctx);
 const char *risp_last_error(const risp_ctx *ctx); /* static text if ctx == NULL */

@@ -40,6 +40,10 @@ int risp_debug_force_plan(risp_ctx *ctx, int mj, int prow, int pc);
  * Returns the rate through *out. */
 int risp_debug_yardstick(risp_ctx *ctx, int which, size_t bytes, int reps, double *out);
 
+/* The six one-electron AO matrices behind risp_transition_properties (Eq. 7-8), on the kept shell pairs:
+ * out_host[6][nao][nao] = <mu|(r-O)_k|nu> for k = x, y, z, then <mu|((r-O) x nabla)_k|nu>.  origin_bohr: HOST [3] or NULL. */
+int risp_debug_oneel_ao(risp_ctx *ctx, const double *origin_bohr, double *out_host);
+
 #ifdef __cplusplus
 }
 #endif

@@ -10,7 +10,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
 EXPORTED_SYMBOLS = ["risp_setup", "risp_matvec", "risp_matvec_host", "risp_tda_solve", "risp_destroy", "risp_last_error",
-                    "risp_get_dims", "risp_get_timings", "risp_eri3c_shell", "risp_get_stage"]
+                    "risp_get_dims", "risp_get_timings", "risp_eri3c_shell", "risp_get_stage", "risp_transition_properties"]
 
 RISP_MAX_ROOTS = 64
 FLAG_KEEP_STAGES, FLAG_SPILL_HALF = 1, 2
@@ -93,7 +93,9 @@ def load_library():
     lib.risp_get_timings.argtypes = [vp, C.POINTER(_Timings)]
     lib.risp_eri3c_shell.argtypes = [vp, i32, i32, i32, i32, vp]
     lib.risp_get_stage.argtypes = [vp, i32, vp, i64, vp]
+    lib.risp_transition_properties.argtypes = [vp, i32, vp, vp, vp, dbl, vp, vp, vp, vp]
     # include/risp_debug.h
+    lib.risp_debug_oneel_ao.argtypes = [vp, vp, vp]
     lib.risp_debug_dgemm.argtypes = [C.c_int, C.c_int, C.c_int, vp, C.c_longlong, C.c_int, vp, C.c_longlong, C.c_int, vp, C.c_longlong,
                                      dbl, dbl, C.c_int, C.c_longlong, C.c_longlong, C.c_longlong, C.c_int, C.c_int, C.c_longlong, vp]
     lib.risp_debug_sym_eig_lowest.argtypes = [C.c_int, C.c_int, vp, vp, vp]
@@ -189,14 +191,34 @@ class RispContext:
         omega = np.zeros(nroots)
         info = _SolveInfo()
         opt = _SolveOptions(float(tol), int(max_iter), int(n_guess), int(max_sub), int(flags), int(max_block), 0, int(device_budget_bytes))
-        X = torch.empty((nroots, self.nocc, self.nvir), dtype=torch.float64, device=f"cuda:{self.device}") if want_vectors else None
-        rc = self.lib.risp_tda_solve(self.handle, nroots, C.byref(opt), omega.ctypes.data_as(C.POINTER(C.c_double)),
-                                     X.data_ptr() if X is not None else None, C.byref(info))
+        if want_vectors and (flags & 16):      # RISP_SOLVE_X_OUT_HOST: a host array takes the vectors
+            X = np.empty((nroots, self.nocc, self.nvir))
+            xptr = X.ctypes.data
+        else:
+            X = torch.empty((nroots, self.nocc, self.nvir), dtype=torch.float64, device=f"cuda:{self.device}") if want_vectors else None
+            xptr = X.data_ptr() if X is not None else None
+        rc = self.lib.risp_tda_solve(self.handle, nroots, C.byref(opt), omega.ctypes.data_as(C.POINTER(C.c_double)), xptr, C.byref(info))
         if rc != 0 and not (rc == -5 and allow_unconverged):
             self._check(rc)
         d = _struct_dict(info)
         d["resid"] = d["resid"][:nroots]
         return omega, X, d
+
+    def transition_properties(self, X, omega, origin=None, scale=0.0):
+        """risp_transition_properties: (mu[n][3], m[n][3], f[n], R[n]) for the device vectors X[n][nocc][nvir]."""
+        n = X.shape[0]
+        om = np.ascontiguousarray(omega, dtype=np.float64)
+        org = None if origin is None else np.ascontiguousarray(origin, dtype=np.float64)
+        mu, m, f, R = np.zeros((n, 3)), np.zeros((n, 3)), np.zeros(n), np.zeros(n)
+        self._check(self.lib.risp_transition_properties(self.handle, n, X.data_ptr(), om.ctypes.data, org.ctypes.data if org is not None else None,
+                                                        float(scale), mu.ctypes.data, m.ctypes.data, f.ctypes.data, R.ctypes.data))
+        return mu, m, f, R
+
+    def oneel_ao(self, origin=None) -> np.ndarray:
+        org = None if origin is None else np.ascontiguousarray(origin, dtype=np.float64)
+        out = np.zeros((6, self.nao, self.nao))
+        self._check(self.lib.risp_debug_oneel_ao(self.handle, org.ctypes.data if org is not None else None, out.ctypes.data))
+        return out
 
     def force_plan(self, mj: int = 0, prow: int = 0, pc: int = 0):
         """Testing: override the work-space plan (J sub-batch, AO rows per panel, K aux chunk); 0 keeps the automatic choice."""

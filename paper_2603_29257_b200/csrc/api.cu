@@ -18,6 +18,9 @@ extern "C" void risp_destroy(risp_ctx *ctx)
     if (ctx->h_TabP) cudaFreeHost(ctx->h_TabP);
     for (int c = 0; c < 6; ++c) { if (ctx->cls[c].d_pairs) cudaFree(ctx->cls[c].d_pairs); if (ctx->cls[c].d_permB) cudaFree(ctx->cls[c].d_permB); }
     if (ctx->d_prims) cudaFree(ctx->d_prims);
+    if (ctx->d_oneel_shl) cudaFree(ctx->d_oneel_shl);
+    if (ctx->d_prim_exp) cudaFree(ctx->d_prim_exp);
+    if (ctx->d_prim_d) cudaFree(ctx->d_prim_d);
     if (ctx->d_cenJ) cudaFree(ctx->d_cenJ);
     if (ctx->d_cenK) cudaFree(ctx->d_cenK);
     if (ctx->ev_ok) {

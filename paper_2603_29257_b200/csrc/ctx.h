@@ -73,6 +73,8 @@ struct risp_ctx {
     double *d_Cvir = nullptr;     // [nao][ldvir]
     double *d_eps = nullptr;      // [nmo]
     double *d_boys = nullptr;     // Boys table
+    void *d_oneel_shl = nullptr;  // shell table of the one-electron kernel (properties.cu), uploaded on first use
+    double *d_prim_exp = nullptr, *d_prim_d = nullptr;
     PairClass cls[6];
     risp_eri::PrimPair *d_prims = nullptr;
     risp_eri::AuxCentre *d_cenJ = nullptr, *d_cenK = nullptr;

@@ -690,7 +690,9 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
         for (int c0 = 0; c0 < nroots; c0 += block) {
             const int nc = std::min(block, nroots - c0);
             if ((rc = ritz_vectors(S, false, yv, ky, ky, c0, nc, S.bufA))) return rc;
-            RISP_CUDA_TRY(cudaMemcpyAsync(X_out + (long long)c0 * dim, S.bufA, (size_t)nc * dim * 8, cudaMemcpyDeviceToDevice, S.st));
+            RISP_CUDA_TRY(cudaMemcpyAsync(X_out + (long long)c0 * dim, S.bufA, (size_t)nc * dim * 8,
+                                          (opt.flags & RISP_SOLVE_X_OUT_HOST) ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, S.st));
+            RISP_CUDA_TRY(cudaStreamSynchronize(S.st));
         }
         RISP_CUDA_TRY(cudaStreamSynchronize(S.st));
     }
