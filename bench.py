@@ -237,7 +237,7 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
     same = bool(torch.equal(Sp.view(m, -1)[:, ::997], fp)) if big else bool(np.array_equal(Sp.numpy(), sig_h))
     if not big:
         del X, sigma
-    del flush
+    del flush, Xp, Sp, fp
     torch.cuda.empty_cache()
 
     res = None
@@ -345,15 +345,20 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
                       restarts=info["restarts"], converged=info["converged"], subspace_max=info["subspace_max"], resid_max=float(max(info["resid"])),
                       omega_ev=[float(x) * HARTREE_EV for x in omega], h2d_gb=info["bytes_h2d"] / 1e9, d2h_gb=info["bytes_d2h"] / 1e9,
                       setup_s=round(t_setup, 3), setup_plus_solve_s=round(t_setup + info["sec_total"], 3))
+            if args.progress_file:      # a long solve leaves its record behind even if something after it fails
+                json.dump(sv, open(args.progress_file, "w"))
             # compositional check (v) of SURVEY 8(c).6: residuals ||A x_k - omega_k x_k|| recomputed by fresh risp_matvec calls
-            rmax, blk = 0.0, info["block"]
-            for c0 in range(0, s["nroots"], blk):
-                Xc = (torch.from_numpy(Xs[c0:c0 + blk]).to(dev) if big_dim else Xs[c0:c0 + blk].contiguous())
-                AX = ctx.matvec(Xc)
-                r = (AX - torch.from_numpy(omega[c0:c0 + blk]).to(dev)[:, None, None] * Xc).reshape(Xc.shape[0], -1).norm(dim=1)
-                rmax = max(rmax, float(r.max()))
-                del AX, Xc
-            sv["resid_recomputed_max"] = rmax
+            try:
+                rmax, blk = 0.0, info["block"]
+                for c0 in range(0, s["nroots"], blk):
+                    Xc = (torch.from_numpy(Xs[c0:c0 + blk]).to(dev) if big_dim else Xs[c0:c0 + blk].contiguous())
+                    AX = ctx.matvec(Xc)
+                    r = (AX - torch.from_numpy(omega[c0:c0 + blk]).to(dev)[:, None, None] * Xc).reshape(Xc.shape[0], -1).norm(dim=1)
+                    rmax = max(rmax, float(r.max()))
+                    del AX, Xc
+                sv["resid_recomputed_max"] = rmax
+            except Exception as e:      # reported, not hidden
+                sv["resid_recomputed_error"] = repr(e)
             del Xs
             if smp is not None and smp.full and cfg <= 2:      # the CPU oracle's own Davidson on the same problem (same tolerance)
                 t0 = time.time()
@@ -388,6 +393,7 @@ def main():
     ap.add_argument("--solve-tol", type=float, default=1e-5)
     ap.add_argument("--solve-n-guess", type=int, default=0, help="initial unit vectors of the solve (0: 2 * nroots, the config's batch of 30)")
     ap.add_argument("--solve-fp32-host", action="store_true", help="RISP_SOLVE_HOST_FP32 for the solve of the 1000/3000-atom systems")
+    ap.add_argument("--progress-file", default="", help="write the solve record to this file as soon as risp_tda_solve returns")
     ap.add_argument("--no-solve", action="store_true", help="skip the 15-root risp_tda_solve")
     ap.add_argument("--solve", action="store_true", help="(default) kept for compatibility")
     ap.add_argument("--also", default="4", help="comma separated further configs run briefly after the main one (1 GPU only); '' for none")

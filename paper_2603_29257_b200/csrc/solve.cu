@@ -486,6 +486,10 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
     const size_t vec = (size_t)dim * 8;
 
     // ---------------- block size and memory plan
+    // the staging copies of risp_matvec_host are not needed here and are re-created on demand
+    if (ctx->w_Xin) { cudaFree(ctx->w_Xin); ctx->w_Xin = nullptr; }
+    if (ctx->w_Sout) { cudaFree(ctx->w_Sout); ctx->w_Sout = nullptr; }
+    ctx->xin_cap = 0;
     int block = std::min(std::min(std::max(n_guess, nroots), RISP_MS), ctx->max_batch);
     if (opt.max_block > 0) block = std::min(block, opt.max_block);
     block = std::max(block, 1);
@@ -508,7 +512,7 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
             if (fixed <= room) {
                 const size_t left = room - fixed;
                 if (dev_limit >= want && (size_t)want * 2 * vec <= left) { S.slots = (int)want; S.ncache = (int)want; S.CH = 0; break; }      // all of V, W in HBM
-                S.CH = vec >= ((size_t)256 << 20) ? 4 : 16;
+                S.CH = vec >= ((size_t)1 << 30) ? 2 : (vec >= ((size_t)256 << 20) ? 4 : 16);      // >= 1 GiB per H2D copy either way
                 const size_t stream_bytes = 2 * (size_t)S.CH * vec + (S.fp32_host ? (size_t)block * dim * 4 : 0);
                 if (stream_bytes <= left) {
                     const long long dev_vecs = std::min<long long>(dev_limit, (long long)((left - stream_bytes) / (2 * vec)));

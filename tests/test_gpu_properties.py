@@ -30,7 +30,7 @@ def test_oneel_ao_matrices(which, torch_cuda, sys1, sys_small_rsh):
         kept[pr[:, 0], pr[:, 1]] = True; kept[pr[:, 1], pr[:, 0]] = True
         nf = 2 * np.asarray(s["shl_l"]) + 1
         mask = np.repeat(np.repeat(kept, nf, axis=0), nf, axis=1)
-        assert np.abs(got - ref)[:, mask].max() <= 1e-12
+        assert np.abs(got - ref)[:, mask].max() <= 1e-12 * max(1.0, np.abs(ref).max())      # values reach |r - O| ~ 20 bohr
         assert np.abs(ref[:, ~mask]).max() < 1e-10 if (~mask).any() else True      # what the pair screen drops is negligible here too
         assert np.abs(got[:, ~mask]).max() == 0.0 if (~mask).any() else True
     finally:
