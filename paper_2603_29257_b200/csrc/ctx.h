@@ -121,12 +121,12 @@ cudaError_t risp_dens_to_e0(const PairClass &pc, int p0, int p1, int mj, int lan
 cudaError_t risp_e0_to_U(const PairClass &pc, int p0, int p1, int mj, int lane0, int r0, long long ld, long long mstride, int mode,
                          const double *ubar, double *U, cudaStream_t st);
 cudaError_t risp_j_pass1(const PairClass &pc, const risp_eri::PrimPair *prims, const risp_eri::AuxCentre *cen, int ncen, int ncen_pad,
-                         const double *boys_tab, const double *dbar, double *Rpart, cudaStream_t st);
+                         const double *boys_tab, const double *dbar, double *Rpart, int m, cudaStream_t st);
 cudaError_t risp_j_reduce_R(const double *Rpart, int nchunks, const risp_eri::AuxCentre *cen, int ncen, int ncen_pad, double *R, cudaStream_t st);
 // R~ [nauxJ][MS] -> by centre [ceil32(ncen)*4][MS] (zero padded); pass 2 takes the by-centre array
 cudaError_t risp_rt_by_centre(const double *Rt, const risp_eri::AuxCentre *cen, int ncen, double *RtC, cudaStream_t st);
 cudaError_t risp_j_pass2(const PairClass &pc, const risp_eri::PrimPair *prims, const risp_eri::AuxCentre *cen, int ncen, const double *boys_tab,
-                         const double *Rt, double *ubar, cudaStream_t st);
+                         const double *Rt, double *ubar, int m, cudaStream_t st);
 
 // ---- linalg.cu: Cholesky A = L L^T (lower, in place; upper triangle zeroed) and Linv = L^-1, both [n][n] row-major on the device.
 // *info_host = 0 on success, k+1 if the k-th pivot is not positive.

@@ -32,9 +32,11 @@ constexpr int BOYS_NX = 401;           // x in [0, 40]
 constexpr int BOYS_NK = 14;            // orders 0..13: up to m = 6 with an 8-term Taylor expansion
 constexpr double BOYS_XMAX = 40.0;
 
-// F_0..F_M at x.  x < 40: 8-term Taylor series of F_M about the nearest grid point, then the downward recursion
-// F_{m-1} = (2x F_m + e^-x)/(2m-1) (every term positive); x >= 40: F_0 = sqrt(pi/x)/2 and the upward recursion
-// (e^-x < 5e-18 is dropped).
+// F_0..F_M at x.  x < 40: 8-term Taylor series of F_M AND of F_{M+1} about the nearest grid point (two independent Horner chains
+// over the same table row), e^-x from the recurrence itself, e^-x = (2M+1) F_M - 2x F_{M+1} -- no exp() call, no MUFU, no
+// integer scaling work -- then the downward recursion F_{m-1} = (2x F_m + e^-x)/(2m-1) (every term positive).  The absolute
+// error of that e^-x is ~1e-16 (2M+1) F_M, far below the 2x F_m it is added to.  x >= 40: F_0 = sqrt(pi/x)/2 and the upward
+// recursion (e^-x < 5e-18 is dropped).
 template <int M>
 __device__ __forceinline__ void boys(double x, const double *__restrict__ tab, double (&F)[M + 1])
 {
@@ -42,17 +44,26 @@ __device__ __forceinline__ void boys(double x, const double *__restrict__ tab, d
         int i = (int)(x * (1.0 / BOYS_DX) + 0.5);
         double d = (double)i * BOYS_DX - x;                 // -(x - x_i)
         const double *t = tab + i * BOYS_NK + M;
-        double f = __ldg(t + 7) * (1.0 / 5040.0);
-        f = fma(f, d, __ldg(t + 6) * (1.0 / 720.0));
-        f = fma(f, d, __ldg(t + 5) * (1.0 / 120.0));
-        f = fma(f, d, __ldg(t + 4) * (1.0 / 24.0));
-        f = fma(f, d, __ldg(t + 3) * (1.0 / 6.0));
-        f = fma(f, d, __ldg(t + 2) * 0.5);
-        f = fma(f, d, __ldg(t + 1));
-        f = fma(f, d, __ldg(t));
+        double t8 = M > 0 ? __ldg(t + 8) : 0.0;
+        double f = __ldg(t + 7) * (1.0 / 5040.0), g = t8 * (1.0 / 5040.0);
+        double c6 = __ldg(t + 6), c5 = __ldg(t + 5), c4 = __ldg(t + 4), c3 = __ldg(t + 3), c2 = __ldg(t + 2), c1 = __ldg(t + 1), c0 = __ldg(t);
+        f = fma(f, d, c6 * (1.0 / 720.0));
+        f = fma(f, d, c5 * (1.0 / 120.0));
+        f = fma(f, d, c4 * (1.0 / 24.0));
+        f = fma(f, d, c3 * (1.0 / 6.0));
+        f = fma(f, d, c2 * 0.5);
+        f = fma(f, d, c1);
+        f = fma(f, d, c0);
         F[M] = f;
         if (M > 0) {
-            double ex = exp(-x), x2 = 2.0 * x;
+            g = fma(g, d, __ldg(t + 7) * (1.0 / 720.0));
+            g = fma(g, d, c6 * (1.0 / 120.0));
+            g = fma(g, d, c5 * (1.0 / 24.0));
+            g = fma(g, d, c4 * (1.0 / 6.0));
+            g = fma(g, d, c3 * 0.5);
+            g = fma(g, d, c2);
+            g = fma(g, d, c1);                                  // F_{M+1}(x)
+            const double x2 = 2.0 * x, ex = fma(-x2, g, (double)(2 * M + 1) * f);
 #pragma unroll
             for (int m = M; m > 0; --m) F[m - 1] = fma(x2, F[m], ex) * (1.0 / (2 * m - 1));
         }
@@ -87,95 +98,90 @@ struct AuxCentre {       // s and p functions sharing one exponent on one atom
 };
 struct OpParams { double ca, cb, w2; };   // operator (ca + cb erf(w r))/r, w2 = w*w
 
-// ----------------------------------------------------------------------------- vertical recursion, one primitive pair
-// v[cidx(e)][m] = [e0|0]^(m) for deg(e) <= L, m <= MTOP - deg(e).
-template <int L, int MTOP, bool ERF>
-__device__ __forceinline__ void vrr(const PrimPair &pp, double Ax, double Ay, double Az, const AuxCentre &ax, const OpParams &op,
-                                    const double *__restrict__ boys_tab, double (&v)[coff(L + 1)][MTOP + 1],
-                                    double &WCx, double &WCy, double &WCz, double &c3)
-{
-    const double p = pp.p, g = ax.g;
-    const double q = p + g, rsq = rsqrt(q), iq = rsq * rsq;     // 1/(p+g) from the reciprocal square root the prefactor needs anyway
-    const double rho = p * g * iq;
-    const double PCx = pp.Px - ax.x, PCy = pp.Py - ax.y, PCz = pp.Pz - ax.z;
-    const double r2 = PCx * PCx + PCy * PCy + PCz * PCz;
-    const double T = rho * r2;
-    const double pref = pp.cc * rsq * ax.ig;                // cc carries 2 pi^{5/2}/p
-    double F[MTOP + 1];
-    boys<MTOP>(T, boys_tab, F);
-    if (ERF) {
-        // erf(w r)/r: [0]^(m) -> (rho~/rho)^{m+1/2} F_m(rho~ |PC|^2), rho~ = rho w^2/(rho + w^2)
-        double k2 = op.w2 / (rho + op.w2);
-        double G[MTOP + 1];
-        if (op.cb != 0.0) boys<MTOP>(k2 * T, boys_tab, G);
-        double kf = op.cb * sqrt(k2);
-#pragma unroll
-        for (int m = 0; m <= MTOP; ++m) {
-            F[m] = op.ca * F[m] + (op.cb != 0.0 ? kf * G[m] : 0.0);
-            kf *= k2;
-        }
-    }
-#pragma unroll
-    for (int m = 0; m <= MTOP; ++m) v[0][m] = pref * F[m];
-    const double PA[3] = {pp.Px - Ax, pp.Py - Ay, pp.Pz - Az};
-    const double c2 = g * iq;                                // rho / p
-    const double WP[3] = {-c2 * PCx, -c2 * PCy, -c2 * PCz};  // W - P
-    const double c1 = pp.hp;
-#pragma unroll
-    for (int n = 1; n <= L; ++n) {
-#pragma unroll
-        for (int ex = n; ex >= 0; --ex) {
-#pragma unroll
-            for (int ey = n - ex; ey >= 0; --ey) {
-                const int ez = n - ex - ey;
-                const int dir = ex > 0 ? 0 : (ey > 0 ? 1 : 2);
-                const int fx = ex - (dir == 0), fy = ey - (dir == 1), fz = ez - (dir == 2);
-                const int ei = dir == 0 ? fx : (dir == 1 ? fy : fz);
-                const int i1 = cidx(fx, fy, fz);
-#pragma unroll
-                for (int m = 0; m <= MTOP - n; ++m) {
-                    double val = fma(PA[dir], v[i1][m], WP[dir] * v[i1][m + 1]);
-                    if (ei > 0) {
-                        const int i2 = cidx(fx - (dir == 0), fy - (dir == 1), fz - (dir == 2));
-                        val = fma((double)ei * c1, fma(-c2, v[i2][m + 1], v[i2][m]), val);
-                    }
-                    v[cidx(ex, ey, ez)][m] = val;
-                }
-            }
-        }
-    }
-    const double pq = p * iq;
-    WCx = pq * PCx; WCy = pq * PCy; WCz = pq * PCz;          // W - C
-    c3 = 0.5 * iq;
-}
-
-// Emit the e0 integrals of one primitive pair: sink(e_local, c, value), c = 0 (s), 1..3 (p_x, p_y, p_z);
-// e_local runs over degrees LA..LA+LB in cidx order.  Values include the auxiliary normalisation.
+// ----------------------------------------------------------------------------- vertical recursion + emission, one primitive pair
+// v[cidx(e)][m] = [e0|0]^(m) for deg(e) <= L, m <= MTOP - deg(e), built level by level; the e0 integrals of a level are emitted
+// as soon as the level is complete, so that only the two levels below the current one are alive (the (dd| class otherwise keeps
+// all 105 intermediates in registers and spills).  sink(e_local, c, value): c = 0 (s), 1..3 (p_x, p_y, p_z); e_local runs over
+// degrees LA..LA+LB in cidx order.  Values include the auxiliary normalisation.
 template <int LA, int LB, bool HASP, bool ERF, class Sink>
 __device__ __forceinline__ void eri_e0_prim(const PrimPair &pp, double Ax, double Ay, double Az, const AuxCentre &ax,
                                             const OpParams &op, const double *__restrict__ boys_tab, Sink &&sink)
 {
     constexpr int L = LA + LB, MTOP = L + (HASP ? 1 : 0);
     double v[coff(L + 1)][MTOP + 1];
-    double WC[3], c3;
-    vrr<L, MTOP, ERF>(pp, Ax, Ay, Az, ax, op, boys_tab, v, WC[0], WC[1], WC[2], c3);
+    const double p = pp.p, g = ax.g;
+    const double q = p + g, rsq = rsqrt(q), iq = rsq * rsq;     // 1/(p+g) from the reciprocal square root the prefactor needs anyway
+    const double rho = p * g * iq;
+    const double PCx = pp.Px - ax.x, PCy = pp.Py - ax.y, PCz = pp.Pz - ax.z;
+    const double T = rho * (PCx * PCx + PCy * PCy + PCz * PCz);
+    const double pref = pp.cc * rsq * ax.ig;                // cc carries 2 pi^{5/2}/p
+    {
+        double F[MTOP + 1];
+        boys<MTOP>(T, boys_tab, F);
+        if (ERF) {
+            // erf(w r)/r: [0]^(m) -> (rho~/rho)^{m+1/2} F_m(rho~ |PC|^2), rho~ = rho w^2/(rho + w^2)
+            double k2 = op.w2 / (rho + op.w2);
+            double G[MTOP + 1];
+            if (op.cb != 0.0) boys<MTOP>(k2 * T, boys_tab, G);
+            double kf = op.cb * sqrt(k2);
 #pragma unroll
-    for (int n = LA; n <= L; ++n) {
+            for (int m = 0; m <= MTOP; ++m) {
+                F[m] = op.ca * F[m] + (op.cb != 0.0 ? kf * G[m] : 0.0);
+                kf *= k2;
+            }
+        }
 #pragma unroll
-        for (int ex = n; ex >= 0; --ex) {
+        for (int m = 0; m <= MTOP; ++m) v[0][m] = pref * F[m];
+    }
+    const double PA[3] = {pp.Px - Ax, pp.Py - Ay, pp.Pz - Az};
+    const double c2 = g * iq;                                // rho / p
+    const double WP[3] = {-c2 * PCx, -c2 * PCy, -c2 * PCz};  // W - P
+    const double c1 = pp.hp;
+    const double pq = p * iq;
+    const double WC[3] = {pq * PCx, pq * PCy, pq * PCz};     // W - C
+    const double c3 = 0.5 * iq;
 #pragma unroll
-            for (int ey = n - ex; ey >= 0; --ey) {
-                const int ez = n - ex - ey;
-                const int id = cidx(ex, ey, ez);
-                const int el = id - coff(LA);
-                sink(el, 0, ax.ns * v[id][0]);
-                if (HASP) {
-                    const int e3[3] = {ex, ey, ez};
+    for (int n = 0; n <= L; ++n) {
+        if (n > 0) {
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) {
-                        double val = WC[d] * v[id][1];
-                        if (e3[d] > 0) val = fma((double)e3[d] * c3, v[cidx(ex - (d == 0), ey - (d == 1), ez - (d == 2))][1], val);
-                        sink(el, 1 + d, ax.np * val);
+            for (int ex = n; ex >= 0; --ex) {
+#pragma unroll
+                for (int ey = n - ex; ey >= 0; --ey) {
+                    const int ez = n - ex - ey;
+                    const int dir = ex > 0 ? 0 : (ey > 0 ? 1 : 2);
+                    const int fx = ex - (dir == 0), fy = ey - (dir == 1), fz = ez - (dir == 2);
+                    const int ei = dir == 0 ? fx : (dir == 1 ? fy : fz);
+                    const int i1 = cidx(fx, fy, fz);
+                    // levels that are only emitted need m = 0 (s) and m = 1 (p) -- MTOP - n covers exactly that at n = L
+#pragma unroll
+                    for (int m = 0; m <= MTOP - n; ++m) {
+                        double val = fma(PA[dir], v[i1][m], WP[dir] * v[i1][m + 1]);
+                        if (ei > 0) {
+                            const int i2 = cidx(fx - (dir == 0), fy - (dir == 1), fz - (dir == 2));
+                            val = fma((double)ei * c1, fma(-c2, v[i2][m + 1], v[i2][m]), val);
+                        }
+                        v[cidx(ex, ey, ez)][m] = val;
+                    }
+                }
+            }
+        }
+        if (n >= LA) {
+#pragma unroll
+            for (int ex = n; ex >= 0; --ex) {
+#pragma unroll
+                for (int ey = n - ex; ey >= 0; --ey) {
+                    const int ez = n - ex - ey;
+                    const int id = cidx(ex, ey, ez);
+                    const int el = id - coff(LA);
+                    sink(el, 0, ax.ns * v[id][0]);
+                    if (HASP) {
+                        const int e3[3] = {ex, ey, ez};
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) {
+                            double val = WC[d] * v[id][1];
+                            if (e3[d] > 0) val = fma((double)e3[d] * c3, v[cidx(ex - (d == 0), ey - (d == 1), ez - (d == 2))][1], val);
+                            sink(el, 1 + d, ax.np * val);
+                        }
                     }
                 }
             }

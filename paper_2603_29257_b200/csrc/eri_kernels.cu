@@ -145,12 +145,28 @@ __global__ void __launch_bounds__(128) e0_to_U_kernel(const ShellPair *__restric
 // ------------------------------------------------------------------------------------------------- J passes
 constexpr int JW = 4;   // warps per CTA
 
-// Both passes are bound by FP64 arithmetic only if the global loads (primitive pairs, D-bar, R~) are in flight early: at 8
-// warps per SM nothing else hides their latency (ncu: long-scoreboard stalls on the first use of every such load).  So the
-// next primitive pair is fetched while the current one is processed, and the contraction operands are loaded in batches.
-template <int LA, int LB>
-__device__ __forceinline__ void park_integrals(double *__restrict__ g, int lane, bool valid, const ShellPair &sp,
-                                               const PrimPair *__restrict__ prims, const AuxCentre &ax, const double *__restrict__ boys_tab)
+// Both passes have the same shape.  A warp step covers PW shell pairs x CW = 32 / PW aux centres, one (pair, centre) task per lane
+// (lane = s * CW + a): every lane generates the NE x 4 contracted [e0|P) integrals of its task (s and the three p functions of the
+// centre share one recursion) and parks them in shared memory as G[kappa = s NE + e][c CW + a] with row stride KS.  Then the
+// warp contracts the parked block with the trial-vector operand ON THE FP64 TENSOR CORES (DMMA.8x8x4): the contraction is a
+// dense [.. x ..] x [.. x 32 vectors] product, 2 m flops per integral, and as scalar FMAs with their shared-memory operand
+// loads it used more issue slots than the integral generation itself.
+//   pass 1 (Eq. 14):  R[(c, a)][m]     += sum_kappa G[kappa][(c, a)] Dbar[kappa][m]      A = G^T (rows (c,a)), B = Dbar rows
+//   pass 2 (Eq. 16):  Ubar[kappa][m]   += sum_(c,a) G[kappa][(c, a)] R~[(a, c)][m]        A = G (rows kappa),   B = R~ by centre
+// Fragment maps of mma.m8n8k4.f64: lane (q = lane / 4, r = lane % 4) holds A[q][r], B[r][q], C[q][2r], C[q][2r + 1].  The row
+// strides are chosen so that the 32 lanes of an A-fragment load hit 32 different 8-byte words: pass 1 reads G[4t + r][8 mi + q]
+// (KS = 40: r KS mod 32 = 0, 8, 16, 24), pass 2 reads G[8 mi + q][4t + r] (KS = 4 CW + 4: q KS mod 32 = 0, 4, ..., 28).
+__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+// Both passes are bound by FP64 arithmetic only if the global loads (primitive pairs, operands) are in flight early: at 8-16
+// warps per SM nothing else hides their latency.  So the next primitive pair is fetched while the current one is processed.
+// base = parking address of this lane's task: element (e, c) lives at base[e * KS + c * CW].
+template <int LA, int LB, int KS, int CW>
+__device__ __forceinline__ void park_integrals(double *__restrict__ base, bool valid, const ShellPair &sp, const PrimPair *__restrict__ prims,
+                                               const AuxCentre &ax, const double *__restrict__ boys_tab)
 {
     constexpr int NE = ne_of(LA, LB);
     constexpr bool REG = NE * 4 <= 36;          // small classes accumulate the contraction over primitives in registers
@@ -168,16 +184,19 @@ __device__ __forceinline__ void park_integrals(double *__restrict__ g, int lane,
             }
         }
 #pragma unroll
-        for (int k = 0; k < NE * 4; ++k) g[k * 32 + lane] = a[k];
+        for (int e = 0; e < NE; ++e)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) base[e * KS + c * CW] = a[e * 4 + c];
     } else {
 #pragma unroll
-        for (int k = 0; k < NE * 4; ++k) g[k * 32 + lane] = 0.0;
+        for (int e = 0; e < NE; ++e)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) base[e * KS + c * CW] = 0.0;
         if (valid) {
             OpParams op{1.0, 0.0, 0.0};      // dp, dd: no prefetch, the recursion needs every register
             for (int k = 0; k < sp.npp; ++k) {
                 const PrimPair pp = prims[sp.ppoff + k];
-                eri_e0_prim<LA, LB, true, false>(pp, sp.Ax, sp.Ay, sp.Az, ax, op, boys_tab,
-                                                 [&](int e, int c, double v) { g[(e * 4 + c) * 32 + lane] += v; });
+                eri_e0_prim<LA, LB, true, false>(pp, sp.Ax, sp.Ay, sp.Az, ax, op, boys_tab, [&](int e, int c, double v) { base[e * KS + c * CW] += v; });
             }
         }
     }
@@ -193,130 +212,140 @@ __global__ void rt_by_centre_kernel(const double *__restrict__ Rt, const AuxCent
     RtC[(long long)k * MS + lane] = q >= 0 ? Rt[(long long)q * MS + lane] : 0.0;
 }
 
-// pass 2: one pair per warp, 32 aux centres per step.  ubar[(e_off + pair*NE + e)*MS + mi]
+template <int LA, int LB>
+struct Pass2Cfg {
+    static constexpr int NE = ne_of(LA, LB);
+    // pairs per warp step: as many as keep the accumulator tile (8-row blocks of PW NE rows x 32 vectors) at <= 32 doubles per lane
+    static constexpr int PW = NE <= 6 ? 4 : (NE <= 16 ? 2 : 1);
+    static constexpr int CW = 32 / PW, KS = 4 * CW + 4, MROWS = PW * NE, M8 = (MROWS + 7) / 8 * 8, MT = M8 / 8;
+    static constexpr size_t SMEM_PER_WARP = (size_t)M8 * KS * sizeof(double);
+};
+
+// pass 2: a warp owns PW pairs and walks over all aux centres, CW per step.  ubar[(e_off + pair*NE + e)*MS + m]
 template <int LA, int LB>
 __global__ void __launch_bounds__(32 * JW) j_pass2_kernel(const ShellPair *__restrict__ pairs, int npairs, const PrimPair *__restrict__ prims,
                                                           const AuxCentre *__restrict__ cen, int ncen, const double *__restrict__ boys_tab,
-                                                          const double *__restrict__ RtC, long long e_off, double *__restrict__ ubar)
+                                                          const double *__restrict__ RtC, long long e_off, double *__restrict__ ubar, int njn)
 {
-    constexpr int NE = ne_of(LA, LB);
+    using C = Pass2Cfg<LA, LB>;
+    constexpr int NE = C::NE, PW = C::PW, CW = C::CW, KS = C::KS, MROWS = C::MROWS, M8 = C::M8, MT = C::MT;
     extern __shared__ double smem[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    double *g = smem + (size_t)w * NE * 4 * 32;
-    const int pi = blockIdx.x * JW + w;
-    if (pi >= npairs) return;
-    const ShellPair sp = pairs[pi];
-    double acc[NE];
+    double *g = smem + (size_t)w * M8 * KS;
+    const int pg = (blockIdx.x * JW + w) * PW;
+    if (pg >= npairs) return;
+    const int s = lane / CW, a = lane % CW, q = lane >> 2, r = lane & 3;
+    const bool pvalid = pg + s < npairs;
+    const ShellPair sp = pairs[min(pg + s, npairs - 1)];
+    for (int i = MROWS * KS + lane; i < M8 * KS; i += 32) g[i] = 0.0;      // padding rows of the last 8-row block
+    double acc[MT][4][2];
 #pragma unroll
-    for (int e = 0; e < NE; ++e) acc[e] = 0.0;
-    AuxCentre ax = cen[min(lane, ncen - 1)];
-    for (int c0 = 0; c0 < ncen; c0 += 32) {
-        const bool valid = c0 + lane < ncen;
-        const AuxCentre ax_next = cen[min(c0 + 32 + lane, ncen - 1)];
-        park_integrals<LA, LB>(g, lane, valid, sp, prims, ax, boys_tab);
+    for (int i = 0; i < MT; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    AuxCentre ax = cen[min(a, ncen - 1)];
+    double *base = g + (size_t)s * NE * KS + a;
+    for (int c0 = 0; c0 < ncen; c0 += CW) {
+        const bool valid = pvalid && c0 + a < ncen;
+        const AuxCentre ax_next = cen[min(c0 + CW + a, ncen - 1)];
+        park_integrals<LA, LB, KS, CW>(base, valid, sp, prims, ax, boys_tab);
         ax = ax_next;
         __syncwarp();
-        const double *rc = RtC + (long long)c0 * 4 * MS + lane;
-#pragma unroll 2
-        for (int s = 0; s < 32; s += 4) {           // padding centres carry zero integrals and zero R~
-            double rt[4][4];
+#pragma unroll 4
+        for (int t = 0; t < CW; ++t) {              // K = 4 CW = (c, a) in steps of 4
+            const int kk = 4 * t + r, c = kk / CW, aa = kk % CW;
+            const double *rc = RtC + ((long long)(c0 + aa) * 4 + c) * MS + q;      // padding centres carry zero integrals and zero R~
+            double bf[4], af[MT];
 #pragma unroll
-            for (int h = 0; h < 4; ++h)
+            for (int j = 0; j < 4; ++j) bf[j] = j < njn ? rc[8 * j] : 0.0;
 #pragma unroll
-                for (int c = 0; c < 4; ++c) rt[h][c] = rc[(long long)((s + h) * 4 + c) * MS];
+            for (int i = 0; i < MT; ++i) af[i] = g[(8 * i + q) * KS + kk];
 #pragma unroll
-            for (int e = 0; e < NE; ++e)
+            for (int i = 0; i < MT; ++i)
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    const double2 g0 = *reinterpret_cast<const double2 *>(&g[(e * 4 + c) * 32 + s]);
-                    const double2 g1 = *reinterpret_cast<const double2 *>(&g[(e * 4 + c) * 32 + s + 2]);
-                    acc[e] = fma(g0.x, rt[0][c], fma(g0.y, rt[1][c], fma(g1.x, rt[2][c], fma(g1.y, rt[3][c], acc[e]))));
-                }
+                for (int j = 0; j < 4; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
         }
         __syncwarp();
     }
 #pragma unroll
-    for (int e = 0; e < NE; ++e) ubar[(e_off + (long long)pi * NE + e) * MS + lane] = acc[e];
+    for (int i = 0; i < MT; ++i) {
+        const int row = 8 * i + q;
+        if (row < MROWS && pg + row / NE < npairs) {
+            double *dst = ubar + (e_off + (long long)pg * NE + row) * MS + 2 * r;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) *reinterpret_cast<double2 *>(dst + 8 * j) = make_double2(acc[i][j][0], acc[i][j][1]);
+        }
+    }
 }
 
 // pass 1: CTA = (pair chunk, 8 aux centres); warp step = 4 pairs x 8 centres.
 // Rpart[((chunk_global * ncen_pad + centre) * 4 + comp) * MS + mi]
+constexpr int P1_KS = 40;
 template <int LA, int LB>
 __global__ void __launch_bounds__(32 * JW) j_pass1_kernel(const ShellPair *__restrict__ pairs, int npairs, int chunk, int chunk_base,
                                                           const PrimPair *__restrict__ prims, const AuxCentre *__restrict__ cen, int ncen,
                                                           int ncen_pad, const double *__restrict__ boys_tab, const double *__restrict__ dbar,
-                                                          long long e_off, double *__restrict__ Rpart)
+                                                          long long e_off, double *__restrict__ Rpart, int njn)
 {
-    constexpr int NE = ne_of(LA, LB);
-    constexpr bool PRE = 4 * NE <= 12;      // D-bar of the step's four pairs fetched before the integrals are generated
+    constexpr int NE = ne_of(LA, LB), KS = P1_KS, KROWS = 4 * NE;
     extern __shared__ double smem[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    double *g = smem + (size_t)w * NE * 4 * 32;
+    double *g = smem + (size_t)w * KROWS * KS;
     const int p_begin = blockIdx.x * chunk, p_end = min(npairs, p_begin + chunk);
-    const int ci = blockIdx.y * 8 + (lane & 7), slot = lane >> 3;
+    const int slot = lane >> 3, a = lane & 7, q = lane >> 2, r = lane & 3;
+    const int ci = blockIdx.y * 8 + a;
     const bool cvalid = ci < ncen;
     const AuxCentre ax = cen[cvalid ? ci : 0];
-    double acc[32];
+    double acc[4][4][2];
 #pragma unroll
-    for (int k = 0; k < 32; ++k) acc[k] = 0.0;
-    constexpr bool LEAN = NE > 10;          // dp, dd: the recursion already spills; no operand batching, no shell-pair prefetch
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    constexpr bool LEAN = NE > 10;          // dp, dd: the recursion already spills; no shell-pair prefetch
     ShellPair sp = pairs[min(p_begin + w * 4 + slot, p_end - 1)];
+    double *base = g + (size_t)slot * NE * KS + a;
     for (int pg = p_begin + w * 4; pg < p_end; pg += JW * 4) {
         const int pi = pg + slot;
         const bool valid = cvalid && pi < p_end;
         if constexpr (LEAN) sp = pairs[min(pi, p_end - 1)];
         ShellPair sp_next;
         if constexpr (!LEAN) sp_next = pairs[min(pi + JW * 4, p_end - 1)];
-        const double *db = dbar + (e_off + (long long)pg * NE) * MS + lane;
-        const int ns = min(4, p_end - pg);
-        double dpre[PRE ? 4 * NE : 1];
-        if constexpr (PRE) {
-#pragma unroll
-            for (int k = 0; k < 4 * NE; ++k) dpre[k] = (k / NE < ns) ? db[(long long)k * MS] : 0.0;
-        }
-        park_integrals<LA, LB>(g, lane, valid, sp, prims, ax, boys_tab);
+        park_integrals<LA, LB, KS, 8>(base, valid, sp, prims, ax, boys_tab);
         if constexpr (!LEAN) sp = sp_next;
         __syncwarp();
-#pragma unroll(LEAN ? 1 : 4)
-        for (int s = 0; s < 4; ++s) {
-            if (s >= ns) break;
-            double dv[LEAN ? 1 : NE];
-            if constexpr (!LEAN) {
+        const double *db = dbar + (e_off + (long long)pg * NE) * MS + q;
+#pragma unroll 4
+        for (int t = 0; t < NE; ++t) {              // K = 4 NE = (pair, e) in steps of 4
+            const int kk = 4 * t + r;
+            const bool kv = pg + kk / NE < p_end;   // rows of pairs beyond the chunk: parked zeros, operand not read
+            double bf[4], af[4];
 #pragma unroll
-                for (int e = 0; e < NE; ++e) {
-                    if constexpr (PRE) dv[e] = dpre[s * NE + e];
-                    else dv[e] = db[(long long)(s * NE + e) * MS];
-                }
-            }
+            for (int j = 0; j < 4; ++j) bf[j] = (kv && j < njn) ? db[(long long)kk * MS + 8 * j] : 0.0;
 #pragma unroll
-            for (int e = 0; e < NE; ++e) {
-                double d;
-                if constexpr (LEAN) d = db[(long long)(s * NE + e) * MS];
-                else d = dv[e];
+            for (int i = 0; i < 4; ++i) af[i] = g[kk * KS + 8 * i + q];
 #pragma unroll
-                for (int c = 0; c < 4; ++c)
+            for (int i = 0; i < 4; ++i)
 #pragma unroll
-                    for (int a = 0; a < 8; a += 2) {
-                        const double2 gg = *reinterpret_cast<const double2 *>(&g[(e * 4 + c) * 32 + s * 8 + a]);
-                        acc[a * 4 + c] = fma(gg.x, d, acc[a * 4 + c]);
-                        acc[(a + 1) * 4 + c] = fma(gg.y, d, acc[(a + 1) * 4 + c]);
-                    }
-            }
+                for (int j = 0; j < 4; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
         }
         __syncwarp();
     }
-    // cross-warp reduction (fixed order -> deterministic) in a dedicated region after the parking area
+    // cross-warp reduction (fixed order -> deterministic) in a dedicated region after the parking area: red[w][k = a*4 + c][m];
+    // this lane holds, for component c = i, centre a = q and vectors m = 8j + 2r, 8j + 2r + 1
     __syncthreads();
-    double *red = smem + (size_t)JW * NE * 4 * 32;     // [JW][32][32]
+    double *red = smem + (size_t)JW * KROWS * KS;     // [JW][32][32]
 #pragma unroll
-    for (int k = 0; k < 32; ++k) red[(w * 32 + k) * 32 + lane] = acc[k];
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            *reinterpret_cast<double2 *>(&red[(w * 32 + q * 4 + i) * 32 + 8 * j + 2 * r]) = make_double2(acc[i][j][0], acc[i][j][1]);
     __syncthreads();
     for (int k = w; k < 32; k += JW) {
         double s = 0.0;
 #pragma unroll
         for (int ww = 0; ww < JW; ++ww) s += red[(ww * 32 + k) * 32 + lane];
-        const int a = k >> 2, c = k & 3;
-        const int cc = blockIdx.y * 8 + a;
+        const int aa = k >> 2, c = k & 3;
+        const int cc = blockIdx.y * 8 + aa;
         if (cc < ncen) Rpart[(((long long)(chunk_base + blockIdx.x) * ncen_pad + cc) * 4 + c) * MS + lane] = s;
     }
 }
@@ -367,7 +396,7 @@ template <class K>
 cudaError_t ensure_smem(K kernel, size_t bytes)
 {
     if (bytes <= 48 * 1024) return cudaSuccess;
-    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);      // per device, cheap: set on every launch
 }
 
 }  // namespace
@@ -418,18 +447,18 @@ cudaError_t risp_e0_to_U(const PairClass &pc, int p0, int p1, int mj, int lane0,
 }
 
 cudaError_t risp_j_pass1(const PairClass &pc, const PrimPair *prims, const AuxCentre *cen, int ncen, int ncen_pad, const double *boys_tab,
-                         const double *dbar, double *Rpart, cudaStream_t st)
+                         const double *dbar, double *Rpart, int m, cudaStream_t st)
 {
     if (pc.npairs <= 0) return cudaSuccess;
     cudaError_t err = cudaSuccess;
     dispatch_class(pc.la, pc.lb, [&](auto LA, auto LB) {
         constexpr int A = decltype(LA)::value, B = decltype(LB)::value;
-        size_t smem = ((size_t)JW * ne_of(A, B) * 4 * 32 + (size_t)JW * 32 * 32) * sizeof(double);
+        size_t smem = ((size_t)JW * 4 * ne_of(A, B) * P1_KS + (size_t)JW * 32 * 32) * sizeof(double);
         err = ensure_smem(j_pass1_kernel<A, B>, smem);
         if (err != cudaSuccess) return;
         dim3 grid(pc.nchunks, (ncen + 7) / 8);
         j_pass1_kernel<A, B><<<grid, 32 * JW, smem, st>>>(pc.d_pairs, pc.npairs, pc.chunk, pc.chunk_base, prims, cen, ncen, ncen_pad, boys_tab,
-                                                          dbar, pc.e_off, Rpart);
+                                                          dbar, pc.e_off, Rpart, (m + 7) / 8);
     });
     return err != cudaSuccess ? err : cudaGetLastError();
 }
@@ -448,16 +477,19 @@ cudaError_t risp_rt_by_centre(const double *Rt, const AuxCentre *cen, int ncen, 
 }
 
 cudaError_t risp_j_pass2(const PairClass &pc, const PrimPair *prims, const AuxCentre *cen, int ncen, const double *boys_tab, const double *Rt,
-                         double *ubar, cudaStream_t st)
+                         double *ubar, int m, cudaStream_t st)
 {
     if (pc.npairs <= 0) return cudaSuccess;
     cudaError_t err = cudaSuccess;
     dispatch_class(pc.la, pc.lb, [&](auto LA, auto LB) {
         constexpr int A = decltype(LA)::value, B = decltype(LB)::value;
-        size_t smem = (size_t)JW * ne_of(A, B) * 4 * 32 * sizeof(double);
+        using C = Pass2Cfg<A, B>;
+        size_t smem = (size_t)JW * C::SMEM_PER_WARP;
         err = ensure_smem(j_pass2_kernel<A, B>, smem);
         if (err != cudaSuccess) return;
-        j_pass2_kernel<A, B><<<(pc.npairs + JW - 1) / JW, 32 * JW, smem, st>>>(pc.d_pairs, pc.npairs, prims, cen, ncen, boys_tab, Rt, pc.e_off, ubar);
+        const int per_cta = JW * C::PW;
+        j_pass2_kernel<A, B><<<(pc.npairs + per_cta - 1) / per_cta, 32 * JW, smem, st>>>(pc.d_pairs, pc.npairs, prims, cen, ncen, boys_tab, Rt, pc.e_off,
+                                                                                         ubar, (m + 7) / 8);
     });
     return err != cudaSuccess ? err : cudaGetLastError();
 }

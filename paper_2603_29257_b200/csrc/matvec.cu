@@ -205,7 +205,7 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
     if ((rc = fork_classes(ctx, st))) return rc;
     for (int c = 5; c >= 0; --c)          // heaviest recursion first
         if (ctx->cls[c].npairs) {
-            RISP_CUDA_TRY(risp_j_pass1(ctx->cls[c], ctx->d_prims, ctx->d_cenJ, ctx->ncenJ, ctx->ncenJ_pad, ctx->d_boys, ctx->w_dbar, ctx->w_Rpart, ctx->cls_st[c]));
+            RISP_CUDA_TRY(risp_j_pass1(ctx->cls[c], ctx->d_prims, ctx->d_cenJ, ctx->ncenJ, ctx->ncenJ_pad, ctx->d_boys, ctx->w_dbar, ctx->w_Rpart, m, ctx->cls_st[c]));
             ++launches;
         }
     if ((rc = join_classes(ctx, st))) return rc;
@@ -219,7 +219,7 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
     if ((rc = fork_classes(ctx, st))) return rc;
     for (int c = 5; c >= 0; --c)
         if (ctx->cls[c].npairs) {
-            RISP_CUDA_TRY(risp_j_pass2(ctx->cls[c], ctx->d_prims, ctx->d_cenJ, ctx->ncenJ, ctx->d_boys, ctx->w_RtC, ctx->w_dbar, ctx->cls_st[c]));
+            RISP_CUDA_TRY(risp_j_pass2(ctx->cls[c], ctx->d_prims, ctx->d_cenJ, ctx->ncenJ, ctx->d_boys, ctx->w_RtC, ctx->w_dbar, m, ctx->cls_st[c]));
             ++launches;
         }
     if ((rc = join_classes(ctx, st))) return rc;
