@@ -88,6 +88,8 @@ typedef struct {
 
 #define RISP_FLAG_KEEP_STAGES 1   /* keep J_mia of the last risp_matvec for risp_get_stage (costs one more [m][nocc][nvir] buffer) */
 #define RISP_FLAG_SPILL_HALF 2    /* testing: place the upper half of the K-tensor slices in pinned host memory regardless of the budget */
+#define RISP_FLAG_TDDFT 8         /* also build T_ia^P' over the exchange window, kept whole in HBM: enables risp_matvec_tddft
+                                     and risp_tddft_solve (full TDDFT-risp, Eq. 1-2) */
 #define RISP_FLAG_SMALL_KBUILD 4  /* testing: build the K tensors in runs of at most 5 auxiliary functions (the large-system code path) */
 
 typedef struct {
@@ -163,6 +165,13 @@ int risp_setup(const risp_system *sys, const risp_options *opt, risp_ctx **out);
  * (RISP_ENOMEM if that no longer fits beside the K tensors).  risp_get_timings / risp_get_stage refer to the last sub-batch. */
 int risp_matvec(risp_ctx *ctx, int32_t m, const double *X_dev, double *sigma_dev, void *cuda_stream);
 
+/* Full TDDFT-risp (Eq. 1-2; XC kernel dropped): for m trial vectors
+ *     sigma_plus  = (A+B) X = Delta X + 4 J X - K1 X - K2 X,        sigma_minus = (A-B) X = Delta X - K1 X + K2 X,
+ * J = (ia|jb)_RI-J, K1 = (ij|J^|ab)_RI-K, K2 = (ib|J^|ja)_RI-K, the two exchange terms restricted to the exchange window
+ * (reading G25: Eq. 2a's "2(ia|jb)" is read as 4(ia|jb), consistent with Eq. 10 and Eq. 2b).  Needs RISP_FLAG_TDDFT at
+ * setup.  All three buffers DEVICE [m][nocc][nvir], pairwise disjoint; asynchronous on cuda_stream. */
+int risp_matvec_tddft(risp_ctx *ctx, int32_t m, const double *X_dev, double *sigma_plus_dev, double *sigma_minus_dev, void *cuda_stream);
+
 /* Same with HOST buffers: copies X in, runs risp_matvec, copies sigma out, synchronises. */
 int risp_matvec_host(risp_ctx *ctx, int32_t m, const double *X_host, double *sigma_host);
 
@@ -182,6 +191,15 @@ int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_options *opt,
  * (one AO matrix, one half-transformed matrix, six [nocc][nvir] blocks). */
 int risp_transition_properties(risp_ctx *ctx, int32_t n, const double *X_dev, const double *omega_hartree, const double *origin_bohr,
                                double scale, double *mu_out, double *m_out, double *f_out, double *R_out);
+
+/* Lowest `nroots` (<= 32) excitation energies of full TDDFT-risp, the symplectic problem Eq. 1, by a Davidson
+ * iteration that projects A+B and A-B into one orthonormal trial space (reading G26).  Needs
+ * RISP_FLAG_TDDFT at setup; the subspace (b, (A+B) b, (A-B) b) is device resident and the iteration restarts from {X+Y, X-Y} when
+ * it is full.  omega_hartree: HOST [nroots] ascending; X_out, Y_out: DEVICE [nroots][nocc][nvir] or NULL, normalised to
+ * <X|X> - <Y|Y> = 1.  Options as risp_tda_solve (tol on max(|r1|, |r2|), max_iter, n_guess, max_sub, device_budget_bytes);
+ * RISP_ENOTPD if the projected A-B is not positive definite. */
+int risp_tddft_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_options *opt, double *omega_hartree, double *X_out, double *Y_out,
+                     risp_solve_info *info);
 
 void risp_destroy(risp_ctx *ctx);
 const char *risp_last_error(const risp_ctx *ctx); /* static text if ctx == NULL */

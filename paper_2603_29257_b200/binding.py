@@ -10,10 +10,10 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
 EXPORTED_SYMBOLS = ["risp_setup", "risp_matvec", "risp_matvec_host", "risp_tda_solve", "risp_destroy", "risp_last_error",
-                    "risp_get_dims", "risp_get_timings", "risp_eri3c_shell", "risp_get_stage", "risp_transition_properties"]
+                    "risp_get_dims", "risp_get_timings", "risp_eri3c_shell", "risp_get_stage", "risp_transition_properties", "risp_matvec_tddft", "risp_tddft_solve"]
 
 RISP_MAX_ROOTS = 64
-FLAG_KEEP_STAGES, FLAG_SPILL_HALF = 1, 2
+FLAG_KEEP_STAGES, FLAG_SPILL_HALF, FLAG_SMALL_KBUILD, FLAG_TDDFT = 1, 2, 4, 8
 SOLVE_NO_CACHE, SOLVE_TINY_CACHE, SOLVE_PERTURBED_GUESS, SOLVE_HOST_FP32 = 1, 2, 4, 8
 STAGE = dict(R=1, RTILDE=2, J=3, K=4, TIJ=5, TAB=6, PAIRS=7, METRIC_J=8, METRIC_K=9, U=10)
 _ERR = {-1: "RISP_EINVAL", -2: "RISP_ENOMEM", -3: "RISP_ECUDA", -4: "RISP_ENOTPD", -5: "RISP_ENOTCONV"}
@@ -93,6 +93,8 @@ def load_library():
     lib.risp_get_timings.argtypes = [vp, C.POINTER(_Timings)]
     lib.risp_eri3c_shell.argtypes = [vp, i32, i32, i32, i32, vp]
     lib.risp_get_stage.argtypes = [vp, i32, vp, i64, vp]
+    lib.risp_matvec_tddft.argtypes = [vp, i32, vp, vp, vp, vp]
+    lib.risp_tddft_solve.argtypes = [vp, i32, C.POINTER(_SolveOptions), C.POINTER(dbl), vp, vp, C.POINTER(_SolveInfo)]
     lib.risp_transition_properties.argtypes = [vp, i32, vp, vp, vp, dbl, vp, vp, vp, vp]
     # include/risp_debug.h
     lib.risp_debug_oneel_ao.argtypes = [vp, vp, vp]
@@ -203,6 +205,32 @@ class RispContext:
         d = _struct_dict(info)
         d["resid"] = d["resid"][:nroots]
         return omega, X, d
+
+    def matvec_tddft(self, X, stream=None):
+        """risp_matvec_tddft: ((A+B) X, (A-B) X) for the device vectors X[m][nocc][nvir]."""
+        import torch
+        assert X.is_cuda and X.dtype == torch.float64 and X.is_contiguous()
+        sp, sm = torch.empty_like(X), torch.empty_like(X)
+        st = torch.cuda.current_stream(X.device).cuda_stream if stream is None else stream
+        self._check(self.lib.risp_matvec_tddft(self.handle, X.shape[0], X.data_ptr(), sp.data_ptr(), sm.data_ptr(), st))
+        return sp, sm
+
+    def tddft_solve(self, nroots, tol=1e-5, max_iter=100, n_guess=0, max_sub=0, want_vectors=False, allow_unconverged=False, device_budget_bytes=0):
+        import torch
+        omega = np.zeros(nroots)
+        info = _SolveInfo()
+        opt = _SolveOptions(float(tol), int(max_iter), int(n_guess), int(max_sub), 0, 0, 0, int(device_budget_bytes))
+        X = Y = None
+        if want_vectors:
+            X = torch.empty((nroots, self.nocc, self.nvir), dtype=torch.float64, device=f"cuda:{self.device}")
+            Y = torch.empty_like(X)
+        rc = self.lib.risp_tddft_solve(self.handle, nroots, C.byref(opt), omega.ctypes.data_as(C.POINTER(C.c_double)),
+                                       X.data_ptr() if X is not None else None, Y.data_ptr() if Y is not None else None, C.byref(info))
+        if rc != 0 and not (rc == -5 and allow_unconverged):
+            self._check(rc)
+        d = _struct_dict(info)
+        d["resid"] = d["resid"][:nroots]
+        return omega, X, Y, d
 
     def transition_properties(self, X, omega, origin=None, scale=0.0):
         """risp_transition_properties: (mu[n][3], m[n][3], f[n], R[n]) for the device vectors X[n][nocc][nvir]."""

@@ -85,6 +85,8 @@ struct risp_ctx {
     long long tri_o = 0, tri_v = 0;
     int nK_dev = 0;
     double *d_TijP = nullptr, *d_TabP = nullptr;    // [nK_dev][tri_o], [nK_dev][tri_v]
+    double *d_LinvK = nullptr;    // L_K^-1 of the K metric (RISP_FLAG_TDDFT only)
+    double *d_Tov = nullptr;      // full TDDFT only (RISP_FLAG_TDDFT): L_K^-1 (ia|J^|Q) over the window, [nauxK][noccK][nv_p] (T_ia^P')
     double *h_TijP = nullptr, *h_TabP = nullptr;    // pinned [nauxK - nK_dev][tri]
     // ---- matvec work space (sized for m_cap vectors)
     int m_cap = 0;
@@ -137,6 +139,7 @@ cudaError_t risp_metric_solve32(const double *Linv, int n, const double *R, doub
 cudaError_t risp_gather_window(const double *X, double *Xk, int m, int nocc, int nvir, int o0, int no, int v0, int nv, int ldk, cudaStream_t st);
 cudaError_t risp_diag_sigma(const double *X, const double *eps, double *sigma, int m, int nocc, int nvir, cudaStream_t st);
 cudaError_t risp_sub_window(const double *Kk, double *sigma, int m, int nocc, int nvir, int o0, int no, int v0, int nv, int ldk, cudaStream_t st);
+cudaError_t risp_axpy_window(const double *Kk, double scale, double *sigma, int m, int nocc, int nvir, int o0, int no, int v0, int nv, int ldk, cudaStream_t st);
 cudaError_t risp_scatter_window(const double *Kk, double *Kfull, int m, int nocc, int nvir, int o0, int no, int v0, int nv, int ldk, cudaStream_t st);
 // packed lower triangle [n(n+1)/2] <-> full symmetric [n][ld]; batched over np slices
 cudaError_t risp_pack_sym(const double *full, long long full_stride, int ld, int n, int np, double *packed, long long tri, cudaStream_t st);
@@ -146,6 +149,11 @@ cudaError_t risp_expand_sym(const double *packed, long long tri, int n, int np, 
 // ---- setup.cu / matvec.cu / solve.cu internals
 int risp_ensure_workspace(risp_ctx *ctx, int m);
 size_t risp_plan_workspace(const risp_ctx *ctx, int m, size_t avail, MatvecPlan &plan, bool spilled);
-int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaStream_t st);
+// sigma = A X (TDA).  With sigma_minus != nullptr (full TDDFT, needs d_Tov): sigma = (A+B) X, sigma_minus = (A-B) X (Eq. 2).
+int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaStream_t st, double *sigma_minus = nullptr);
 int risp_build_pair(risp_ctx *ctx, int shA, int shB, risp_eri::ShellPair &sp, std::vector<risp_eri::PrimPair> &pp, double prim_tol);
 void risp_free_workspace(risp_ctx *ctx);
+int risp_rows_gram(risp_ctx *ctx, const double *A, int na, const double *B, int nb, long long dim, long long slice, double *dPart, double *dSmall,
+                   std::vector<double> &out, cudaStream_t st);
+int risp_rows_lincomb(risp_ctx *ctx, const double *coef_host, int nc, int na, const double *A, double *C, long long dim, double alpha, double beta,
+                      double *dCoef, cudaStream_t st);

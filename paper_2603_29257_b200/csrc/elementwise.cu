@@ -55,6 +55,19 @@ __global__ void __launch_bounds__(256) sub_window_kernel(const double *__restric
     }
 }
 
+// sigma[m][o0+i][v0+a] += scale * K'[m][i][a]   (the (ib|ja) term of full TDDFT enters A+B and A-B with opposite signs, Eq. 2)
+__global__ void __launch_bounds__(256) axpy_window_kernel(const double *__restrict__ Kk, double scale, double *__restrict__ sigma, long long rows, int nocc,
+                                                          int nvir, int o0, int no, int v0, int nv, int ldk)
+{
+    for (long long r = blockIdx.x; r < rows; r += gridDim.x) {
+        const long long mi = r / no;
+        const int i = (int)(r - mi * no);
+        double *dst = sigma + (mi * nocc + o0 + i) * (long long)nvir + v0;
+        const double *src = Kk + r * ldk;
+        for (int a = threadIdx.x; a < nv; a += blockDim.x) dst[a] = fma(scale, src[a], dst[a]);
+    }
+}
+
 __global__ void scatter_window_kernel(const double *__restrict__ Kk, double *__restrict__ Kf, long long total, int nocc, int nvir, int o0,
                                       int no, int v0, int nv, int ldk)
 {
@@ -132,6 +145,13 @@ cudaError_t risp_sub_window(const double *Kk, double *sigma, int m, int nocc, in
     long long rows = (long long)m * no;
     if (rows == 0 || nv == 0) return cudaSuccess;
     sub_window_kernel<<<rows_grid(rows), nv >= 256 ? 256 : 128, 0, st>>>(Kk, sigma, rows, nocc, nvir, o0, no, v0, nv, ldk);
+    return cudaGetLastError();
+}
+cudaError_t risp_axpy_window(const double *Kk, double scale, double *sigma, int m, int nocc, int nvir, int o0, int no, int v0, int nv, int ldk, cudaStream_t st)
+{
+    long long rows = (long long)m * no;
+    if (rows == 0 || nv == 0) return cudaSuccess;
+    axpy_window_kernel<<<rows_grid(rows), nv >= 256 ? 256 : 128, 0, st>>>(Kk, scale, sigma, rows, nocc, nvir, o0, no, v0, nv, ldk);
     return cudaGetLastError();
 }
 cudaError_t risp_scatter_window(const double *Kk, double *Kf, int m, int nocc, int nvir, int o0, int no, int v0, int nv, int ldk, cudaStream_t st)

@@ -156,8 +156,10 @@ static int join_classes(risp_ctx *ctx, cudaStream_t st)
     return RISP_OK;
 }
 
-int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaStream_t st)
+int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaStream_t st, double *sigma_minus)
 {
+    const bool tddft = sigma_minus != nullptr;
+    if (tddft && ctx->has_K && !ctx->d_Tov) { risp_set_error(ctx, "risp_matvec_tddft: the context was set up without RISP_FLAG_TDDFT"); return RISP_EINVAL; }
     const int nao = ctx->nao, nocc = ctx->nocc, nvir = ctx->nvir, nJ = ctx->nauxJ;
     const int no = ctx->noccK, nv = ctx->nvirK, nK = ctx->nauxK, no_p = ctx->no_p, nv_p = ctx->nv_p;
     const long long ldao = ctx->ldao, ldocc = ctx->ldocc, ldvir = ctx->ldvir;
@@ -169,6 +171,7 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
     RISP_CUDA_TRY(cudaEventRecord(ev[0], st));
     // ---------------- diagonal (Eq. 10)
     RISP_CUDA_TRY(risp_diag_sigma(X, ctx->d_eps, sigma, m, nocc, nvir, st)); ++launches;
+    if (tddft) { RISP_CUDA_TRY(risp_diag_sigma(X, ctx->d_eps, sigma_minus, m, nocc, nvir, st)); ++launches; }
     // J-phase views of the arena
     double *wY = ctx->w_arena;                                   // [mj][nocc][ldao]
     double *wD = wY + (size_t)pl.mj * nocc * ldao;               // [mj][prow][ldao]
@@ -253,7 +256,8 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
             GemmDesc e = gemm_desc(mj * nocc, nvir, nao, wY, ldao, true, ctx->d_Cvir, ldvir, false, ctx->w_J + (size_t)l0 * nocc * nvir, nvir);
             RISP_CUDA_TRY(risp_dgemm(e, st)); ++launches;
         }
-        GemmDesc e = gemm_desc(mj * nocc, nvir, nao, wY, ldao, true, ctx->d_Cvir, ldvir, false, Sb, nvir, 2.0, 1.0);
+        // the Coulomb term enters A with 2 (ia|jb) (Eq. 10) and A+B with 4 (ia|jb) (Eq. 2a, reading G25); A-B has none
+        GemmDesc e = gemm_desc(mj * nocc, nvir, nao, wY, ldao, true, ctx->d_Cvir, ldvir, false, Sb, nvir, tddft ? 4.0 : 2.0, 1.0);
         RISP_CUDA_TRY(risp_dgemm(e, st)); ++launches;
     }
     RISP_CUDA_TRY(cudaEventRecord(ev[5], st));
@@ -333,6 +337,29 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
         }
         RISP_CUDA_TRY(cudaEventRecord(ev[7], st));
         RISP_CUDA_TRY(risp_sub_window(wKk, sigma, m, nocc, nvir, ctx->occK0, no, ctx->virK0, nv, nv_p, st)); ++launches;
+        if (tddft) {
+            RISP_CUDA_TRY(risp_sub_window(wKk, sigma_minus, m, nocc, nvir, ctx->occK0, no, ctx->virK0, nv, nv_p, st)); ++launches;
+            // ---------------- (ib|ja) term of full TDDFT (Eq. 2): K2_mia = sum_P sum_j (sum_b T_ib^P X'_mjb) T_ja^P with the whitened
+            //                  T^P = L_K^-1 (ov|J^|Q).  Contracting b first costs 4 m N_auxK o'^2 v' flops (o' < v').
+            const long long ldw_max = (long long)((ctx->plan.arena_bytes / 8 - 2 * (size_t)m * no * nv_p) / ((size_t)m * no)) & ~1LL;
+            const int pc2 = (int)std::min<long long>(nK, ldw_max / std::max(no, 1));
+            if (pc2 < 1) { risp_set_error(ctx, "risp_matvec_tddft: work space too small for the (ib|ja) contraction"); return RISP_ENOMEM; }
+            const long long ldw = ((long long)pc2 * no + 1) & ~1LL;
+            double *wW = wKk + (size_t)m * no * nv_p;                   // [m][no][ldw]: W_m[i][(P, j)] = sum_b T_ib^P X'_mjb
+            for (int p0 = 0; p0 < nK; p0 += pc2) {
+                const int np = std::min(pc2, nK - p0);
+                const double *Tp = ctx->d_Tov + (size_t)p0 * no * nv_p;
+                GemmDesc d = gemm_desc(no, no, nv, Tp, nv_p, true, wXk, nv_p, true, wW, ldw);
+                d.nb1 = np; d.sA1 = (long long)no * nv_p; d.sB1 = 0; d.sC1 = no;
+                d.nb2 = m; d.sA2 = 0; d.sB2 = (long long)no * nv_p; d.sC2 = (long long)no * ldw;
+                RISP_CUDA_TRY(risp_dgemm(d, st)); ++launches;
+                GemmDesc e = gemm_desc(no, nv, np * no, wW, ldw, true, Tp, nv_p, false, wKk, nv_p, 1.0, p0 == 0 ? 0.0 : 1.0);
+                e.nb1 = m; e.sA1 = (long long)no * ldw; e.sB1 = 0; e.sC1 = (long long)no * nv_p;
+                RISP_CUDA_TRY(risp_dgemm(e, st)); ++launches;
+            }
+            RISP_CUDA_TRY(risp_axpy_window(wKk, -1.0, sigma, m, nocc, nvir, ctx->occK0, no, ctx->virK0, nv, nv_p, st)); ++launches;
+            RISP_CUDA_TRY(risp_axpy_window(wKk, 1.0, sigma_minus, m, nocc, nvir, ctx->occK0, no, ctx->virK0, nv, nv_p, st)); ++launches;
+        }
     } else {
         RISP_CUDA_TRY(cudaEventRecord(ev[6], st));
         RISP_CUDA_TRY(cudaEventRecord(ev[7], st));
@@ -386,6 +413,26 @@ extern "C" int risp_matvec_host(risp_ctx *ctx, int32_t m, const double *X_host, 
         RISP_CUDA_TRY(cudaMemcpyAsync(sigma_host + (size_t)m0 * vec, ctx->w_Sout, bytes, cudaMemcpyDeviceToHost, 0));
     }
     RISP_CUDA_TRY(cudaStreamSynchronize(0));
+    return RISP_OK;
+}
+
+// (A+B) X and (A-B) X of full TDDFT-risp (Eq. 2) for m trial vectors; same conventions as risp_matvec
+extern "C" int risp_matvec_tddft(risp_ctx *ctx, int32_t m, const double *X_dev, double *sigma_plus_dev, double *sigma_minus_dev, void *cuda_stream)
+{
+    if (!ctx) return RISP_EINVAL;
+    if (m <= 0 || !X_dev || !sigma_plus_dev || !sigma_minus_dev) { risp_set_error(ctx, "risp_matvec_tddft: need m >= 1 and non-NULL device pointers"); return RISP_EINVAL; }
+    const size_t vec = (size_t)ctx->nocc * ctx->nvir, bytes = (size_t)m * vec * sizeof(double);
+    const char *x = (const char *)X_dev, *a = (const char *)sigma_plus_dev, *b = (const char *)sigma_minus_dev;
+    if ((x < a + bytes && a < x + bytes) || (x < b + bytes && b < x + bytes) || (a < b + bytes && b < a + bytes)) {
+        risp_set_error(ctx, "risp_matvec_tddft: X, sigma_plus and sigma_minus overlap"); return RISP_EINVAL;
+    }
+    if (!(ctx->flags & RISP_FLAG_TDDFT)) { risp_set_error(ctx, "risp_matvec_tddft: the context was set up without RISP_FLAG_TDDFT"); return RISP_EINVAL; }
+    RISP_CUDA_TRY(cudaSetDevice(ctx->device));
+    int rc = risp_ensure_workspace(ctx, std::min<int>(m, RISP_MS));
+    if (rc) return rc;
+    for (int m0 = 0; m0 < m; m0 += RISP_MS)
+        if ((rc = risp_matvec_impl(ctx, std::min<int>(RISP_MS, m - m0), X_dev + (size_t)m0 * vec, sigma_plus_dev + (size_t)m0 * vec, (cudaStream_t)cuda_stream,
+                                   sigma_minus_dev + (size_t)m0 * vec))) return rc;
     return RISP_OK;
 }
 

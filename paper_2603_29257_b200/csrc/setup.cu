@@ -388,6 +388,10 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
             RISP_CUDA_TRY(scr.alloc(tmpI, nK * nK));
             RISP_CUDA_TRY(cudaMemcpy(tmpL, ctx->d_MK, nK * nK * sizeof(double), cudaMemcpyDeviceToDevice));
             RISP_CUDA_TRY(risp_cholesky_inverse(tmpL, tmpI, ctx->nauxK, &info, 0));
+            if (!info && (ctx->flags & RISP_FLAG_TDDFT)) {      // full TDDFT whitens (ov|J^|Q) with L_K^-1 (symmetric placement of the metric)
+                if ((rc = dalloc(ctx, ctx->d_LinvK, nK * nK))) return rc;
+                RISP_CUDA_TRY(cudaMemcpy(ctx->d_LinvK, tmpI, nK * nK * sizeof(double), cudaMemcpyDeviceToDevice));
+            }
             if (!info) {
                 // (P|Q)^-1 = L^-T L^-1
                 GemmDesc d = gemm_desc(ctx->nauxK, ctx->nauxK, ctx->nauxK, tmpI, ctx->nauxK, false, tmpI, ctx->nauxK, false, ctx->d_MKinv, ctx->nauxK);
@@ -423,6 +427,7 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
             size_t reserve = ((size_t)ctx->e_rows * RISP_MS + (size_t)ctx->total_chunks * ctx->ncenJ_pad * 4 * RISP_MS + 3 * (size_t)ctx->nauxJ * RISP_MS) * 8;
             if (!opt.hbm_budget_bytes) reserve += 2 * (size_t)ctx->max_batch * dimb;
             if (ctx->flags & RISP_FLAG_KEEP_STAGES) reserve += (size_t)ctx->max_batch * dimb;
+            if (ctx->flags & RISP_FLAG_TDDFT) reserve += (size_t)nK * no * nv_p * 8 + (!opt.hbm_budget_bytes ? (size_t)ctx->max_batch * dimb : 0);
             size_t left = ctx->hbm_budget > ctx->setup_bytes + reserve ? ctx->hbm_budget - ctx->setup_bytes - reserve : 0;
             // work space if everything had to be streamed (upper bound of the staging need), then the slices
             MatvecPlan tmp;
@@ -449,6 +454,12 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
         RISP_CUDA_TRY(scr.alloc(F, (size_t)max_fn * sq));
         RISP_CUDA_TRY(scr.alloc(Pk, (size_t)max_fn * std::max(tri_o, tri_v)));
         RISP_CUDA_TRY(scr.alloc(d_cenRun, (size_t)ctx->ncenK));
+        double *Fov = nullptr;
+        if (ctx->flags & RISP_FLAG_TDDFT) {      // T_ia^P': kept whole in HBM; needed by the (ib|ja) term of Eq. 2 only
+            if ((rc = dalloc(ctx, ctx->d_Tov, (size_t)nK * no * nv_p))) { risp_set_error(ctx, "risp_setup: the (ia|P) tensor of full TDDFT does not fit in HBM"); return rc; }
+            RISP_CUDA_TRY(cudaMemset(ctx->d_Tov, 0, (size_t)nK * no * nv_p * sizeof(double)));
+            RISP_CUDA_TRY(scr.alloc(Fov, (size_t)max_fn * no * nv_p));
+        }
         // window blocks of C with even leading dimensions and aligned bases
         RISP_CUDA_TRY(scr.alloc(CoK, (size_t)nao * no_p));
         RISP_CUDA_TRY(scr.alloc(CvK, (size_t)nao * nv_p));
@@ -508,6 +519,14 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
                     for (int j = 0; j < nf; ++j)
                         RISP_CUDA_TRY(risp_pack_sym(F + (size_t)j * n * n_p, (long long)n * n_p, n_p, n, 1, bp_slice(fn_of[j]), tri, 0));
                 } else {
+                    if (ctx->d_Tov) {      // (ia|J^|P) = C_o'^T [(mu nu|P) C_v'] from the half-transformed H of this pass
+                        GemmDesc d3 = gemm_desc(no, nv, nao, CoK, no_p, false, H, nv_p, false, Fov, nv_p);
+                        d3.nb1 = nf; d3.sB1 = (long long)nao * nv_p; d3.sC1 = (long long)no * nv_p;
+                        RISP_CUDA_TRY(risp_dgemm(d3, 0));
+                        for (int j = 0; j < nf; ++j)
+                            RISP_CUDA_TRY(cudaMemcpy2DAsync(ctx->d_Tov + (size_t)fn_of[j] * no * nv_p, (size_t)nv_p * 8, Fov + (size_t)j * no * nv_p, (size_t)nv_p * 8,
+                                                            (size_t)nv * 8, no, cudaMemcpyDeviceToDevice, 0));
+                    }
                     RISP_CUDA_TRY(risp_pack_sym(F, (long long)n * n_p, n_p, n, nf, Pk, tri, 0));
                     for (int j = 0; j < nf; ++j) {
                         const int f = fn_of[j];
@@ -549,6 +568,20 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
             }
         }
         RISP_CUDA_TRY(cudaDeviceSynchronize());
+        if (ctx->d_Tov) {
+            // T^P <- sum_Q L_K^-1[P][Q] (ov|J^|Q): [nK x nK] x [nK x (o' v')] in column panels, in place
+            const long long cols = (long long)no * nv_p;
+            const long long w = std::min<long long>(cols, std::max<long long>(2, (((long long)1 << 30) / ((long long)nK * 8)) & ~1LL));
+            double *tmpw = nullptr;
+            RISP_CUDA_TRY(scr.alloc(tmpw, (size_t)nK * w));
+            for (long long col = 0; col < cols; col += w) {
+                const int wc = (int)std::min<long long>(w, cols - col);
+                GemmDesc d7 = gemm_desc(nK, wc, nK, ctx->d_LinvK, nK, true, ctx->d_Tov + col, cols, false, tmpw, w);
+                RISP_CUDA_TRY(risp_dgemm(d7, 0));
+                RISP_CUDA_TRY(cudaMemcpy2DAsync(ctx->d_Tov + col, (size_t)cols * 8, tmpw, (size_t)w * 8, (size_t)wc * 8, nK, cudaMemcpyDeviceToDevice, 0));
+            }
+            RISP_CUDA_TRY(cudaDeviceSynchronize());
+        }
     }
     RISP_CUDA_TRY(cudaDeviceSynchronize());
     RISP_CUDA_TRY(cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking));

@@ -206,55 +206,16 @@ struct Solver {
 
 #define KERNEL_CHECK() RISP_CUDA_TRY(cudaGetLastError())
 
-// out[na][nb] = sum_x A[i][x] B[j][x]: split-K batched DMMA GEMM + fixed-order reduction.  The smaller operand goes to the M side
-// (16-row tiles exist, the N tile is always 128 wide); the product is HBM-bound: it reads (na + nb) dim doubles.
-// Needs min(na, nb) <= 64 and max(na, nb) <= 128 (scratch size); callers chunk accordingly.
+// out[na][nb] = sum_x A[i][x] B[j][x]; needs min(na, nb) <= 64 and max(na, nb) <= 128 (scratch size); callers chunk accordingly
 int gram(Solver &S, const double *A, int na, const double *B, int nb, std::vector<double> &out)
 {
-    risp_ctx *ctx = S.ctx;
-    const bool swap = na > nb;
-    const double *P = swap ? B : A, *Q = swap ? A : B;
-    const int np = swap ? nb : na, nq = swap ? na : nb;
-    if (np > 64 || nq > 128) { risp_set_error(ctx, "risp_tda_solve: internal Gram block too large"); return RISP_EINVAL; }
-    const long long slice = S.slice;
-    int nfull = (int)(S.dim / slice);
-    long long tail = S.dim - (long long)nfull * slice;
-    int nz = nfull + (tail ? 1 : 0);
-    if (nfull) {
-        GemmDesc d = gemm_desc(np, nq, (int)slice, P, S.dim, true, Q, S.dim, true, S.dPart, nq);
-        d.nb1 = nfull; d.sA1 = slice; d.sB1 = slice; d.sC1 = (long long)np * nq;
-        RISP_CUDA_TRY(risp_dgemm(d, S.st));
-    }
-    if (tail) {
-        GemmDesc d = gemm_desc(np, nq, (int)tail, P + (long long)nfull * slice, S.dim, true, Q + (long long)nfull * slice, S.dim, true,
-                               S.dPart + (long long)nfull * np * nq, nq);
-        RISP_CUDA_TRY(risp_dgemm(d, S.st));
-    }
-    reduce_partials_kernel<<<(np * nq + 127) / 128, 128, 0, S.st>>>(S.dPart, nz, np * nq, S.dSmall);
-    KERNEL_CHECK();
-    out.resize((size_t)na * nb);
-    if (!swap) {
-        RISP_CUDA_TRY(cudaMemcpyAsync(out.data(), S.dSmall, (size_t)na * nb * 8, cudaMemcpyDeviceToHost, S.st));
-        RISP_CUDA_TRY(cudaStreamSynchronize(S.st));
-    } else {
-        S.tmp.resize((size_t)na * nb);
-        RISP_CUDA_TRY(cudaMemcpyAsync(S.tmp.data(), S.dSmall, (size_t)na * nb * 8, cudaMemcpyDeviceToHost, S.st));
-        RISP_CUDA_TRY(cudaStreamSynchronize(S.st));
-        for (int i = 0; i < na; ++i)
-            for (int j = 0; j < nb; ++j) out[(size_t)i * nb + j] = S.tmp[(size_t)j * na + i];
-    }
-    return RISP_OK;
+    return risp_rows_gram(S.ctx, A, na, B, nb, S.dim, S.slice, S.dPart, S.dSmall, out, S.st);
 }
 
 // C[nc][dim] = alpha * coef[nc][na] * A[na][dim] + beta * C
 int lincomb(Solver &S, const std::vector<double> &coef, int nc, int na, const double *A, double *C, double alpha, double beta)
 {
-    risp_ctx *ctx = S.ctx;
-    RISP_CUDA_TRY(cudaMemcpyAsync(S.dCoef, coef.data(), (size_t)nc * na * 8, cudaMemcpyHostToDevice, S.st));
-    GemmDesc d = gemm_desc(nc, (int)std::min<long long>(S.dim, 1 << 30), na, S.dCoef, na, true, A, S.dim, false, C, S.dim, alpha, beta);
-    RISP_CUDA_TRY(risp_dgemm(d, S.st));
-    RISP_CUDA_TRY(cudaStreamSynchronize(S.st));   // coef is a host temporary
-    return RISP_OK;
+    return risp_rows_lincomb(S.ctx, coef.data(), nc, na, A, C, S.dim, alpha, beta, S.dCoef, S.st);
 }
 
 // pass over subspace vectors [0, n): the first ncache come from the device cache (chunks of up to 128), the others are streamed
@@ -460,6 +421,56 @@ int orthonormalise(Solver &S, double *T, double *tmp, int &nb)
 }
 
 }  // namespace
+
+// ---- dense row-block products shared by the TDA and the TDDFT solver (declared in ctx.h)
+// out[na][nb] = sum_x A[i][x] B[j][x]: split-K batched DMMA GEMM + fixed-order reduction.  The smaller operand goes to the M side
+// (16-row tiles exist, the N tile is always 128 wide); the product is HBM-bound: it reads (na + nb) dim doubles.
+// dPart: [dim / slice + 2][128 * 64] doubles, dSmall: [128 * 64].
+int risp_rows_gram(risp_ctx *ctx, const double *A, int na, const double *B, int nb, long long dim, long long slice, double *dPart, double *dSmall,
+                   std::vector<double> &out, cudaStream_t st)
+{
+    const bool swap = na > nb;
+    const double *P = swap ? B : A, *Q = swap ? A : B;
+    const int np = swap ? nb : na, nq = swap ? na : nb;
+    if (np > 64 || nq > 128) { risp_set_error(ctx, "risp solver: internal Gram block too large"); return RISP_EINVAL; }
+    int nfull = (int)(dim / slice);
+    long long tail = dim - (long long)nfull * slice;
+    int nz = nfull + (tail ? 1 : 0);
+    if (nfull) {
+        GemmDesc d = gemm_desc(np, nq, (int)slice, P, dim, true, Q, dim, true, dPart, nq);
+        d.nb1 = nfull; d.sA1 = slice; d.sB1 = slice; d.sC1 = (long long)np * nq;
+        RISP_CUDA_TRY(risp_dgemm(d, st));
+    }
+    if (tail) {
+        GemmDesc d = gemm_desc(np, nq, (int)tail, P + (long long)nfull * slice, dim, true, Q + (long long)nfull * slice, dim, true,
+                               dPart + (long long)nfull * np * nq, nq);
+        RISP_CUDA_TRY(risp_dgemm(d, st));
+    }
+    reduce_partials_kernel<<<(np * nq + 127) / 128, 128, 0, st>>>(dPart, nz, np * nq, dSmall);
+    RISP_CUDA_TRY(cudaGetLastError());
+    out.resize((size_t)na * nb);
+    if (!swap) {
+        RISP_CUDA_TRY(cudaMemcpyAsync(out.data(), dSmall, (size_t)na * nb * 8, cudaMemcpyDeviceToHost, st));
+        RISP_CUDA_TRY(cudaStreamSynchronize(st));
+    } else {
+        std::vector<double> tmp((size_t)na * nb);
+        RISP_CUDA_TRY(cudaMemcpyAsync(tmp.data(), dSmall, (size_t)na * nb * 8, cudaMemcpyDeviceToHost, st));
+        RISP_CUDA_TRY(cudaStreamSynchronize(st));
+        for (int i = 0; i < na; ++i)
+            for (int j = 0; j < nb; ++j) out[(size_t)i * nb + j] = tmp[(size_t)j * na + i];
+    }
+    return RISP_OK;
+}
+
+int risp_rows_lincomb(risp_ctx *ctx, const double *coef_host, int nc, int na, const double *A, double *C, long long dim, double alpha, double beta,
+                      double *dCoef, cudaStream_t st)
+{
+    RISP_CUDA_TRY(cudaMemcpyAsync(dCoef, coef_host, (size_t)nc * na * 8, cudaMemcpyHostToDevice, st));
+    GemmDesc d = gemm_desc(nc, (int)std::min<long long>(dim, 1 << 30), na, dCoef, na, true, A, dim, false, C, dim, alpha, beta);
+    RISP_CUDA_TRY(risp_dgemm(d, st));
+    RISP_CUDA_TRY(cudaStreamSynchronize(st));   // coef is a host temporary
+    return RISP_OK;
+}
 
 extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_options *opt_in, double *omega_out, double *X_out,
                               risp_solve_info *info)
