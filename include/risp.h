@@ -84,6 +84,9 @@ typedef struct {
     int32_t max_batch;          /* largest m the caller will pass to risp_matvec (0 -> 32); HBM is reserved for its X, sigma
                                    and work space before the K tensors are placed */
     int32_t reserved;
+    int32_t shard_rank, shard_count; /* P-sharded sigma-build over several GPUs: shard_count > 1 makes this context
+                                   hold every shard_count-th kept shell pair and the K-tensor slices of every shard_count-th
+                                   auxiliary centre, all in HBM; see risp_matvec_shard_begin / _end.  0 or 1: not sharded */
 } risp_options;
 
 #define RISP_FLAG_KEEP_STAGES 1   /* keep J_mia of the last risp_matvec for risp_get_stage (costs one more [m][nocc][nvir] buffer) */
@@ -171,6 +174,18 @@ int risp_matvec(risp_ctx *ctx, int32_t m, const double *X_dev, double *sigma_dev
  * (reading G25: Eq. 2a's "2(ia|jb)" is read as 4(ia|jb), consistent with Eq. 10 and Eq. 2b).  Needs RISP_FLAG_TDDFT at
  * setup.  All three buffers DEVICE [m][nocc][nvir], pairwise disjoint; asynchronous on cuda_stream. */
 int risp_matvec_tddft(risp_ctx *ctx, int32_t m, const double *X_dev, double *sigma_plus_dev, double *sigma_minus_dev, void *cuda_stream);
+
+/* P-sharded sigma-build, one context per GPU (set up with shard_rank / shard_count; X replicated on every rank):
+ *     risp_matvec_shard_begin   D (Eq. 12) and pass 1 (Eq. 14) over this rank's shell pairs -> R_partial_dev [nauxJ][32] (DEVICE,
+ *                               trial vector fastest, zero beyond m);
+ *     -- the caller sums R_partial over the ranks (one all-reduce of nauxJ * 32 doubles, < 2 MB) --
+ *     risp_matvec_shard_end     R~ (Eq. 15), pass 2 (Eq. 16) and the back-transform (Eq. 17) on this rank's pairs, Eq. 22-23 over this
+ *                               rank's K slices, the diagonal on rank 0 -> sigma_partial_dev [m][nocc][nvir];
+ *     -- the caller sums sigma_partial over the ranks (all-reduce or reduce-scatter of m * nocc * nvir doubles) --
+ * m <= 32 per call.  Both calls are asynchronous on cuda_stream; the sum of the partial results equals risp_matvec of an
+ * unsharded context up to the order of the floating-point sums. */
+int risp_matvec_shard_begin(risp_ctx *ctx, int32_t m, const double *X_dev, double *R_partial_dev, void *cuda_stream);
+int risp_matvec_shard_end(risp_ctx *ctx, int32_t m, const double *X_dev, const double *R_dev, double *sigma_partial_dev, void *cuda_stream);
 
 /* Same with HOST buffers: copies X in, runs risp_matvec, copies sigma out, synchronises. */
 int risp_matvec_host(risp_ctx *ctx, int32_t m, const double *X_host, double *sigma_host);

@@ -10,7 +10,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
 EXPORTED_SYMBOLS = ["risp_setup", "risp_matvec", "risp_matvec_host", "risp_tda_solve", "risp_destroy", "risp_last_error",
-                    "risp_get_dims", "risp_get_timings", "risp_eri3c_shell", "risp_get_stage", "risp_transition_properties", "risp_matvec_tddft", "risp_tddft_solve"]
+                    "risp_get_dims", "risp_get_timings", "risp_eri3c_shell", "risp_get_stage", "risp_transition_properties", "risp_matvec_tddft", "risp_tddft_solve", "risp_matvec_shard_begin", "risp_matvec_shard_end"]
 
 RISP_MAX_ROOTS = 64
 FLAG_KEEP_STAGES, FLAG_SPILL_HALF, FLAG_SMALL_KBUILD, FLAG_TDDFT = 1, 2, 4, 8
@@ -39,7 +39,8 @@ class _System(C.Structure):
 
 class _Options(C.Structure):
     _fields_ = [("screen_tol", C.c_double), ("hbm_budget_bytes", C.c_size_t), ("host_budget_bytes", C.c_size_t),
-                ("device", C.c_int32), ("flags", C.c_int32), ("max_batch", C.c_int32), ("reserved", C.c_int32)]
+                ("device", C.c_int32), ("flags", C.c_int32), ("max_batch", C.c_int32), ("reserved", C.c_int32),
+                ("shard_rank", C.c_int32), ("shard_count", C.c_int32)]
 
 
 class _SolveOptions(C.Structure):
@@ -93,6 +94,8 @@ def load_library():
     lib.risp_get_timings.argtypes = [vp, C.POINTER(_Timings)]
     lib.risp_eri3c_shell.argtypes = [vp, i32, i32, i32, i32, vp]
     lib.risp_get_stage.argtypes = [vp, i32, vp, i64, vp]
+    lib.risp_matvec_shard_begin.argtypes = [vp, i32, vp, vp, vp]
+    lib.risp_matvec_shard_end.argtypes = [vp, i32, vp, vp, vp, vp]
     lib.risp_matvec_tddft.argtypes = [vp, i32, vp, vp, vp, vp]
     lib.risp_tddft_solve.argtypes = [vp, i32, C.POINTER(_SolveOptions), C.POINTER(dbl), vp, vp, C.POINTER(_SolveInfo)]
     lib.risp_transition_properties.argtypes = [vp, i32, vp, vp, vp, dbl, vp, vp, vp, vp]
@@ -119,7 +122,7 @@ class RispContext:
     """Owns one `risp_ctx`.  X / sigma are torch CUDA tensors (device pointers go straight through the ABI)."""
 
     def __init__(self, sys: dict, screen_tol: float = 0.0, hbm_budget_bytes: int = 0, host_budget_bytes: int = 0, device: int = 0,
-                 flags: int = 0, max_batch: int = 0):
+                 flags: int = 0, max_batch: int = 0, shard_rank: int = 0, shard_count: int = 0):
         self.lib = load_library()
         keep = {}
 
@@ -139,7 +142,7 @@ class RispContext:
         s.nao, s.nocc, s.nvir = int(sys["nao"]), int(sys["nocc"]), int(sys["nvir"])
         s.C = arr("C", np.float64); s.eps = arr("eps", np.float64)
         s.alpha, s.beta, s.omega, s.cutoff_ev = float(sys["alpha"]), float(sys["beta"]), float(sys["omega"]), float(sys["cutoff_ev"])
-        o = _Options(float(screen_tol), int(hbm_budget_bytes), int(host_budget_bytes), int(device), int(flags), int(max_batch), 0)
+        o = _Options(float(screen_tol), int(hbm_budget_bytes), int(host_budget_bytes), int(device), int(flags), int(max_batch), 0, int(shard_rank), int(shard_count))
         self.handle = C.c_void_p()
         self.nocc, self.nvir, self.nao = s.nocc, s.nvir, s.nao
         self.device = device
@@ -205,6 +208,23 @@ class RispContext:
         d = _struct_dict(info)
         d["resid"] = d["resid"][:nroots]
         return omega, X, d
+
+    def matvec_shard_begin(self, X, R=None, stream=None):
+        """first half of a P-sharded sigma-build: this rank's partial R_mQ as a [nauxJ][32] device tensor"""
+        import torch
+        if R is None:
+            R = torch.empty((self.dims()["nauxJ"], 32), dtype=torch.float64, device=X.device)
+        st = torch.cuda.current_stream(X.device).cuda_stream if stream is None else stream
+        self._check(self.lib.risp_matvec_shard_begin(self.handle, X.shape[0], X.data_ptr(), R.data_ptr(), st))
+        return R
+
+    def matvec_shard_end(self, X, R, sigma=None, stream=None):
+        import torch
+        if sigma is None:
+            sigma = torch.empty_like(X)
+        st = torch.cuda.current_stream(X.device).cuda_stream if stream is None else stream
+        self._check(self.lib.risp_matvec_shard_end(self.handle, X.shape[0], X.data_ptr(), R.data_ptr(), sigma.data_ptr(), st))
+        return sigma
 
     def matvec_tddft(self, X, stream=None):
         """risp_matvec_tddft: ((A+B) X, (A-B) X) for the device vectors X[m][nocc][nvir]."""

@@ -190,7 +190,7 @@ extern "C" int risp_get_stage(risp_ctx *ctx, int32_t which, const int64_t *sel, 
         return RISP_OK;
     case RISP_STAGE_METRIC_K:
         if (!ctx->has_K) { risp_set_error(ctx, "risp_get_stage: no K metric"); return RISP_EINVAL; }
-        RISP_CUDA_TRY(cudaMemcpy(out, ctx->d_MK, (size_t)ctx->nauxK * ctx->nauxK * 8, cudaMemcpyDeviceToHost));
+        RISP_CUDA_TRY(cudaMemcpy(out, ctx->d_MK, (size_t)ctx->nauxK_global * ctx->nauxK_global * 8, cudaMemcpyDeviceToHost));
         return RISP_OK;
     case RISP_STAGE_U: {
         // rebuilt from the e0-space U-bar that the last matvec left in place (pass 2 output)

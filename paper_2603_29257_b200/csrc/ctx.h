@@ -61,6 +61,7 @@ struct risp_ctx {
     int total_chunks = 0;
     size_t hbm_budget = 0, host_budget = 0;
     int max_batch = RISP_MS, flags = 0;
+    int shard_rank = 0, shard_count = 1, nauxK_global = 0;      // P-sharded sigma-build: this context holds 1 / shard_count of the pairs and K slices
     // ---- host copies needed after setup (getters, solver)
     std::vector<double> h_xyz, h_prim_exp, h_prim_d /* coef*radial norm, shell-normalised */, h_eps;
     std::vector<int> h_shl_atom, h_shl_l, h_shl_nprim, h_shl_poff, h_shl_ao;
@@ -150,7 +151,9 @@ cudaError_t risp_expand_sym(const double *packed, long long tri, int n, int np, 
 int risp_ensure_workspace(risp_ctx *ctx, int m);
 size_t risp_plan_workspace(const risp_ctx *ctx, int m, size_t avail, MatvecPlan &plan, bool spilled);
 // sigma = A X (TDA).  With sigma_minus != nullptr (full TDDFT, needs d_Tov): sigma = (A+B) X, sigma_minus = (A-B) X (Eq. 2).
-int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaStream_t st, double *sigma_minus = nullptr);
+// phase 0: the whole sigma-build.  Sharded contexts: phase 1 = up to the partial R_mQ of pass 1 (Eq. 14), phase 2 = from the metric
+// solve on (the caller has summed R over the shards in between).
+int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaStream_t st, double *sigma_minus = nullptr, int phase = 0);
 int risp_build_pair(risp_ctx *ctx, int shA, int shB, risp_eri::ShellPair &sp, std::vector<risp_eri::PrimPair> &pp, double prim_tol);
 void risp_free_workspace(risp_ctx *ctx);
 int risp_rows_gram(risp_ctx *ctx, const double *A, int na, const double *B, int nb, long long dim, long long slice, double *dPart, double *dSmall,

@@ -156,7 +156,7 @@ static int join_classes(risp_ctx *ctx, cudaStream_t st)
     return RISP_OK;
 }
 
-int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaStream_t st, double *sigma_minus)
+int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaStream_t st, double *sigma_minus, int phase)
 {
     const bool tddft = sigma_minus != nullptr;
     if (tddft && ctx->has_K && !ctx->d_Tov) { risp_set_error(ctx, "risp_matvec_tddft: the context was set up without RISP_FLAG_TDDFT"); return RISP_EINVAL; }
@@ -168,13 +168,16 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
     const bool dense = npanel == 1;
     int launches = 0, rc;
     cudaEvent_t *ev = ctx->ev;
-    RISP_CUDA_TRY(cudaEventRecord(ev[0], st));
-    // ---------------- diagonal (Eq. 10)
-    RISP_CUDA_TRY(risp_diag_sigma(X, ctx->d_eps, sigma, m, nocc, nvir, st)); ++launches;
-    if (tddft) { RISP_CUDA_TRY(risp_diag_sigma(X, ctx->d_eps, sigma_minus, m, nocc, nvir, st)); ++launches; }
-    // J-phase views of the arena
-    double *wY = ctx->w_arena;                                   // [mj][nocc][ldao]
+    double *wY = ctx->w_arena;                                   // [mj][nocc][ldao]   (J-phase views of the arena)
     double *wD = wY + (size_t)pl.mj * nocc * ldao;               // [mj][prow][ldao]
+    if (phase == 2) goto after_pass1;
+    RISP_CUDA_TRY(cudaEventRecord(ev[0], st));
+    if (phase == 1) goto density;
+    // ---------------- diagonal (Eq. 10); in a sharded sigma-build rank 0 carries it
+    if (ctx->shard_rank == 0) { RISP_CUDA_TRY(risp_diag_sigma(X, ctx->d_eps, sigma, m, nocc, nvir, st)); ++launches; }
+    else RISP_CUDA_TRY(cudaMemsetAsync(sigma, 0, (size_t)m * nocc * nvir * sizeof(double), st));
+    if (tddft) { RISP_CUDA_TRY(risp_diag_sigma(X, ctx->d_eps, sigma_minus, m, nocc, nvir, st)); ++launches; }
+density:
     // ---------------- J: AO transition density (Eq. 12) on the kept pairs, in e0 space
     if (!dense) RISP_CUDA_TRY(cudaMemsetAsync(ctx->w_dbar, 0, (size_t)ctx->e_rows * RISP_MS * sizeof(double), st));   // panels accumulate
     for (int l0 = 0; l0 < m; l0 += pl.mj) {
@@ -214,6 +217,12 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
     if ((rc = join_classes(ctx, st))) return rc;
     RISP_CUDA_TRY(risp_j_reduce_R(ctx->w_Rpart, ctx->total_chunks, ctx->d_cenJ, ctx->ncenJ, ctx->ncenJ_pad, ctx->w_R, st)); ++launches;
     RISP_CUDA_TRY(cudaEventRecord(ev[2], st));
+    if (phase == 1) { ctx->last_m = m; return RISP_OK; }
+after_pass1:
+    if (phase == 2) {      // the diagonal of the second half of a sharded sigma-build
+        if (ctx->shard_rank == 0) { RISP_CUDA_TRY(risp_diag_sigma(X, ctx->d_eps, sigma, m, nocc, nvir, st)); ++launches; }
+        else RISP_CUDA_TRY(cudaMemsetAsync(sigma, 0, (size_t)m * nocc * nvir * sizeof(double), st));
+    }
     // ---------------- R~ = (P|Q)^-1 R = L^-T (L^-1 R)  (Eq. 15)
     RISP_CUDA_TRY(risp_metric_solve32(ctx->d_LinvJ, nJ, ctx->w_R, ctx->w_Rtmp, ctx->w_Rt, st)); launches += 2;
     RISP_CUDA_TRY(risp_rt_by_centre(ctx->w_Rt, ctx->d_cenJ, ctx->ncenJ, ctx->w_RtC, st)); ++launches;
@@ -414,6 +423,32 @@ extern "C" int risp_matvec_host(risp_ctx *ctx, int32_t m, const double *X_host, 
     }
     RISP_CUDA_TRY(cudaStreamSynchronize(0));
     return RISP_OK;
+}
+
+// P-sharded sigma-build: first half -- this rank's pairs contribute to R_mQ (Eq. 14)
+extern "C" int risp_matvec_shard_begin(risp_ctx *ctx, int32_t m, const double *X_dev, double *R_partial_dev, void *cuda_stream)
+{
+    if (!ctx) return RISP_EINVAL;
+    if (m <= 0 || m > RISP_MS || !X_dev || !R_partial_dev) { risp_set_error(ctx, "risp_matvec_shard_begin: need 1 <= m <= 32 and non-NULL device pointers"); return RISP_EINVAL; }
+    RISP_CUDA_TRY(cudaSetDevice(ctx->device));
+    int rc = risp_ensure_workspace(ctx, m);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((rc = risp_matvec_impl(ctx, m, X_dev, nullptr, st, nullptr, 1))) return rc;
+    RISP_CUDA_TRY(cudaMemcpyAsync(R_partial_dev, ctx->w_R, (size_t)ctx->nauxJ * RISP_MS * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    return RISP_OK;
+}
+
+// second half: R_dev holds the sum of all shards' partial R; returns this rank's share of sigma (rank 0 carries the diagonal)
+extern "C" int risp_matvec_shard_end(risp_ctx *ctx, int32_t m, const double *X_dev, const double *R_dev, double *sigma_partial_dev, void *cuda_stream)
+{
+    if (!ctx) return RISP_EINVAL;
+    if (m <= 0 || m > RISP_MS || !X_dev || !R_dev || !sigma_partial_dev) { risp_set_error(ctx, "risp_matvec_shard_end: need 1 <= m <= 32 and non-NULL device pointers"); return RISP_EINVAL; }
+    if (m != ctx->last_m || m > ctx->m_cap) { risp_set_error(ctx, "risp_matvec_shard_end: no matching risp_matvec_shard_begin"); return RISP_EINVAL; }
+    RISP_CUDA_TRY(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    RISP_CUDA_TRY(cudaMemcpyAsync(ctx->w_R, R_dev, (size_t)ctx->nauxJ * RISP_MS * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    return risp_matvec_impl(ctx, m, X_dev, sigma_partial_dev, st, nullptr, 2);
 }
 
 // (A+B) X and (A-B) X of full TDDFT-risp (Eq. 2) for m trial vectors; same conventions as risp_matvec

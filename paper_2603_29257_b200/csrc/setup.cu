@@ -255,6 +255,7 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
         if (sys->aux_in_K[s]) { ctx->h_aux_fnK[s] = ctx->nauxK; ctx->nauxK += 2 * sys->aux_l[s] + 1; }
     }
     if (ctx->nauxJ == 0) return bad("empty auxiliary basis");
+    ctx->nauxK_global = ctx->nauxK;
 
     // ---------------------------------------------------------------- a2: window (reading G6: absolute energies)
     {
@@ -276,6 +277,10 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
 
     // ---------------------------------------------------------------- device constants
     ctx->flags = opt.flags;
+    ctx->shard_count = opt.shard_count > 1 ? opt.shard_count : 1;
+    ctx->shard_rank = ctx->shard_count > 1 ? opt.shard_rank : 0;
+    if (ctx->shard_rank < 0 || ctx->shard_rank >= ctx->shard_count) return bad("shard_rank outside [0, shard_count)");
+    if (ctx->shard_count > 1 && (opt.flags & (RISP_FLAG_TDDFT | RISP_FLAG_SPILL_HALF))) return bad("a sharded context supports neither RISP_FLAG_TDDFT nor host-spilled K slices");
     ctx->max_batch = opt.max_batch > 0 ? std::min(opt.max_batch, RISP_MS) : RISP_MS;
     auto even = [](int n) { return (n + 1) & ~1; };
     ctx->ldao = even(ctx->nao); ctx->ldocc = even(ctx->nocc); ctx->ldvir = even(ctx->nvir);
@@ -311,6 +316,7 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
         std::vector<ShellPair> pairs[6];
         std::vector<PrimPair> prims;
         ctx->n_shell_pairs = (long long)sys->nshl * (sys->nshl + 1) / 2;
+        long long kept_seen = 0;
         for (int sa = 0; sa < sys->nshl; ++sa)
             for (int sb = 0; sb <= sa; ++sb) {
                 int A = sa, B = sb;
@@ -319,6 +325,9 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
                 size_t mark = prims.size();
                 double est = pair_estimate_and_build(ctx, A, B, sp, prims, tau < 0 ? -1.0 : tau * 1e-3, vmax);
                 if ((tau >= 0 && est < tau) || sp.npp == 0) { prims.resize(mark); continue; }
+                // P-sharded sigma-build: the kept pairs are dealt round robin; every rank runs both integral
+                // passes and the pair-sparse halves of the J transforms on its own pairs only
+                if (ctx->shard_count > 1 && (kept_seen++ % ctx->shard_count) != ctx->shard_rank) { prims.resize(mark); continue; }
                 pairs[class_index(sys->shl_l[A], sys->shl_l[B])].push_back(sp);
                 ctx->h_kept_pairs.push_back(A); ctx->h_kept_pairs.push_back(B);
                 ctx->n_ao_pairs_kept += (A == B) ? (long long)(2 * sys->shl_l[A] + 1) * (2 * sys->shl_l[A] + 2) / 2
@@ -437,6 +446,26 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
             left -= std::min(left, ws);
             ctx->nK_dev = (int)std::min<size_t>((size_t)nK, left / slice);
             if (ctx->flags & RISP_FLAG_SPILL_HALF) ctx->nK_dev = std::min(ctx->nK_dev, nK / 2);
+            if (ctx->shard_count > 1) {
+                // sharded: this rank keeps the slices of its own aux centres only, all of them in HBM; every (ij|Q) is needed while
+                // the metric is applied (Eq. 20 mixes all Q), so T_ij is built whole and cut down afterwards
+                int nloc = 0;
+                for (int c = 0; c < ctx->ncenK; ++c)
+                    if (c % ctx->shard_count == ctx->shard_rank) nloc += (cenK[c].qs >= 0 ? 1 : 0) + (cenK[c].qp >= 0 ? 3 : 0);
+                if ((size_t)nK * tri_o * 8 + (size_t)nloc * tri_v * 8 > left) {
+                    risp_set_error(ctx, "risp_setup: a sharded context keeps its K slices in HBM; the budget is too small (use more shards)");
+                    return RISP_ENOMEM;
+                }
+                ctx->nK_dev = nK;
+            }
+        }
+        const bool sharded = ctx->shard_count > 1;
+        std::vector<int> loc_of(nK, -1);                 // sharded: index of a K function among this rank's slices, or -1
+        int nK_loc = 0;
+        for (int c = 0; c < ctx->ncenK; ++c) {
+            if (sharded && c % ctx->shard_count != ctx->shard_rank) continue;
+            if (cenK[c].qs >= 0) loc_of[cenK[c].qs] = nK_loc++;
+            if (cenK[c].qp >= 0) for (int t = 0; t < 3; ++t) loc_of[cenK[c].qp + t] = nK_loc++;
         }
         const int nK_host = nK - ctx->nK_dev;
         // ---- scratch for a chunk of aux functions: G[f][nao][ldao], H[f][nao][max(no_p,nv_p)], full B / T[f][n][n_p], packed
@@ -479,7 +508,7 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
         }
         OpParams opK{sys->alpha, sys->beta, sys->omega * sys->omega};
         for (int pass = 0; pass < 2; ++pass) {          // pass 0: occupied window -> BP ; pass 1: virtual window -> T_ab
-            if (pass == 1 && ctx->nK_dev > 0) { if ((rc = dalloc(ctx, ctx->d_TabP, (size_t)ctx->nK_dev * tri_v))) return rc; }
+            if (pass == 1 && ctx->nK_dev > 0) { if ((rc = dalloc(ctx, ctx->d_TabP, (size_t)(sharded ? nK_loc : ctx->nK_dev) * tri_v))) return rc; }
             const int n = pass == 0 ? no : nv, n_p = pass == 0 ? no_p : nv_p;
             const long long tri = pass == 0 ? tri_o : tri_v;
             const double *Cw = pass == 0 ? CoK : CvK;
@@ -492,6 +521,7 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
                 std::vector<int> fn_of;
                 int c1 = c0;
                 while (c1 < ctx->ncenK) {
+                    if (pass == 1 && sharded && c1 % ctx->shard_count != ctx->shard_rank) { ++c1; continue; }      // (ab|P): own centres only
                     const int add = (cenK[c1].qs >= 0 ? 1 : 0) + (cenK[c1].qp >= 0 ? 3 : 0);
                     if (c1 > c0 && (int)fn_of.size() + add > max_fn) break;
                     AuxCentre cc = cenK[c1];
@@ -501,6 +531,7 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
                     ++c1;
                 }
                 const int nf = (int)fn_of.size();
+                if (nf == 0) { c0 = c1; continue; }
                 RISP_CUDA_TRY(cudaMemcpy(d_cenRun, run.data(), run.size() * sizeof(AuxCentre), cudaMemcpyHostToDevice));
                 RISP_CUDA_TRY(cudaMemsetAsync(G, 0, (size_t)nf * nao * ldao * sizeof(double), 0));
                 for (int c = 0; c < 6; ++c) {
@@ -529,7 +560,7 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
                     }
                     RISP_CUDA_TRY(risp_pack_sym(F, (long long)n * n_p, n_p, n, nf, Pk, tri, 0));
                     for (int j = 0; j < nf; ++j) {
-                        const int f = fn_of[j];
+                        const int f = sharded ? loc_of[fn_of[j]] : fn_of[j];
                         const double *src = Pk + (size_t)j * tri;
                         if (f < ctx->nK_dev) RISP_CUDA_TRY(cudaMemcpyAsync(ctx->d_TabP + (size_t)f * tri, src, (size_t)tri * 8, cudaMemcpyDeviceToDevice, 0));
                         else RISP_CUDA_TRY(cudaMemcpyAsync(ctx->h_TabP + (size_t)(f - ctx->nK_dev) * tri, src, (size_t)tri * 8, cudaMemcpyDeviceToHost, 0));
@@ -568,6 +599,18 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
             }
         }
         RISP_CUDA_TRY(cudaDeviceSynchronize());
+        if (sharded) {
+            double *loc = nullptr;
+            if (nK_loc > 0) RISP_CUDA_TRY(cudaMalloc((void **)&loc, (size_t)nK_loc * tri_o * 8));
+            for (int f = 0; f < nK; ++f)
+                if (loc_of[f] >= 0) RISP_CUDA_TRY(cudaMemcpyAsync(loc + (size_t)loc_of[f] * tri_o, ctx->d_TijP + (size_t)f * tri_o, (size_t)tri_o * 8, cudaMemcpyDeviceToDevice, 0));
+            RISP_CUDA_TRY(cudaDeviceSynchronize());
+            cudaFree(ctx->d_TijP);
+            ctx->setup_bytes -= (size_t)(nK - nK_loc) * tri_o * 8;
+            ctx->d_TijP = loc;
+            ctx->nauxK_global = nK; ctx->nauxK = nK_loc; ctx->nK_dev = nK_loc;
+            if (nK_loc == 0) ctx->has_K = false;
+        }
         if (ctx->d_Tov) {
             // T^P <- sum_Q L_K^-1[P][Q] (ov|J^|Q): [nK x nK] x [nK x (o' v')] in column panels, in place
             const long long cols = (long long)no * nv_p;

@@ -119,3 +119,74 @@ def test_bench_reference_arm_prints_the_contract_line():
         assert k in line, k
     assert line["impl"] == "reference" and line["value"] > 0 and line["config"]["workload"].startswith("cfg1")
     assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
+
+
+_SHARD_WORKER = r"""
+import os, sys, numpy as np, torch, torch.distributed as dist
+sys.path.insert(0, sys.argv[1])
+from workloads import make_system, trial_vectors
+from oracle.risp_oracle import Oracle
+from paper_2603_29257_b200.sharded import sharded_matvec, shard_of_pair, shard_of_aux_centre
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+s = make_system(3, counts=(6, 4, 1, 1))
+o = Oracle(s); o.build()
+X = trial_vectors(s, 3)
+
+
+class OracleShard:
+    # a CPU stand-in for one rank's sharded context, built on the oracle: AO pairs and whitened K aux functions dealt round robin
+    def __init__(self):
+        self.I3 = o.int3c(o.selJ)
+        n = o.nao
+        iu = np.array([(a, b) for a in range(n) for b in range(a + 1)])
+        mine = np.array([shard_of_pair(k, world) == rank for k in range(len(iu))])
+        self.mask = np.zeros((n, n), dtype=bool)
+        self.mask[iu[mine, 0], iu[mine, 1]] = True
+        self.full = np.zeros((n, n)); self.full[self.mask] = 1.0
+        self.w = self.full + np.tril(self.full, -1).T                  # (mu, nu) and (nu, mu) of an owned lower-triangular pair
+        self.kfun = [p for p in range(o.BijW.shape[0]) if shard_of_aux_centre(p, world) == rank]
+
+    def matvec_shard_begin(self, Xt):
+        Xn = Xt.numpy()
+        D = [o.Co @ Xn[k] @ o.Cv.T for k in range(len(Xn))]
+        R = np.zeros((self.I3.shape[0], 32))
+        for k, Dk in enumerate(D):
+            R[:, k] = np.einsum('qmn,mn->q', self.I3, Dk * self.w)
+        return torch.from_numpy(R)
+
+    def matvec_shard_end(self, Xt, R):
+        Xn = Xt.numpy(); m = len(Xn)
+        Rt = np.linalg.solve(o.MJ, R.numpy()[:, :m])
+        sig = np.zeros_like(Xn)
+        for k in range(m):
+            U = np.einsum('pmn,p->mn', self.I3, Rt[:, k]) * self.w
+            sig[k] = 2.0 * (o.Co.T @ U @ o.Cv)
+        Xw = Xn[:, o.occK][:, :, o.virK]
+        Kw = np.zeros_like(Xw)
+        for P in self.kfun:
+            Kw += o.BijW[P][None] @ (Xw @ o.BabW[P].T)
+        sig[np.ix_(np.arange(m), o.occK, o.virK)] -= Kw
+        if rank == 0:
+            sig += o.delta[None] * Xn
+        return torch.from_numpy(sig)
+
+
+sig = sharded_matvec(OracleShard(), torch.from_numpy(X)).numpy()
+ref = o.sigma(X)
+err = float(np.linalg.norm(sig - ref) / np.linalg.norm(ref))
+assert err < 1e-11, err
+dist.barrier(); dist.destroy_process_group()
+print("ok", rank, err)
+"""
+
+
+def test_p_sharded_driver_world_size_2_gloo(tmp_path):
+    """The two collectives of the P-sharded sigma-build (all-reduce of R between the passes, all-reduce of sigma) under gloo with
+    two ranks; each rank's context is an oracle-backed stand-in that owns every second AO pair and every second K aux function."""
+    w = tmp_path / "shard_worker.py"
+    w.write_text(_SHARD_WORKER)
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2", "--master-addr", "127.0.0.1",
+                        "--master-port", "29547", str(w), ROOT], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert r.stdout.count("ok") == 2
