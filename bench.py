@@ -379,6 +379,52 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
     return res
 
 
+def run_sharded(args, world, rank, local, dist):
+    """--parallel shard (N > 1): ONE problem, P-sharded over the ranks: every rank holds 1/N of the shell pairs
+    and of the K-tensor slices, X is replicated, two all-reduces per batch (R between the integral passes, sigma at the end).
+    Strong scaling: the same m sigma-builds are done by all ranks together."""
+    import torch
+    from paper_2603_29257_b200 import setup
+    from paper_2603_29257_b200.sharded import sharded_matvec
+    from workloads import make_system, trial_vectors
+    dev = torch.device(f"cuda:{local}")
+    s = make_system(args.config)
+    m = min(args.batch if args.batch > 0 else s["m"], 32)
+    X = torch.from_numpy(trial_vectors(s, m)).to(dev)
+    t0 = time.time()
+    ctx = setup(s, device=local, max_batch=m, shard_rank=rank, shard_count=world)
+    t_setup = time.time() - t0
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream(dev)
+    for _ in range(args.warmup):
+        sharded_matvec(ctx, X)
+    dist.barrier(); torch.cuda.synchronize(dev)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in evs:
+        flush.zero_()
+        dist.barrier()
+        a.record(stream)
+        sig = sharded_matvec(ctx, X)
+        b.record(stream)
+        b.synchronize()
+    dist.barrier(); torch.cuda.synchronize(dev)
+    tt = torch.tensor([sum(a.elapsed_time(b) for a, b in evs) * 1e-3], dtype=torch.float64, device=dev)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    d = ctx.dims()
+    launches = ctx.timings()["kernel_launches"] * args.steps
+    ctx.close()
+    if rank == 0:
+        t_dev = float(tt[0])
+        print(json.dumps(dict(metric=METRIC, value=m * args.steps / t_dev, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+                              ms_per_step=1e3 * t_dev / args.steps, higher_is_better=True, scaling="strong", vs_baseline=None, dtype="f64", data="synthetic",
+                              config=dict(workload=s["name"], m=m, atoms=int(s["natm"]), nao=s["nao"], nocc=s["nocc"], nvir=s["nvir"],
+                                          parallelism=f"P-sharded x{world}: shell pairs and K aux centres dealt round robin, all-reduce of R and of sigma",
+                                          shell_pairs_kept_rank0=d["n_shell_pairs_kept"], nauxK_rank0=d["nauxK"], setup_s=round(t_setup, 3),
+                                          l2="flushed between steps (512 MiB write)"),
+                              gpu_launches=launches, e2e=None, roofline=None, cpu_baseline=None,
+                              note="sharded mode: device-resident replicated X; no roofline / e2e legs in this mode")))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -398,6 +444,8 @@ def main():
     ap.add_argument("--solve", action="store_true", help="(default) kept for compatibility")
     ap.add_argument("--also", default="4", help="comma separated further configs run briefly after the main one (1 GPU only); '' for none")
     ap.add_argument("--also-budget-s", type=float, default=420.0, help="an `also` config starts only if the run is younger than this")
+    ap.add_argument("--parallel", default="vectors", choices=["vectors", "shard"],
+                    help="N > 1: 'vectors' = every rank its own batch (weak scaling, no collective); 'shard' = one P-sharded problem (strong scaling)")
     ap.add_argument("--host-budget-gb", type=int, default=0, help="pinned-host budget of the Davidson subspace (0: half of the host memory)")
     args = ap.parse_args()
     # contract: >= 3 warm-up steps; the 1000/3000-atom configs (tens of seconds to minutes per step) are allowed 1 and say so
@@ -415,6 +463,10 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
 
+    if world > 1 and args.parallel == "shard":
+        run_sharded(args, world, rank, local, dist)
+        dist.destroy_process_group()
+        return
     solve_main = not args.no_solve and world == 1 and args.config <= 4
     solve_main = solve_main or (not args.no_solve and world == 1 and args.solve)
     line = run_config(args.config, args, world, rank, local, dist, want_solve=solve_main, want_cpu=not args.no_cpu_baseline,
