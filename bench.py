@@ -219,12 +219,12 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
     if Xp is None:
         Xp = torch.from_numpy(X_h).pin_memory()
     Sp = torch.empty(Xp.shape, dtype=torch.float64, pin_memory=True)
-    for _ in range(2 if cfg <= 3 else 1):
+    for _ in range(0 if args.no_e2e else (2 if cfg <= 3 else 1)):
         ctx.matvec_host_ptr(m, Xp.data_ptr(), Sp.data_ptr())
     barrier()
     t_e2e = 0.0
     e2e_steps = steps if cfg <= 3 else 1
-    for _ in range(e2e_steps):
+    for _ in range(0 if args.no_e2e else e2e_steps):
         flush.zero_(); torch.cuda.synchronize(dev)
         t0 = time.perf_counter()
         ctx.matvec_host_ptr(m, Xp.data_ptr(), Sp.data_ptr())
@@ -234,7 +234,7 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
         tt = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=dev)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         t_dev, t_e2e = float(tt[0]), float(tt[1])
-    same = bool(torch.equal(Sp.view(m, -1)[:, ::997], fp)) if big else bool(np.array_equal(Sp.numpy(), sig_h))
+    same = None if args.no_e2e else (bool(torch.equal(Sp.view(m, -1)[:, ::997], fp)) if big else bool(np.array_equal(Sp.numpy(), sig_h)))
     if not big:
         del X, sigma
     del flush, Xp, Sp, fp
@@ -297,7 +297,7 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
                         l2="flushed between steps (512 MiB write)",
                         parallelism=f"trial-vector shards x{world}", setup_s=round(t_setup, 3)),
             clocks=clocks,
-            e2e=dict(value=world * m * e2e_steps / t_e2e, steps=e2e_steps, unit=UNIT, h2d_bytes_per_step=int(X_h.nbytes), d2h_bytes_per_step=int(X_h.nbytes),
+            e2e=None if args.no_e2e else dict(value=world * m * e2e_steps / t_e2e, steps=e2e_steps, unit=UNIT, h2d_bytes_per_step=int(X_h.nbytes), d2h_bytes_per_step=int(X_h.nbytes),
                      bitwise_equal_to_device_path=same),
             gpu_launches=launches,
             roofline=dict(bound="tensor", kernel="dgemm_tma_kernel<KC,KC,MI> (K contraction M^P = X' T_ab^P, Eq. 22)", achieved=achieved, peak=peak,
@@ -335,8 +335,8 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
             line["cpu_baseline"] = cb
         if want_solve:
             big_dim = s["nocc"] * s["nvir"] >= 5e7
-            kw = dict(tol=args.solve_tol, max_iter=args.solve_max_iter, allow_unconverged=True, n_guess=args.solve_n_guess)
-            flags = (8 if args.solve_fp32_host else 0) | (16 if big_dim else 0)
+            kw = dict(tol=args.solve_tol, max_iter=args.solve_max_iter, allow_unconverged=True, n_guess=args.solve_n_guess, max_seconds=args.solve_max_seconds)
+            flags = (8 if args.solve_fp32_host else 0) | (16 if big_dim else 0) | (32 if args.progress_file else 0)
             omega, Xs, info = ctx.tda_solve(s["nroots"], want_vectors=True, flags=flags, **kw)
             sv = dict(nroots=s["nroots"], tol=args.solve_tol, n_guess=args.solve_n_guess or 2 * s["nroots"], wall_s=info["sec_total"], matvec_s=info["sec_matvec"],
                       alloc_s=info["sec_alloc"], subspace_s=info["sec_subspace"], block=info["block"], capacity=info["capacity"],
@@ -437,6 +437,8 @@ def main():
     ap.add_argument("--batch", type=int, default=0, help="trial vectors per step (0: the config's m)")
     ap.add_argument("--solve-max-iter", type=int, default=150)
     ap.add_argument("--solve-tol", type=float, default=1e-5)
+    ap.add_argument("--solve-max-seconds", type=int, default=0, help="wall-clock guard of the solve (0: none)")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (long runs under a wall-clock limit)")
     ap.add_argument("--solve-n-guess", type=int, default=0, help="initial unit vectors of the solve (0: 2 * nroots, the config's batch of 30)")
     ap.add_argument("--solve-fp32-host", action="store_true", help="RISP_SOLVE_HOST_FP32 for the solve of the 1000/3000-atom systems")
     ap.add_argument("--progress-file", default="", help="write the solve record to this file as soon as risp_tda_solve returns")

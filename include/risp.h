@@ -104,7 +104,8 @@ typedef struct {
     int32_t max_block;          /* trial vectors per sigma-build inside the solver (0 -> min(32, max_batch of risp_setup, n_guess)); the
                                    solver holds two blocks of this many vectors on the device, everything else of the subspace is
                                    cached in what HBM is left or streamed from pinned host memory */
-    int32_t reserved;
+    int32_t max_seconds;        /* wall-clock guard: no new iteration starts after this many seconds (0 -> none); the call then returns
+                                   RISP_ENOTCONV with the current Ritz values, residual norms and vectors */
     size_t device_budget_bytes; /* device memory the solver may allocate (0 -> what is free after the matvec work space); if two
                                    blocks and the streaming buffers do not fit: RISP_ENOMEM, nothing stays allocated */
 } risp_solve_options;
@@ -119,6 +120,9 @@ typedef struct {
 
 #define RISP_SOLVE_X_OUT_HOST 16      /* X_out is a HOST pointer: the Ritz vectors are written there chunk by chunk (3000 atoms: 15 vectors
                                         are 16 GB, more than is left on the device beside the K tensors) */
+
+#define RISP_SOLVE_LOG_STDERR 32     /* one line per iteration on stderr (iteration, subspace size, unconverged roots, largest residual, seconds):
+                                        a long solve leaves its history behind even if the job is cut short */
 
 #define RISP_MAX_ROOTS 64
 typedef struct {

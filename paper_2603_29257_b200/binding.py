@@ -45,7 +45,7 @@ class _Options(C.Structure):
 
 class _SolveOptions(C.Structure):
     _fields_ = [("tol", C.c_double), ("max_iter", C.c_int32), ("n_guess", C.c_int32), ("max_sub", C.c_int32), ("flags", C.c_int32),
-                ("max_block", C.c_int32), ("reserved", C.c_int32), ("device_budget_bytes", C.c_size_t)]
+                ("max_block", C.c_int32), ("max_seconds", C.c_int32), ("device_budget_bytes", C.c_size_t)]
 
 
 class _SolveInfo(C.Structure):
@@ -191,11 +191,11 @@ class RispContext:
         self._check(self.lib.risp_matvec_host(self.handle, m, x_ptr, s_ptr))
 
     def tda_solve(self, nroots, tol=1e-5, max_iter=100, n_guess=0, max_sub=0, want_vectors=False, allow_unconverged=False, flags=0,
-                  max_block=0, device_budget_bytes=0):
+                  max_block=0, device_budget_bytes=0, max_seconds=0):
         import torch
         omega = np.zeros(nroots)
         info = _SolveInfo()
-        opt = _SolveOptions(float(tol), int(max_iter), int(n_guess), int(max_sub), int(flags), int(max_block), 0, int(device_budget_bytes))
+        opt = _SolveOptions(float(tol), int(max_iter), int(n_guess), int(max_sub), int(flags), int(max_block), int(max_seconds), int(device_budget_bytes))
         if want_vectors and (flags & 16):      # RISP_SOLVE_X_OUT_HOST: a host array takes the vectors
             X = np.empty((nroots, self.nocc, self.nvir))
             xptr = X.ctypes.data

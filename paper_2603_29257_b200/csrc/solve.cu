@@ -695,8 +695,16 @@ extern "C" int risp_tda_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_op
             appended += nb;
         }
         n_unconv_prev = n_unconv;
+        if (opt.flags & RISP_SOLVE_LOG_STDERR) {
+            double rmax = 0.0;
+            for (int j = 0; j < nroots; ++j) rmax = std::max(rmax, rn[j]);
+            std::fprintf(stderr, "[risp_tda_solve] it %d  subspace %d  unconverged %d  max residual %.3e  omega_1 %.8f Ha  sigma-builds %d  restarts %d  %.1f s\n", it, S.k,
+                         n_unconv, rmax, theta[0], n_sigma, restarts, std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count());
+            std::fflush(stderr);
+        }
         if (n_unconv == 0) { converged = true; break; }
         if (it == max_iter) break;
+        if (opt.max_seconds > 0 && std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count() > (double)opt.max_seconds) break;
         if (appended == 0 && S.k < S.cap) break;     // nothing new to add although there is room: stagnated
     }
     for (int j = 0; j < nroots; ++j) omega_out[j] = theta[j];
