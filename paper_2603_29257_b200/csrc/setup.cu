@@ -308,32 +308,12 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
     { int rc; if ((rc = upload(ctx, ctx->d_cenJ, cenJ.data(), cenJ.size()))) return rc; if ((rc = upload(ctx, ctx->d_cenK, cenK.data(), cenK.size()))) return rc; }
 
     // ---------------------------------------------------------------- a0: screened shell-pair list
-    {
-        double tau = opt.screen_tol == 0.0 ? 1e-13 : opt.screen_tol;
-        double gmin = 1e300;
-        for (int s = 0; s < sys->naux; ++s) gmin = std::min(gmin, sys->aux_exp[s]);
-        double vmax = 2.0 * 4.48 * std::pow(gmin, -0.25);    // ~ 2 x the peak potential of a unit-normalised s aux Gaussian
-        std::vector<ShellPair> pairs[6];
-        std::vector<PrimPair> prims;
-        ctx->n_shell_pairs = (long long)sys->nshl * (sys->nshl + 1) / 2;
-        long long kept_seen = 0;
-        for (int sa = 0; sa < sys->nshl; ++sa)
-            for (int sb = 0; sb <= sa; ++sb) {
-                int A = sa, B = sb;
-                if (sys->shl_l[A] < sys->shl_l[B]) std::swap(A, B);
-                ShellPair sp;
-                size_t mark = prims.size();
-                double est = pair_estimate_and_build(ctx, A, B, sp, prims, tau < 0 ? -1.0 : tau * 1e-3, vmax);
-                if ((tau >= 0 && est < tau) || sp.npp == 0) { prims.resize(mark); continue; }
-                // P-sharded sigma-build: the kept pairs are dealt round robin; every rank runs both integral
-                // passes and the pair-sparse halves of the J transforms on its own pairs only
-                if (ctx->shard_count > 1 && (kept_seen++ % ctx->shard_count) != ctx->shard_rank) { prims.resize(mark); continue; }
-                pairs[class_index(sys->shl_l[A], sys->shl_l[B])].push_back(sp);
-                ctx->h_kept_pairs.push_back(A); ctx->h_kept_pairs.push_back(B);
-                ctx->n_ao_pairs_kept += (A == B) ? (long long)(2 * sys->shl_l[A] + 1) * (2 * sys->shl_l[A] + 2) / 2
-                                                 : (long long)(2 * sys->shl_l[A] + 1) * (2 * sys->shl_l[B] + 1);
-            }
+    std::vector<ShellPair> pairs[6];
+    std::vector<PrimPair> prims;
+    // (re)install the pair classes from `pairs`: sorted lists, panel indices, e0 offsets, pass-1 chunking, device copies
+    auto install_pairs = [&]() -> int {
         long long e_off = 0, total_pairs = 0;
+        ctx->h_kept_pairs.clear(); ctx->n_ao_pairs_kept = 0;
         for (int c = 0; c < 6; ++c) total_pairs += (long long)pairs[c].size();
         ctx->n_shell_pairs_kept = total_pairs;
         // pass-1 chunking per class: about 16 CTAs per SM over (pair chunks) x (groups of 8 aux centres), at least 16 pairs per chunk
@@ -343,11 +323,18 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
         static const int LA[6] = {0, 1, 1, 2, 2, 2}, LB[6] = {0, 0, 1, 0, 1, 2};
         for (int c = 0; c < 6; ++c) {
             PairClass &pc = ctx->cls[c];
+            if (pc.d_pairs) { cudaFree(pc.d_pairs); pc.d_pairs = nullptr; ctx->setup_bytes -= (size_t)pc.npairs * sizeof(ShellPair); }
+            if (pc.d_permB) { cudaFree(pc.d_permB); pc.d_permB = nullptr; ctx->setup_bytes -= (size_t)pc.npairs * sizeof(int); }
             // sorted by the first AO of shell A: a panel of AO rows of D / U is then a contiguous pair range
             std::stable_sort(pairs[c].begin(), pairs[c].end(), [](const ShellPair &x, const ShellPair &y) { return x.aoA < y.aoA; });
             pc.la = LA[c]; pc.lb = LB[c]; pc.npairs = (int)pairs[c].size();
             pc.h_aoA.resize(pc.npairs);
-            for (int k = 0; k < pc.npairs; ++k) pc.h_aoA[k] = pairs[c][k].aoA;
+            for (int k = 0; k < pc.npairs; ++k) {
+                const ShellPair &q = pairs[c][k];
+                pc.h_aoA[k] = q.aoA;
+                ctx->h_kept_pairs.push_back(q.shA); ctx->h_kept_pairs.push_back(q.shB);
+                ctx->n_ao_pairs_kept += (q.shA == q.shB) ? (long long)(2 * pc.la + 1) * (2 * pc.la + 2) / 2 : (long long)(2 * pc.la + 1) * (2 * pc.lb + 1);
+            }
             {   // second index of the same pairs, sorted by the first AO of shell B (row panels that hold the rows of B)
                 std::vector<int> perm(pc.npairs);
                 for (int k = 0; k < pc.npairs; ++k) perm[k] = k;
@@ -368,7 +355,26 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
             if ((rc = upload(ctx, pc.d_pairs, pairs[c].data(), pairs[c].size()))) return rc;
         }
         ctx->e_rows = e_off; ctx->total_chunks = chunk_base;
+        return RISP_OK;
+    };
+    {
+        double tau = opt.screen_tol == 0.0 ? 1e-13 : opt.screen_tol;
+        double gmin = 1e300;
+        for (int s = 0; s < sys->naux; ++s) gmin = std::min(gmin, sys->aux_exp[s]);
+        double vmax = 2.0 * 4.48 * std::pow(gmin, -0.25);    // ~ 2 x the peak potential of a unit-normalised s aux Gaussian
+        ctx->n_shell_pairs = (long long)sys->nshl * (sys->nshl + 1) / 2;
+        for (int sa = 0; sa < sys->nshl; ++sa)
+            for (int sb = 0; sb <= sa; ++sb) {
+                int A = sa, B = sb;
+                if (sys->shl_l[A] < sys->shl_l[B]) std::swap(A, B);
+                ShellPair sp;
+                size_t mark = prims.size();
+                double est = pair_estimate_and_build(ctx, A, B, sp, prims, tau < 0 ? -1.0 : tau * 1e-3, vmax);
+                if ((tau >= 0 && est < tau) || sp.npp == 0) { prims.resize(mark); continue; }
+                pairs[class_index(sys->shl_l[A], sys->shl_l[B])].push_back(sp);
+            }
         int rc;
+        if ((rc = install_pairs())) return rc;      // the whole list: the K-tensor build below needs (mu nu|P) on every kept pair
         if ((rc = upload(ctx, ctx->d_prims, prims.data(), prims.size()))) return rc;
     }
 
@@ -627,6 +633,18 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
         }
     }
     RISP_CUDA_TRY(cudaDeviceSynchronize());
+    if (ctx->shard_count > 1) {
+        // P-sharded sigma-build: from here on this rank runs both integral passes and the pair-sparse halves
+        // of the J transforms on its own pairs only -- the kept pairs of every class are dealt round robin
+        for (int c = 0; c < 6; ++c) {
+            std::vector<ShellPair> mine;
+            for (size_t k = 0; k < pairs[c].size(); ++k)
+                if ((int)(k % ctx->shard_count) == ctx->shard_rank) mine.push_back(pairs[c][k]);
+            pairs[c].swap(mine);
+        }
+        int rc;
+        if ((rc = install_pairs())) return rc;
+    }
     RISP_CUDA_TRY(cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking));
     for (int i = 0; i < RISP_NEV; ++i) RISP_CUDA_TRY(cudaEventCreate(&ctx->ev[i]));
     RISP_CUDA_TRY(cudaEventCreateWithFlags(&ctx->evFork, cudaEventDisableTiming));
