@@ -287,10 +287,13 @@ __global__ void __launch_bounds__(32 * JW) j_pass1_kernel(const ShellPair *__res
                                                           int ncen_pad, const double *__restrict__ boys_tab, const double *__restrict__ dbar,
                                                           long long e_off, double *__restrict__ Rpart, int njn)
 {
-    constexpr int NE = ne_of(LA, LB), KS = P1_KS, KROWS = 4 * NE;
+    // SKEW: with an even NE the four pair slots of a step would start 0 mod 16 doubles apart and their parking stores would
+    // collide four ways; 8 doubles of skew per slot bring the stores to the two-wavefront optimum (the fragment loads then
+    // collide two ways only in the k-steps that straddle two slots)
+    constexpr int NE = ne_of(LA, LB), KS = P1_KS, KROWS = 4 * NE, SKEW = (NE % 2 == 0) ? 8 : 0, WARP_DOUBLES = KROWS * KS + 4 * SKEW;
     extern __shared__ double smem[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    double *g = smem + (size_t)w * KROWS * KS;
+    double *g = smem + (size_t)w * WARP_DOUBLES;
     const int p_begin = blockIdx.x * chunk, p_end = min(npairs, p_begin + chunk);
     const int slot = lane >> 3, a = lane & 7, q = lane >> 2, r = lane & 3;
     const int ci = blockIdx.y * 8 + a;
@@ -303,26 +306,40 @@ __global__ void __launch_bounds__(32 * JW) j_pass1_kernel(const ShellPair *__res
         for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
     constexpr bool LEAN = NE > 10;          // dp, dd: the recursion already spills; no shell-pair prefetch
     ShellPair sp = pairs[min(p_begin + w * 4 + slot, p_end - 1)];
-    double *base = g + (size_t)slot * NE * KS + a;
+    double *base = g + (size_t)slot * (NE * KS + SKEW) + a;
+    constexpr bool PRE = NE <= 4;           // ss, ps: the operand fragments of the whole step are fetched before the integrals are generated
     for (int pg = p_begin + w * 4; pg < p_end; pg += JW * 4) {
         const int pi = pg + slot;
         const bool valid = cvalid && pi < p_end;
         if constexpr (LEAN) sp = pairs[min(pi, p_end - 1)];
         ShellPair sp_next;
         if constexpr (!LEAN) sp_next = pairs[min(pi + JW * 4, p_end - 1)];
+        const double *db = dbar + (e_off + (long long)pg * NE) * MS + q;
+        double bpre[PRE ? NE : 1][4];
+        if constexpr (PRE) {
+#pragma unroll
+            for (int t = 0; t < NE; ++t) {
+                const int kk = 4 * t + r;
+                const bool kv = pg + kk / NE < p_end;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) bpre[t][j] = (kv && j < njn) ? db[(long long)kk * MS + 8 * j] : 0.0;
+            }
+        }
         park_integrals<LA, LB, KS, 8>(base, valid, sp, prims, ax, boys_tab);
         if constexpr (!LEAN) sp = sp_next;
         __syncwarp();
-        const double *db = dbar + (e_off + (long long)pg * NE) * MS + q;
-#pragma unroll 4
+#pragma unroll(PRE ? NE : 4)
         for (int t = 0; t < NE; ++t) {              // K = 4 NE = (pair, e) in steps of 4
             const int kk = 4 * t + r;
             const bool kv = pg + kk / NE < p_end;   // rows of pairs beyond the chunk: parked zeros, operand not read
             double bf[4], af[4];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) bf[j] = (kv && j < njn) ? db[(long long)kk * MS + 8 * j] : 0.0;
+            for (int j = 0; j < 4; ++j) {
+                if constexpr (PRE) bf[j] = bpre[t][j];
+                else bf[j] = (kv && j < njn) ? db[(long long)kk * MS + 8 * j] : 0.0;
+            }
 #pragma unroll
-            for (int i = 0; i < 4; ++i) af[i] = g[kk * KS + 8 * i + q];
+            for (int i = 0; i < 4; ++i) af[i] = g[kk * KS + (kk / NE) * SKEW + 8 * i + q];
 #pragma unroll
             for (int i = 0; i < 4; ++i)
 #pragma unroll
@@ -333,7 +350,7 @@ __global__ void __launch_bounds__(32 * JW) j_pass1_kernel(const ShellPair *__res
     // cross-warp reduction (fixed order -> deterministic) in a dedicated region after the parking area: red[w][k = a*4 + c][m];
     // this lane holds, for component c = i, centre a = q and vectors m = 8j + 2r, 8j + 2r + 1
     __syncthreads();
-    double *red = smem + (size_t)JW * KROWS * KS;     // [JW][32][32]
+    double *red = smem + (size_t)JW * WARP_DOUBLES;   // [JW][32][32]
 #pragma unroll
     for (int i = 0; i < 4; ++i)
 #pragma unroll
@@ -453,7 +470,7 @@ cudaError_t risp_j_pass1(const PairClass &pc, const PrimPair *prims, const AuxCe
     cudaError_t err = cudaSuccess;
     dispatch_class(pc.la, pc.lb, [&](auto LA, auto LB) {
         constexpr int A = decltype(LA)::value, B = decltype(LB)::value;
-        size_t smem = ((size_t)JW * 4 * ne_of(A, B) * P1_KS + (size_t)JW * 32 * 32) * sizeof(double);
+        size_t smem = ((size_t)JW * (4 * ne_of(A, B) * P1_KS + 32) + (size_t)JW * 32 * 32) * sizeof(double);
         err = ensure_smem(j_pass1_kernel<A, B>, smem);
         if (err != cudaSuccess) return;
         dim3 grid(pc.nchunks, (ncen + 7) / 8);
