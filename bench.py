@@ -275,14 +275,16 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
                           transforms_dense=4.0 * m * s["nocc"] * s["nvir"] * s["nao"] + 4.0 * m * s["nao"] ** 2 * s["nocc"],
                           transforms_pair_sparse=4.0 * m * s["nocc"] * s["nvir"] * s["nao"] + 8.0 * m * z_pairs * s["nocc"])
         eri = _eri_flops_per_task()
-        eri_entry = dict(phase="ERI passes (Eq. 14, 16): FP64 instructions executed, both passes", bound="alu", unit="TFLOP/s", achieved=None, peak=dfma,
+        eri_entry = dict(phase="ERI passes (Eq. 14, 16): FP64 flops executed, both passes (integral generation: 2 DFMA + DMUL + DADD per task from ncu; contraction: DMMA, 2 m flops per integral)", bound="alu", unit="TFLOP/s", achieved=None, peak=dfma,
                          peak_source="risp_debug_yardstick(0): register-resident DFMA chains on all SMs, measured in this run")
         t_eri = (phase["j_pass1"] + phase["j_pass2"]) / steps
         if eri is not None and t_eri > 0:
             fl = 0.0
+            ne_class = [1, 4, 9, 6, 16, 31]           # e0 components of the classes ss, ps, pp, ds, dp, dd
+            mcols = 8 * ((m + 7) // 8)                # trial-vector columns the DMMA contraction really computes
             for c, npairs in enumerate(d["pairs_per_class"]):
                 for ps in ("pass1", "pass2"):
-                    fl += eri[ps][c] * npairs * d["n_aux_centres"]
+                    fl += (eri[ps][c] + 2.0 * mcols * 4 * ne_class[c]) * npairs * d["n_aux_centres"]
             eri_entry.update(achieved=fl / t_eri / 1e12, frac=fl / t_eri / 1e12 / dfma, flops_per_step=fl,
                              note=eri.get("note", ""))
         t_tr = (phase["j_transform_in"] + phase["j_transform_out"]) / steps
@@ -290,7 +292,7 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
             metric=METRIC, value=world * m * steps / t_dev, unit=UNIT, n_gpus=world, steps=steps, warmup=warmup,
             ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
             config=dict(workload=s["name"], m=m, atoms=int(s["natm"]), nao=s["nao"], nocc=s["nocc"], nvir=s["nvir"], nauxJ=d["nauxJ"], nauxK=nK,
-                        noccK=no, nvirK=nv, shell_pairs_kept=d["n_shell_pairs_kept"], shell_pairs=d["n_shell_pairs"],
+                        noccK=no, nvirK=nv, shell_pairs_kept=d["n_shell_pairs_kept"], shell_pairs=d["n_shell_pairs"], pairs_per_class=list(d["pairs_per_class"]), aux_centres=d["n_aux_centres"],
                         ao_pair_survival=round(2.0 * d["n_ao_pairs_kept"] / (s["nao"] * (s["nao"] + 1)), 4),
                         K_tensors=f"packed lower triangles; {d['nauxK_device']} of {nK} aux slices in HBM, {d['bytes_T_host']} B in pinned host memory",
                         bytes_T=d["bytes_Tij"] + d["bytes_Tab"], aux_chunk=d["aux_chunk"], j_sub_batch=d["j_sub_batch"], j_panels=d["j_panels"],
