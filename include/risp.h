@@ -172,6 +172,20 @@ int risp_setup(const risp_system *sys, const risp_options *opt, risp_ctx **out);
  * (RISP_ENOMEM if that no longer fits beside the K tensors).  risp_get_timings / risp_get_stage refer to the last sub-batch. */
 int risp_matvec(risp_ctx *ctx, int32_t m, const double *X_dev, double *sigma_dev, void *cuda_stream);
 
+/* Precision of the exchange contractions Eq. 22-23 of every following sigma-build of this context
+ * (risp_matvec, risp_matvec_host, risp_matvec_shard_*, risp_tda_solve):
+ *   RISP_PRECISION_FP64    (default) FP64 DMMA GEMMs; sigma within 1e-10 of the FP64 oracle;
+ *   RISP_PRECISION_FP32_K  the paper's own precision for everything after the integrals: X', T_ij, T_ab and M^P are
+ *                          carried as three bf16 terms each (24 significand bits), the products run on the tcgen05 tensor cores with
+ *                          FP32 accumulation in tensor memory, the aux chunks are summed in FP64.  The K term then carries a
+ *                          relative error of order 1e-7 (DESIGN.md "FP32 mode" derives the bound; oracle/risp_fp32.py is the
+ *                          plain binary32 contraction it is compared with).  Diagonal, J term and the Davidson algebra stay FP64;
+ *                          the K tensors stay stored in FP64.  risp_matvec_tddft returns RISP_EINVAL in this mode.
+ * Returns RISP_OK or RISP_EINVAL (unknown mode, or RISP_PRECISION_FP32_K on a device without tcgen05). */
+#define RISP_PRECISION_FP64 0
+#define RISP_PRECISION_FP32_K 1
+int risp_set_precision(risp_ctx *ctx, int32_t mode);
+
 /* Full TDDFT-risp (Eq. 1-2; XC kernel dropped): for m trial vectors
  *     sigma_plus  = (A+B) X = Delta X + 4 J X - K1 X - K2 X,        sigma_minus = (A-B) X = Delta X - K1 X + K2 X,
  * J = (ia|jb)_RI-J, K1 = (ij|J^|ab)_RI-K, K2 = (ib|J^|ja)_RI-K, the two exchange terms restricted to the exchange window

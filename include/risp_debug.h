@@ -44,6 +44,18 @@ int risp_debug_yardstick(risp_ctx *ctx, int which, size_t bytes, int reps, doubl
  * out_host[6][nao][nao] = <mu|(r-O)_k|nu> for k = x, y, z, then <mu|((r-O) x nabla)_k|nu>.  origin_bohr: HOST [3] or NULL. */
 int risp_debug_oneel_ao(risp_ctx *ctx, const double *origin_bohr, double *out_host);
 
+/* The GEMM of the single-precision mode (RISP_PRECISION_FP32_K; Eq. 22-23 on the tcgen05 tensor cores with operands carried as
+ * three bf16 terms, FP32 accumulation) on its own:  C[z][c][r] (+)= sum_k A[z][r][k] B[z][c][k]  for z < nbatch, all DEVICE FP64,
+ * A [nbatch][M][K], B [nbatch][N][K], C [nbatch][N][M] contiguous.  via_planes != 0 routes the result through the three-bf16-plane
+ * store that feeds Eq. 23; seg_kb = number of 32-k stages accumulated in tensor memory before the partial sum is added, rounded to
+ * nearest, to the FP32 running sum in registers (0: the default of the library).  Synchronous.  Returns RISP_OK, RISP_EINVAL,
+ * RISP_ENOMEM or RISP_ECUDA. */
+int risp_debug_tcgemm(int32_t M, int32_t N, int32_t K, int32_t nbatch, const double *A_dev, const double *B_dev, double *C_dev,
+                      int32_t accumulate, int32_t via_planes, int32_t seg_kb, void *stream);
+
+/* The same segment length for the Eq. 22-23 GEMMs of the following risp_matvec calls in RISP_PRECISION_FP32_K (0: default). */
+int risp_debug_set_tc_segment(risp_ctx *ctx, int32_t seg_kb);
+
 #ifdef __cplusplus
 }
 #endif

@@ -94,6 +94,7 @@ def load_library():
     lib.risp_get_timings.argtypes = [vp, C.POINTER(_Timings)]
     lib.risp_eri3c_shell.argtypes = [vp, i32, i32, i32, i32, vp]
     lib.risp_get_stage.argtypes = [vp, i32, vp, i64, vp]
+    lib.risp_set_precision.argtypes = [vp, i32]
     lib.risp_matvec_shard_begin.argtypes = [vp, i32, vp, vp, vp]
     lib.risp_matvec_shard_end.argtypes = [vp, i32, vp, vp, vp, vp]
     lib.risp_matvec_tddft.argtypes = [vp, i32, vp, vp, vp, vp]
@@ -103,6 +104,8 @@ def load_library():
     lib.risp_debug_oneel_ao.argtypes = [vp, vp, vp]
     lib.risp_debug_dgemm.argtypes = [C.c_int, C.c_int, C.c_int, vp, C.c_longlong, C.c_int, vp, C.c_longlong, C.c_int, vp, C.c_longlong,
                                      dbl, dbl, C.c_int, C.c_longlong, C.c_longlong, C.c_longlong, C.c_int, C.c_int, C.c_longlong, vp]
+    lib.risp_debug_tcgemm.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, vp]
+    lib.risp_debug_set_tc_segment.argtypes = [vp, C.c_int32]
     lib.risp_debug_sym_eig_lowest.argtypes = [C.c_int, C.c_int, vp, vp, vp]
     lib.risp_debug_force_plan.argtypes = [vp, C.c_int, C.c_int, C.c_int]
     lib.risp_debug_yardstick.argtypes = [vp, C.c_int, C.c_size_t, C.c_int, C.POINTER(dbl)]
@@ -267,6 +270,10 @@ class RispContext:
         out = np.zeros((6, self.nao, self.nao))
         self._check(self.lib.risp_debug_oneel_ao(self.handle, org.ctypes.data if org is not None else None, out.ctypes.data))
         return out
+
+    def set_precision(self, mode: int):
+        """0: FP64 (default); 1: the K contractions in the paper's single precision on the tcgen05 tensor cores."""
+        self._check(self.lib.risp_set_precision(self.handle, int(mode)))
 
     def force_plan(self, mj: int = 0, prow: int = 0, pc: int = 0):
         """Testing: override the work-space plan (J sub-batch, AO rows per panel, K aux chunk); 0 keeps the automatic choice."""

@@ -155,7 +155,8 @@ extern "C" int risp_get_stage(risp_ctx *ctx, int32_t which, const int64_t *sel, 
         if (!ctx->has_K) { std::memset(out, 0, n * 8); return RISP_OK; }
         double *tmp = nullptr;
         RISP_CUDA_TRY(scr.alloc(tmp, n));
-        const double *wKk = ctx->w_arena + (size_t)m * ctx->noccK * ctx->nv_p;     // K' of the last matvec (matvec.cu arena layout)
+        // K' of the last matvec (matvec.cu arena layout: behind X' in FP64 mode, first in the single-precision mode)
+        const double *wKk = ctx->w_arena + (ctx->precision == RISP_PRECISION_FP32_K ? 0 : (size_t)m * ctx->noccK * ctx->nv_p);
         RISP_CUDA_TRY(risp_scatter_window(wKk, tmp, m, ctx->nocc, ctx->nvir, ctx->occK0, ctx->noccK, ctx->virK0, ctx->nvirK, ctx->nv_p, 0));
         RISP_CUDA_TRY(cudaMemcpy(out, tmp, n * 8, cudaMemcpyDeviceToHost));
         return RISP_OK;
@@ -222,4 +223,24 @@ extern "C" int risp_debug_dgemm(int M, int N, int K, const double *A, long long 
     d.nb1 = nbatch; d.sA1 = sA; d.sB1 = sB; d.sC1 = sC;
     d.variant = variant; d.c_rpg = c_rpg; d.c_gstride = c_gstride;
     return risp_dgemm(d, (cudaStream_t)stream) == cudaSuccess ? RISP_OK : RISP_ECUDA;
+}
+
+extern "C" int risp_set_precision(risp_ctx *ctx, int32_t mode)
+{
+    if (!ctx) return RISP_EINVAL;
+    if (mode != RISP_PRECISION_FP64 && mode != RISP_PRECISION_FP32_K) { risp_set_error(ctx, "risp_set_precision: unknown mode"); return RISP_EINVAL; }
+    if (mode == RISP_PRECISION_FP32_K) {
+        cudaDeviceProp prop;
+        RISP_CUDA_TRY(cudaGetDeviceProperties(&prop, ctx->device));
+        if (prop.major != 10) { risp_set_error(ctx, "risp_set_precision: the single-precision mode needs the tcgen05 tensor cores (sm_100)"); return RISP_EINVAL; }
+    }
+    ctx->precision = mode;
+    return RISP_OK;
+}
+
+extern "C" int risp_debug_set_tc_segment(risp_ctx *ctx, int32_t seg_kb)
+{
+    if (!ctx || seg_kb < 0) return RISP_EINVAL;
+    ctx->tc_seg_kb = seg_kb;
+    return RISP_OK;
 }

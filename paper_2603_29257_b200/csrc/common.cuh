@@ -61,6 +61,25 @@ __device__ __forceinline__ void risp_store_c_pair(const GemmDesc &d, double *Cp,
 }
 #endif
 cudaError_t risp_dgemm(const GemmDesc &d, cudaStream_t st);
+
+// ---------------------------------------------------------------------------------------------------
+// Single-precision-mode GEMM on tcgen05 (gemm_tc.cu): operands are three bf16 planes each (x = x1 + x2 + x3), both K-contiguous,
+//   acc(r, c) = sum_k A[z](r, k) B[z](c, k)   in FP32,   stored transposed:
+//   out(r, c) at z*sC + (rpg ? (r / rpg)*gstride + r % rpg : r) + c*ldc;  out_kind 0: FP64 (accumulate: += ), 1: three bf16 planes.
+// Leading dimensions, plane and batch strides are in elements and multiples of 8; sA / sB = 0: the operand is shared by the batch.
+struct TcGemmDesc {
+    int M, N, K, nb;
+    const void *A; long long lda, planeA, sA;
+    const void *B; long long ldb, planeB, sB;
+    void *C; long long ldc, sC, planeC;
+    int out_kind, rpg; long long gstride; int accumulate;
+    int seg_kb = 0;          // 32-k stages per accumulation segment (0: the default, 4)
+};
+cudaError_t risp_tcgemm(const TcGemmDesc &d, cudaStream_t st);
+cudaError_t risp_split_rows_bf3(const double *X, long long ldx, long long rows, int n, void *out, long long ldo, long long plane, int rpg,
+                                long long gstride, cudaStream_t st);
+cudaError_t risp_expand_sym_bf3(const double *packed, long long tri, int n, int np, void *full, long long row_stride, long long p_stride, long long plane,
+                                cudaStream_t st);
 inline GemmDesc gemm_desc(int M, int N, int K, const double *A, long long lda, bool a_kc, const double *B, long long ldb, bool b_kc,
                           double *C, long long ldc, double alpha = 1.0, double beta = 0.0)
 {

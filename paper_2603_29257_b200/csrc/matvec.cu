@@ -272,18 +272,43 @@ after_pass1:
     RISP_CUDA_TRY(cudaEventRecord(ev[5], st));
     // ---------------- K (Eq. 22-23)
     if (ctx->has_K) {
-        const int pc = pl.pc;
+        const bool f32 = ctx->precision == RISP_PRECISION_FP32_K;
+        if (f32 && tddft) { risp_set_error(ctx, "risp_matvec_tddft: the single-precision mode covers the TDA sigma-build only"); return RISP_EINVAL; }
+        int pc = pl.pc;
         double *wXk = ctx->w_arena;                                  // [m][no][nv_p]
         double *wKk = wXk + (size_t)m * no * nv_p;                   // [m][no][nv_p]
         double *wM = wKk + (size_t)m * no * nv_p;                    // [m][pc][no_p][nv_p]
         double *wTab = wM + (size_t)m * pc * no_p * nv_p;            // [pc][nv][nv_p]
         double *wTij = wTab + (size_t)pc * nv * nv_p;                // [no][pc][no_p]
+        // single-precision mode (gemm_tc.cu): every operand is three bf16 planes with rows padded to 8 elements;
+        // K' stays FP64 (the chunks are summed in FP64), X' FP64 is not needed
+        const long long nv_q = (nv + 7) & ~7, no_q = (no + 7) & ~7;
+        long long ldK = 0, plX = 0, plM = 0, plTab = 0, plTij = 0;
+        unsigned short *qX = nullptr, *qM = nullptr, *qTab = nullptr, *qTij = nullptr;      // bf16 bit patterns
+        if (f32) {
+            auto need = [&](long long c) {
+                return 8 * (size_t)m * no * nv_p + 6 * ((size_t)m * no * nv_q + (size_t)m * nv * c * no_q + (size_t)c * nv * nv_q + (size_t)no * c * no_q) + 64;
+            };
+            while (pc > 1 && need(pc) > ctx->plan.arena_bytes) --pc;
+            if (need(pc) > ctx->plan.arena_bytes) { risp_set_error(ctx, "risp_matvec: work space too small for the single-precision K contractions"); return RISP_ENOMEM; }
+            ldK = (long long)pc * no_q;
+            plX = (long long)m * no * nv_q; plM = (long long)m * nv * ldK; plTab = (long long)pc * nv * nv_q; plTij = (long long)no * ldK;
+            wKk = ctx->w_arena;
+            qX = (unsigned short *)(((size_t)(wKk + (size_t)m * no * nv_p) + 15) & ~(size_t)15);
+            qM = qX + 3 * plX; qTab = qM + 3 * plM; qTij = qTab + 3 * plTab;
+            if (no_q != no) {       // the padding columns j of (P, j) enter Eq. 23 as 0 * M: both must be finite, T_ij's must be zero
+                RISP_CUDA_TRY(cudaMemsetAsync(qM, 0, (size_t)3 * plM * 2, st));
+                RISP_CUDA_TRY(cudaMemsetAsync(qTij, 0, (size_t)3 * plTij * 2, st));
+            }
+            RISP_CUDA_TRY(risp_split_rows_bf3(X + (size_t)ctx->occK0 * nvir + ctx->virK0, nvir, (long long)m * no, nv, qX, nv_q, plX, no,
+                                              (long long)nocc * nvir, st)); ++launches;
+        } else
         if (nv_p != nv) {   // padding columns of X' must not carry NaNs of the J phase into the TMA boxes (they are never read
                             // as operands -- K = nv bounds the boxes -- but keep the buffers clean anyway)
             RISP_CUDA_TRY(cudaMemsetAsync(wXk, 0, (size_t)m * no * nv_p * sizeof(double), st));
         }
-        RISP_CUDA_TRY(risp_gather_window(X, wXk, m, nocc, nvir, ctx->occK0, no, ctx->virK0, nv, nv_p, st)); ++launches;
-        if (no_p != no) {
+        if (!f32) { RISP_CUDA_TRY(risp_gather_window(X, wXk, m, nocc, nvir, ctx->occK0, no, ctx->virK0, nv, nv_p, st)); ++launches; }
+        if (!f32 && no_p != no) {
             // the contraction index (P, j) of Eq. 23 runs over no_p per P: the padding row of M and the padding column of T_ij are zero
             RISP_CUDA_TRY(cudaMemset2DAsync(wM + (size_t)no * nv_p, (size_t)no_p * nv_p * 8, 0, (size_t)nv_p * 8, (size_t)m * pc, st));
             RISP_CUDA_TRY(cudaMemset2DAsync(wTij + no, (size_t)no_p * 8, 0, 8, (size_t)no * pc, st));
@@ -326,6 +351,30 @@ after_pass1:
                 ++nhost_seen;
             } else {
                 pij = ctx->d_TijP + (size_t)c.p0 * ctx->tri_o; pab = ctx->d_TabP + (size_t)c.p0 * ctx->tri_v;
+            }
+            if (f32) {
+                // packed lower triangles -> bf16 planes of T_ab [P][a][b] and T_ij [i][(P, j)]
+                RISP_CUDA_TRY(risp_expand_sym_bf3(pab, ctx->tri_v, nv, c.np, qTab, nv_q, (long long)nv * nv_q, plTab, st)); ++launches;
+                RISP_CUDA_TRY(risp_expand_sym_bf3(pij, ctx->tri_o, no, c.np, qTij, ldK, no_q, plTij, st)); ++launches;
+                if (c.host) RISP_CUDA_TRY(cudaEventRecord(ctx->evStageFree[buf], st));
+                if (ci == 0) RISP_CUDA_TRY(cudaEventRecord(ev[11], st));
+                // Eq. 22, stored transposed: Mt[mi][a][(P, j)] = sum_b X'[(mi, j)][b] T_ab^P[a][b]
+                TcGemmDesc d;
+                d.M = m * no; d.N = nv; d.K = nv; d.nb = c.np;
+                d.A = qX; d.lda = nv_q; d.planeA = plX; d.sA = 0;
+                d.B = qTab; d.ldb = nv_q; d.planeB = plTab; d.sB = (long long)nv * nv_q;
+                d.C = qM; d.ldc = ldK; d.sC = no_q; d.planeC = plM; d.out_kind = 1; d.rpg = no; d.gstride = (long long)nv * ldK; d.accumulate = 0; d.seg_kb = ctx->tc_seg_kb;
+                RISP_CUDA_TRY(risp_tcgemm(d, st)); ++launches;
+                if (ci == 0) RISP_CUDA_TRY(cudaEventRecord(ev[9], st));
+                // Eq. 23, stored transposed: K'[mi][i][a] (+)= sum_{(P, j)} Mt[mi][a][(P, j)] T_ij[i][(P, j)]
+                TcGemmDesc e;
+                e.M = nv; e.N = no; e.K = (int)(c.np * no_q); e.nb = m;
+                e.A = qM; e.lda = ldK; e.planeA = plM; e.sA = (long long)nv * ldK;
+                e.B = qTij; e.ldb = ldK; e.planeB = plTij; e.sB = 0;
+                e.C = wKk; e.ldc = nv_p; e.sC = (long long)no * nv_p; e.planeC = 0; e.out_kind = 0; e.rpg = 0; e.gstride = 0; e.accumulate = ci != 0; e.seg_kb = ctx->tc_seg_kb;
+                RISP_CUDA_TRY(risp_tcgemm(e, st)); ++launches;
+                if (ci == 0) { RISP_CUDA_TRY(cudaEventRecord(ev[10], st)); ctx->tim.first_chunk_naux = c.np; }
+                continue;
             }
             // packed lower triangles -> T_ab [P][a][b] and T_ij [i][(P, j)]
             RISP_CUDA_TRY(risp_expand_sym(pab, ctx->tri_v, nv, c.np, wTab, nv_p, (long long)nv * nv_p, st)); ++launches;
