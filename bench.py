@@ -122,6 +122,54 @@ class OracleSample:
                 f"{self.fJ:.1f} / {self.fK:.1f} to the whole auxiliary basis; tensor build of the sample ({self.t_build:.1f} s) excluded like risp_setup")
 
 
+def _fp32_mode(torch, ctx, X, sigma, flush, stream, steps, warmup, m, d, small):
+    """risp_matvec with RISP_PRECISION_FP32_K: Eq. 22-23 on the tcgen05 tensor cores (three bf16 terms per operand, six MMAs per
+    k step, FP32 accumulation).  Reported beside the FP64 headline, never instead of it."""
+    no, nv, nK = d["noccK"], d["nvirK"], d["nauxK"]
+    K64 = torch.from_numpy(ctx.stage("K", m)).to(X.device) if small else None      # K' of the FP64 step just timed
+    sig64 = sigma.clone() if small else sigma.view(m, -1)[:, ::997].clone()
+    ctx.set_precision(1)
+    try:
+        for _ in range(warmup):
+            ctx.matvec(X, sigma)
+        torch.cuda.synchronize()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        phase = {}
+        for a, b in evs:
+            flush.zero_()
+            a.record(stream)
+            ctx.matvec(X, sigma)
+            b.record(stream)
+            b.synchronize()
+            for k, v in ctx.timings().items():
+                phase[k] = phase.get(k, 0.0) + (v if isinstance(v, float) else 0.0)
+        tim = ctx.timings()
+        t_dev = sum(a.elapsed_time(b) for a, b in evs) * 1e-3
+        s32 = sigma if small else sigma.view(m, -1)[:, ::997]
+        out = dict(value=m * steps / t_dev, unit=UNIT, ms_per_step=1e3 * t_dev / steps, dtype="f64 integrals, J and Davidson algebra; K contractions "
+                   "bf16x3 operands (24 significand bits) with FP32 accumulation on tcgen05, aux chunks summed in FP64",
+                   phases_ms={k: round(1e3 * v / steps, 4) for k, v in phase.items() if k not in ("kernel_launches", "first_chunk_naux")},
+                   gpu_launches=tim["kernel_launches"] * steps,
+                   sigma_rel_diff_vs_fp64=float((s32 - sig64).norm() / sig64.norm()))
+        if small:
+            K32 = torch.from_numpy(ctx.stage("K", m)).to(X.device)
+            out["K_rel_diff_vs_fp64"] = float((K32 - K64).norm() / K64.norm())
+            del K32
+        npf = tim["first_chunk_naux"]
+        t1, t2 = phase["k_gemm1"] / steps, phase["k_gemm2"] / steps
+        f1, f2 = 2.0 * m * no * nv * nv * npf, 2.0 * m * no * no * nv * npf
+        # the tensor cores execute six bf16 MMAs per product: `achieved` is the executed bf16 rate, the peak is the measured bf16 one
+        out["roofline"] = dict(bound="tensor", kernel="tcgemm_bf16x3_kernel (Eq. 22, M^P = X' T_ab^P)", unit="TFLOP/s", achieved=6 * f1 / t1 / 1e12,
+                               fp32_equivalent_tflops=f1 / t1 / 1e12, launch_ms=1e3 * t1, flops_per_launch_fp32=f1)
+        out["roofline_eq23"] = dict(bound="tensor", kernel="tcgemm_bf16x3_kernel (Eq. 23, K' += T_ij M)", unit="TFLOP/s", achieved=6 * f2 / t2 / 1e12,
+                                    fp32_equivalent_tflops=f2 / t2 / 1e12, launch_ms=1e3 * t2, flops_per_launch_fp32=f2)
+        out["k_phase_fp32_equivalent_tflops"] = 2.0 * m * nK * no * nv * (no + nv) / (phase["k_total"] / steps) / 1e12
+        return out
+    finally:
+        ctx.set_precision(0)
+        del K64, sig64
+
+
 def run_reference(args):
     """The CPU oracle as the reference arm: sigma-builds/s of the oracle on a bounded sample of the same workload."""
     rank = int(os.environ.get("RANK", "0"))
@@ -208,6 +256,11 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
     tim = ctx.timings()
     d = ctx.dims()
     launches = tim["kernel_launches"] * steps
+
+    # ---- the single-precision mode of the K contractions, same batch, same timing rules
+    fp32 = None
+    if rank == 0 and world == 1 and not args.no_fp32 and d["nauxK"] > 0 and (cfg <= 3 or args.fp32_large):
+        fp32 = _fp32_mode(torch, ctx, X, sigma, flush, stream, steps, warmup, m, d, small=cfg <= 3)
 
     # ---- end to end: pinned host buffers through risp_matvec_host
     fp = None
@@ -325,6 +378,13 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
             ],
             flops_per_step=flops_step,
         )
+        if fp32 is not None:
+            pk16 = pk["bf16_sustained"] if fp32["ms_per_step"] >= 1000.0 else pk["bf16"]
+            for key in ("roofline", "roofline_eq23"):
+                r = fp32[key]
+                r["peak"] = pk16; r["frac"] = r["achieved"] / pk16
+                r["peak_source"] = f"{pk['src']} bf16 cuBLAS throughput ({'sustained' if fp32['ms_per_step'] >= 1000.0 else 'burst'})"
+            line["fp32_mode"] = fp32
         smp = None
         if want_cpu and world == 1 and cfg <= 4:
             ms_ = min(m, 30 if cfg <= 2 else args.ref_vectors)
@@ -372,6 +432,15 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
                 sv["cpu_oracle_estimate"] = dict(wall_s=info["n_sigma"] / line["cpu_baseline"]["value"], cores=os.cpu_count(),
                                                  note="n_sigma of the GPU solve / sampled oracle sigma-builds/s; the oracle's own Davidson is not run at this size")
             line["solve"] = sv
+            if fp32 is not None and not big_dim:
+                ctx.set_precision(1)
+                try:
+                    om32, _, i32 = ctx.tda_solve(s["nroots"], want_vectors=False, flags=flags & ~32, **kw)
+                    fp32["solve"] = dict(wall_s=i32["sec_total"], matvec_s=i32["sec_matvec"], iterations=i32["iterations"], n_sigma=i32["n_sigma"],
+                                         converged=i32["converged"], resid_max=float(max(i32["resid"])), tol=args.solve_tol,
+                                         max_abs_diff_vs_fp64_solve_ev=float(np.abs(np.asarray(om32) - np.asarray(omega)).max() * HARTREE_EV))
+                finally:
+                    ctx.set_precision(0)
         res = line
     ctx.close()
     del ctx
@@ -445,6 +514,8 @@ def main():
     ap.add_argument("--solve-fp32-host", action="store_true", help="RISP_SOLVE_HOST_FP32 for the solve of the 1000/3000-atom systems")
     ap.add_argument("--progress-file", default="", help="write the solve record to this file as soon as risp_tda_solve returns")
     ap.add_argument("--no-solve", action="store_true", help="skip the 15-root risp_tda_solve")
+    ap.add_argument("--no-fp32", action="store_true", help="skip the single-precision-mode leg (RISP_PRECISION_FP32_K)")
+    ap.add_argument("--fp32-large", action="store_true", help="run the single-precision-mode leg on the 1000/3000-atom systems too")
     ap.add_argument("--solve", action="store_true", help="(default) kept for compatibility")
     ap.add_argument("--also", default="4", help="comma separated further configs run briefly after the main one (1 GPU only); '' for none")
     ap.add_argument("--also-budget-s", type=float, default=420.0, help="an `also` config starts only if the run is younger than this")

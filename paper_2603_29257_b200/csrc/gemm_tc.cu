@@ -96,7 +96,19 @@ struct TcArgs {
     void *C; long long ldc, sC, planeC; int rpg; long long gstride; int accumulate;
     int tiles_m, tiles_n;
     int seg_kb;                  // stages (of 32 k) per accumulation segment
+    int gm;                      // row tiles per group of the tile order
 };
+
+// tile order inside one batch entry: groups of gm row tiles x all column tiles, m fastest inside a group, so that one wave of CTAs
+// works on operands that stay in L2 (the same order as gemm_tma.cu)
+__device__ __forceinline__ void tile_coords(int tt, int tiles_m, int tiles_n, int gm, int &tm, int &tn)
+{
+    const int per_group = gm * tiles_n;
+    const int g = tt / per_group, r = tt - g * per_group;
+    const int rows = min(gm, tiles_m - g * gm);
+    tm = g * gm + r % rows;
+    tn = r / rows;
+}
 
 __device__ __forceinline__ void split3(float v, __nv_bfloat16 &b1, __nv_bfloat16 &b2, __nv_bfloat16 &b3)
 {
@@ -147,7 +159,8 @@ __global__ void __launch_bounds__(NT, 1) tcgemm_bf16x3_kernel(const __grid_const
             int slot = 0; unsigned par = 1;
             for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
                 const int z = tile / tiles_per_batch, tt = tile % tiles_per_batch;
-                const int tm = tt % g.tiles_m, tn = tt / g.tiles_m;
+                int tm, tn;
+                tile_coords(tt, g.tiles_m, g.tiles_n, g.gm, tm, tn);
                 for (int kb = 0; kb < nk; ++kb) {
                     mbar_wait(empty0 + 8 * slot, par);
                     const unsigned fb = full0 + 8 * slot, dst = smem_u + slot * STAGE_BYTES;
@@ -205,7 +218,8 @@ __global__ void __launch_bounds__(NT, 1) tcgemm_bf16x3_kernel(const __grid_const
         int acc = 0; unsigned apar = 0;
         for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
             const int z = tile / tiles_per_batch, tt = tile % tiles_per_batch;
-            const int tm = tt % g.tiles_m, tn = tt / g.tiles_m;
+            int tm, tn;
+            tile_coords(tt, g.tiles_m, g.tiles_n, g.gm, tm, tn);
             float run[128];
 #pragma unroll
             for (int c = 0; c < 128; ++c) run[c] = 0.f;
@@ -399,6 +413,7 @@ cudaError_t risp_tcgemm(const TcGemmDesc &d, cudaStream_t st)
     if (!make_map(enc, &ma, (const __nv_bfloat16 *)d.A, d.M, d.K, d.lda, d.planeA, d.sA, d.nb, BM)) return cudaErrorNotSupported;
     if (!make_map(enc, &mb, (const __nv_bfloat16 *)d.B, d.N, d.K, d.ldb, d.planeB, d.sB, d.nb, g.BN)) return cudaErrorNotSupported;
     const int grid = (int)std::min<long long>(total, sms[dev & 63]);
+    g.gm = std::max(1, std::min(g.tiles_m, (sms[dev & 63] + g.tiles_n - 1) / g.tiles_n));
     tcgemm_bf16x3_kernel<<<grid, NT, SMEM_BYTES, st>>>(ma, mb, g);
     return cudaGetLastError();
 }
