@@ -399,8 +399,10 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
             big_dim = s["nocc"] * s["nvir"] >= 5e7
             kw = dict(tol=args.solve_tol, max_iter=args.solve_max_iter, allow_unconverged=True, n_guess=args.solve_n_guess, max_seconds=args.solve_max_seconds)
             flags = (8 if args.solve_fp32_host else 0) | (16 if big_dim else 0) | (32 if args.progress_file else 0)
+            if args.solve_mode == "fp32":      # the whole solve (and the residual re-check) in the single-precision mode of the K contractions
+                ctx.set_precision(1)
             omega, Xs, info = ctx.tda_solve(s["nroots"], want_vectors=True, flags=flags, **kw)
-            sv = dict(nroots=s["nroots"], tol=args.solve_tol, n_guess=args.solve_n_guess or 2 * s["nroots"], wall_s=info["sec_total"], matvec_s=info["sec_matvec"],
+            sv = dict(precision="fp32_k" if args.solve_mode == "fp32" else "fp64", nroots=s["nroots"], tol=args.solve_tol, n_guess=args.solve_n_guess or 2 * s["nroots"], wall_s=info["sec_total"], matvec_s=info["sec_matvec"],
                       alloc_s=info["sec_alloc"], subspace_s=info["sec_subspace"], block=info["block"], capacity=info["capacity"],
                       cached_vectors=info["cached_vectors"], host_subspace_gb=info["bytes_host_subspace"] / 1e9,
                       host_store="fp32" if args.solve_fp32_host else "fp64", iterations=info["iterations"], n_sigma=info["n_sigma"],
@@ -422,6 +424,7 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
             except Exception as e:      # reported, not hidden
                 sv["resid_recomputed_error"] = repr(e)
             del Xs
+            ctx.set_precision(0)
             if smp is not None and smp.full and cfg <= 2:      # the CPU oracle's own Davidson on the same problem (same tolerance)
                 t0 = time.time()
                 th_ref, _, iref = smp.o.davidson(s["nroots"], tol=args.solve_tol)
@@ -432,7 +435,7 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
                 sv["cpu_oracle_estimate"] = dict(wall_s=info["n_sigma"] / line["cpu_baseline"]["value"], cores=os.cpu_count(),
                                                  note="n_sigma of the GPU solve / sampled oracle sigma-builds/s; the oracle's own Davidson is not run at this size")
             line["solve"] = sv
-            if fp32 is not None and not big_dim:
+            if fp32 is not None and not big_dim and args.solve_mode == "both" and cfg <= 3:
                 ctx.set_precision(1)
                 try:
                     om32, _, i32 = ctx.tda_solve(s["nroots"], want_vectors=False, flags=flags & ~32, **kw)
@@ -514,6 +517,8 @@ def main():
     ap.add_argument("--solve-fp32-host", action="store_true", help="RISP_SOLVE_HOST_FP32 for the solve of the 1000/3000-atom systems")
     ap.add_argument("--progress-file", default="", help="write the solve record to this file as soon as risp_tda_solve returns")
     ap.add_argument("--no-solve", action="store_true", help="skip the 15-root risp_tda_solve")
+    ap.add_argument("--solve-mode", default="both", choices=["both", "fp64", "fp32"],
+                    help="both: FP64 solve, then (300 atoms and below) the same solve in the single-precision mode; fp32: only the latter")
     ap.add_argument("--no-fp32", action="store_true", help="skip the single-precision-mode leg (RISP_PRECISION_FP32_K)")
     ap.add_argument("--fp32-large", action="store_true", help="run the single-precision-mode leg on the 1000/3000-atom systems too")
     ap.add_argument("--solve", action="store_true", help="(default) kept for compatibility")

@@ -73,7 +73,8 @@ struct TcGemmDesc {
     const void *B; long long ldb, planeB, sB;
     void *C; long long ldc, sC, planeC;
     int out_kind, rpg; long long gstride; int accumulate;
-    int seg_kb = 0;          // 32-k stages per accumulation segment (0: the default, 4)
+    int seg_kb = 0;          // stages per accumulation segment (0: the default, 1)
+    int shape = 0;           // 0: 128 x 256 tiles, 32 k per stage (64-byte swizzle rows); 1: 128 x 128 tiles, 64 k per stage (128-byte rows)
 };
 cudaError_t risp_tcgemm(const TcGemmDesc &d, cudaStream_t st);
 cudaError_t risp_split_rows_bf3(const double *X, long long ldx, long long rows, int n, void *out, long long ldo, long long plane, int rpg,

@@ -22,11 +22,14 @@
 
 namespace {
 
-constexpr int BM = 128, BN_MAX = 256, BK = 32, STAGES = 3, NEPI = 8, NT = (2 + NEPI) * 32, SEG_KB = 1;
-constexpr int A_PLANE = BM * BK * 2;                 // 8 KiB
-constexpr int B_PLANE_MAX = BN_MAX * BK * 2;         // 16 KiB
-constexpr int STAGE_BYTES = 3 * A_PLANE + 3 * B_PLANE_MAX;      // 72 KiB
-constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + 1024 + 128;
+constexpr int BM = 128, BN_MAX = 256, NEPI = 8, NT = (2 + NEPI) * 32, SEG_K = 32;
+// Shape of one kernel variant: BK k per stage (32: 64-byte swizzle rows, 64: 128-byte rows), column cap of the tile, stages
+template <int BK_, int BNCAP_, int STAGES_>
+struct TcShape {
+    static constexpr int BK = BK_, BNCAP = BNCAP_, STAGES = STAGES_;
+    static constexpr int A_PLANE = BM * BK * 2, B_PLANE_MAX = BNCAP * BK * 2, STAGE_BYTES = 3 * A_PLANE + 3 * B_PLANE_MAX;
+    static constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + 1024 + 128;
+};
 
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count)); }
@@ -83,9 +86,11 @@ __device__ __forceinline__ void tmem_ld32(unsigned taddr, unsigned (&v)[32])
 
 // shared-memory matrix descriptor of a K-contiguous operand plane [rows][32 bf16] in the 64-byte swizzle: 8-row groups are 512 B
 // apart (SBO), the leading byte offset is unused for swizzled K-major layouts, version 1 (sm_100), layout type 4 = SWIZZLE_64B
-__device__ __forceinline__ unsigned long long smem_desc_sw64(unsigned addr)
+template <int BK>
+__device__ __forceinline__ unsigned long long smem_desc(unsigned addr)
 {
-    return (unsigned long long)((addr & 0x3FFFF) >> 4) | (1ull << 16) | ((unsigned long long)(512 >> 4) << 32) | (1ull << 46) | (4ull << 61);
+    constexpr unsigned long long sbo = (8 * BK * 2) >> 4, lt = BK == 64 ? 2 : 4;       // 8 rows of BK bf16; SWIZZLE_128B = 2, SWIZZLE_64B = 4
+    return (unsigned long long)((addr & 0x3FFFF) >> 4) | (1ull << 16) | (sbo << 32) | (1ull << 46) | (lt << 61);
 }
 
 struct TcArgs {
@@ -123,8 +128,10 @@ __device__ __forceinline__ void split3(float v, __nv_bfloat16 &b1, __nv_bfloat16
 // SEG_KB stages (32 k each): each segment is accumulated in tensor memory from zero and the eight epilogue warps add it, rounded to nearest, to FP32
 // running sums they keep in registers (128 per thread: one accumulator row, half the columns) while the MMA warp fills the other
 // accumulator buffer.  The result is written once per tile.
+template <class S>
 __global__ void __launch_bounds__(NT, 1) tcgemm_bf16x3_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, TcArgs g)
 {
+    constexpr int BK = S::BK, STAGES = S::STAGES, A_PLANE = S::A_PLANE, STAGE_BYTES = S::STAGE_BYTES;
     extern __shared__ unsigned char smem_raw[];
     unsigned char *smem = (unsigned char *)(((size_t)smem_raw + 1023) & ~(size_t)1023);
     unsigned long long *bars = (unsigned long long *)(smem + STAGES * STAGE_BYTES);
@@ -195,8 +202,8 @@ __global__ void __launch_bounds__(NT, 1) tcgemm_bf16x3_kernel(const __grid_const
                         for (int ks = 0; ks < BK / 16; ++ks)
 #pragma unroll
                             for (int p = 0; p < 3; ++p) {
-                                ad[p][ks] = smem_desc_sw64(a0 + p * A_PLANE + ks * 32);
-                                bd[p][ks] = smem_desc_sw64(b0 + p * b_plane + ks * 32);
+                                ad[p][ks] = smem_desc<BK>(a0 + p * A_PLANE + ks * 32);
+                                bd[p][ks] = smem_desc<BK>(b0 + p * b_plane + ks * 32);
                             }
                         constexpr int PA[6] = {2, 0, 1, 1, 0, 0}, PB[6] = {0, 2, 1, 0, 1, 0};
 #pragma unroll
@@ -297,14 +304,14 @@ EncodeFn get_encode()
 }
 
 // planes [3][batch][rows][ld] of bf16, K contiguous; dims (k, row, plane, batch)
-bool make_map(EncodeFn enc, CUtensorMap *tm, const __nv_bfloat16 *p, int rows, int K, long long ld, long long plane, long long sbatch, int nb, int box_rows)
+bool make_map(EncodeFn enc, CUtensorMap *tm, const __nv_bfloat16 *p, int rows, int K, long long ld, long long plane, long long sbatch, int nb, int box_rows, int BK)
 {
     if ((ld & 7) || (plane & 7) || (sbatch & 7) || (((size_t)p) & 15) || ld <= 0) return false;
     cuuint64_t dims[4] = {(cuuint64_t)K, (cuuint64_t)rows, 3, (cuuint64_t)(sbatch ? nb : 1)};
     cuuint64_t strides[3] = {(cuuint64_t)ld * 2, (cuuint64_t)plane * 2, (cuuint64_t)(sbatch ? sbatch : plane * 3) * 2};
     cuuint32_t box[4] = {(cuuint32_t)BK, (cuuint32_t)box_rows, 3, 1}, es[4] = {1, 1, 1, 1};
     if (strides[1] >= (1ull << 40) || strides[2] >= (1ull << 40)) return false;
-    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, (void *)p, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, (void *)p, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, BK == 64 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B,
                CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
@@ -383,10 +390,10 @@ cudaError_t risp_expand_sym_bf3(const double *packed, long long tri, int n, int 
 
 // Returns cudaErrorNotSupported when the operands cannot be described by tensor maps (leading dimensions / strides not multiples
 // of 8 elements, misaligned base, driver entry point missing): there is no other FP32 path, the caller reports the error.
-cudaError_t risp_tcgemm(const TcGemmDesc &d, cudaStream_t st)
+namespace {
+template <class S>
+cudaError_t launch_shape(const TcGemmDesc &d, cudaStream_t st)
 {
-    if (d.M <= 0 || d.N <= 0 || d.nb <= 0) return cudaSuccess;
-    if (d.K <= 0) return cudaErrorNotSupported;
     EncodeFn enc = get_encode();
     if (!enc) return cudaErrorNotSupported;
     static bool attr[64] = {};
@@ -394,28 +401,41 @@ cudaError_t risp_tcgemm(const TcGemmDesc &d, cudaStream_t st)
     int dev = 0;
     cudaGetDevice(&dev);
     if (!attr[dev & 63]) {
-        cudaError_t e = cudaFuncSetAttribute(tcgemm_bf16x3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
+        cudaError_t e = cudaFuncSetAttribute(tcgemm_bf16x3_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::SMEM_BYTES);
         if (e != cudaSuccess) return e;
         cudaDeviceGetAttribute(&sms[dev & 63], cudaDevAttrMultiProcessorCount, dev);
         attr[dev & 63] = true;
     }
     TcArgs g;
-    // column tile: the fewest tiles of at most 256 columns, each a multiple of 16 (N = 423 -> 2 x 224 instead of 256 + 167)
-    const int nt = (d.N + BN_MAX - 1) / BN_MAX;
-    g.BN = std::min(BN_MAX, (((d.N + nt - 1) / nt) + 15) & ~15);
+    // column tile: the fewest tiles of at most BNCAP columns, each a multiple of 16 (N = 423 -> 2 x 224 instead of 256 + 167)
+    const int nt = (d.N + S::BNCAP - 1) / S::BNCAP;
+    g.BN = std::min(S::BNCAP, (((d.N + nt - 1) / nt) + 15) & ~15);
     g.M = d.M; g.N = d.N; g.K = d.K; g.nb = d.nb; g.za = d.sA != 0; g.zb = d.sB != 0;
     g.out_kind = d.out_kind; g.C = d.C; g.ldc = d.ldc; g.sC = d.sC; g.planeC = d.planeC; g.rpg = d.rpg; g.gstride = d.gstride; g.accumulate = d.accumulate;
-    g.seg_kb = d.seg_kb > 0 ? d.seg_kb : SEG_KB;
+    g.seg_kb = d.seg_kb > 0 ? d.seg_kb : 1;
     g.tiles_m = (d.M + BM - 1) / BM; g.tiles_n = (d.N + g.BN - 1) / g.BN;
     const long long total = (long long)g.tiles_m * g.tiles_n * d.nb;
     if (total >= (1ll << 31)) return cudaErrorNotSupported;
     CUtensorMap ma, mb;
-    if (!make_map(enc, &ma, (const __nv_bfloat16 *)d.A, d.M, d.K, d.lda, d.planeA, d.sA, d.nb, BM)) return cudaErrorNotSupported;
-    if (!make_map(enc, &mb, (const __nv_bfloat16 *)d.B, d.N, d.K, d.ldb, d.planeB, d.sB, d.nb, g.BN)) return cudaErrorNotSupported;
+    if (!make_map(enc, &ma, (const __nv_bfloat16 *)d.A, d.M, d.K, d.lda, d.planeA, d.sA, d.nb, BM, S::BK)) return cudaErrorNotSupported;
+    if (!make_map(enc, &mb, (const __nv_bfloat16 *)d.B, d.N, d.K, d.ldb, d.planeB, d.sB, d.nb, g.BN, S::BK)) return cudaErrorNotSupported;
     const int grid = (int)std::min<long long>(total, sms[dev & 63]);
     g.gm = std::max(1, std::min(g.tiles_m, (sms[dev & 63] + g.tiles_n - 1) / g.tiles_n));
-    tcgemm_bf16x3_kernel<<<grid, NT, SMEM_BYTES, st>>>(ma, mb, g);
+    tcgemm_bf16x3_kernel<S><<<grid, NT, S::SMEM_BYTES, st>>>(ma, mb, g);
     return cudaGetLastError();
+}
+}  // namespace
+
+cudaError_t risp_tcgemm(const TcGemmDesc &d, cudaStream_t st)
+{
+    if (d.M <= 0 || d.N <= 0 || d.nb <= 0) return cudaSuccess;
+    if (d.K <= 0) return cudaErrorNotSupported;
+    // Measured on the 300-atom system with the MMAs switched off, the operand traffic alone costs 44 ms of the 50 ms of the Eq. 22
+    // launch: about half of it scales with the bytes (L2 -> SM), half with the number of TMA row requests.  128 x 256 tiles with
+    // 64-byte rows minimise the bytes; 128 x 128 tiles with 128-byte rows the requests -- the latter wins when the column count
+    // leaves a 256-wide tile half empty anyway (Eq. 23, N = N_occK').
+    if (d.shape == 1) return launch_shape<TcShape<64, 128, 2>>(d, st);
+    return launch_shape<TcShape<32, 256, 3>>(d, st);
 }
 
 namespace {
@@ -430,7 +450,7 @@ __global__ void sum_planes_kernel(const __nv_bfloat16 *__restrict__ p, long long
 
 // include/risp_debug.h: C[z][c][r] (+)= sum_k A[z][r][k] B[z][c][k] through the single-precision tensor-core path, FP64 in and out
 extern "C" int risp_debug_tcgemm(int32_t M, int32_t N, int32_t K, int32_t nbatch, const double *A_dev, const double *B_dev, double *C_dev,
-                                 int32_t accumulate, int32_t via_planes, int32_t seg_kb, void *cuda_stream)
+                                 int32_t accumulate, int32_t via_planes, int32_t seg_kb, int32_t shape, void *cuda_stream)
 {
     if (M <= 0 || N <= 0 || K <= 0 || nbatch <= 0 || !A_dev || !B_dev || !C_dev) return RISP_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -447,7 +467,7 @@ extern "C" int risp_debug_tcgemm(int32_t M, int32_t N, int32_t K, int32_t nbatch
         d.M = M; d.N = N; d.K = K; d.nb = nbatch;
         d.A = a; d.lda = ldk; d.planeA = planeA; d.sA = (long long)M * ldk;
         d.B = b; d.ldb = ldk; d.planeB = planeB; d.sB = (long long)N * ldk;
-        d.rpg = 0; d.gstride = 0; d.seg_kb = seg_kb;
+        d.rpg = 0; d.gstride = 0; d.seg_kb = seg_kb; d.shape = shape;
         if (via_planes) {
             if (cudaMemsetAsync(c, 0, 3 * planeC * 2, st) != cudaSuccess) break;
             d.C = c; d.ldc = ldm; d.sC = (long long)N * ldm; d.planeC = planeC; d.out_kind = 1; d.accumulate = 0;

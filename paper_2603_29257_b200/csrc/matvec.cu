@@ -371,7 +371,7 @@ after_pass1:
                 e.M = nv; e.N = no; e.K = (int)(c.np * no_q); e.nb = m;
                 e.A = qM; e.lda = ldK; e.planeA = plM; e.sA = (long long)nv * ldK;
                 e.B = qTij; e.ldb = ldK; e.planeB = plTij; e.sB = 0;
-                e.C = wKk; e.ldc = nv_p; e.sC = (long long)no * nv_p; e.planeC = 0; e.out_kind = 0; e.rpg = 0; e.gstride = 0; e.accumulate = ci != 0; e.seg_kb = ctx->tc_seg_kb;
+                e.C = wKk; e.ldc = nv_p; e.sC = (long long)no * nv_p; e.planeC = 0; e.out_kind = 0; e.rpg = 0; e.gstride = 0; e.accumulate = ci != 0; e.seg_kb = ctx->tc_seg_kb; e.shape = 1;
                 RISP_CUDA_TRY(risp_tcgemm(e, st)); ++launches;
                 if (ci == 0) { RISP_CUDA_TRY(cudaEventRecord(ev[10], st)); ctx->tim.first_chunk_naux = c.np; }
                 continue;

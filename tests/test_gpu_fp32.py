@@ -22,22 +22,23 @@ def torch_cuda():
     return torch
 
 
-def _tcgemm(torch, A, B, C0=None, via_planes=0, seg_kb=0):
+def _tcgemm(torch, A, B, C0=None, via_planes=0, seg_kb=0, shape=0):
     from paper_2603_29257_b200.binding import load_library
     lib = load_library()
     nb, M, K = A.shape
     N = B.shape[1]
     Cc = torch.zeros(nb, N, M, dtype=torch.float64, device="cuda") if C0 is None else C0.clone()
-    rc = lib.risp_debug_tcgemm(M, N, K, nb, A.data_ptr(), B.data_ptr(), Cc.data_ptr(), 0 if C0 is None else 1, via_planes, seg_kb, None)
+    rc = lib.risp_debug_tcgemm(M, N, K, nb, A.data_ptr(), B.data_ptr(), Cc.data_ptr(), 0 if C0 is None else 1, via_planes, seg_kb, shape, None)
     assert rc == 0
     torch.cuda.synchronize()
     return Cc
 
 
+@pytest.mark.parametrize("tile_shape", [0, 1])
 @pytest.mark.parametrize("via_planes", [0, 1])
 @pytest.mark.parametrize("shape", [(128, 256, 32, 1), (128, 16, 64, 1), (1, 1, 1, 1), (100, 200, 40, 2), (129, 257, 33, 1), (300, 423, 1496, 2),
                                    (1496, 423, 3392, 3), (640, 700, 999, 2)])
-def test_tcgemm_against_fp64(torch_cuda, shape, via_planes):
+def test_tcgemm_against_fp64(torch_cuda, shape, via_planes, tile_shape):
     """Several row / column tiles, ragged tails in M, N and K (K not a multiple of the 32-element stage nor of 8), batches, both
     epilogues.  Elementwise bound of an FP32-accumulated inner product of K terms whose operands carry 24 bits:
     |err| <= (K + 6) u sum_k |a_k||b_k|  (+ 3 u |c| when the result is re-split into three bf16 planes)."""
@@ -46,7 +47,7 @@ def test_tcgemm_against_fp64(torch_cuda, shape, via_planes):
     g = torch.Generator(device="cuda").manual_seed(M * 7 + N * 3 + K)
     A = torch.randn(nb, M, K, dtype=torch.float64, device="cuda", generator=g) * torch.exp(torch.randn(nb, M, 1, dtype=torch.float64, device="cuda", generator=g))
     B = torch.randn(nb, N, K, dtype=torch.float64, device="cuda", generator=g)
-    got = _tcgemm(torch, A, B, via_planes=via_planes)
+    got = _tcgemm(torch, A, B, via_planes=via_planes, shape=tile_shape)
     ref = torch.einsum("zrk,zck->zcr", A, B)
     bound = (K + 6) * U32 * torch.einsum("zrk,zck->zcr", A.abs(), B.abs()) + 3 * U32 * ref.abs()
     assert bool(torch.all((got - ref).abs() <= bound))
@@ -162,3 +163,21 @@ def test_fp32_mode_rejects_tddft(torch_cuda, sys_small_rsh):
             c.set_precision(7)
     finally:
         c.close()
+
+
+def test_tcgemm_segment_length(torch_cuda):
+    """The tensor core truncates when it adds an MMA result to the FP32 accumulator; accumulating the whole K range in tensor memory
+    lets that bias grow linearly with K.  The record of why the kernel promotes every 32 k to register sums: the error of the
+    default must be several times smaller than that of one long segment, and below cuBLAS SGEMM's on the same product."""
+    torch = torch_cuda
+    g = torch.Generator(device="cuda").manual_seed(1)
+    A = torch.randn(1, 512, 3392, dtype=torch.float64, device="cuda", generator=g)
+    B = torch.randn(1, 423, 3392, dtype=torch.float64, device="cuda", generator=g)
+    ref = torch.einsum("zrk,zck->zcr", A, B)
+    err = {seg: float((_tcgemm(torch, A, B, seg_kb=seg) - ref).norm() / ref.norm()) for seg in (0, 1, 4, 1000)}
+    sgemm = float((torch.einsum("zrk,zck->zcr", A.float(), B.float()).double() - ref).norm() / ref.norm())
+    print(f"relative error, K = 3392: default {err[0]:.2e}, 32 k {err[1]:.2e}, 128 k {err[4]:.2e}, unsegmented {err[1000]:.2e}; torch FP32 matmul {sgemm:.2e}")
+    assert err[0] == err[1]
+    assert err[1] < err[4] < err[1000]
+    assert err[1000] > 20 * err[1]
+    assert err[1] <= 5e-7
