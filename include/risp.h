@@ -234,6 +234,22 @@ int risp_transition_properties(risp_ctx *ctx, int32_t n, const double *X_dev, co
 int risp_tddft_solve(risp_ctx *ctx, int32_t nroots, const risp_solve_options *opt, double *omega_hartree, double *X_out, double *Y_out,
                      risp_solve_info *info);
 
+/* The single-precision-mode GEMM on its own, for callers that must not allocate (CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc):
+ *     C[c][r] (+)= sum_k A[r][k] B[c][k]        A_dev [M][K], B_dev [N][K], C_dev [N][M], contiguous DEVICE FP64,
+ * the arithmetic of RISP_PRECISION_FP32_K (operands as three bf16 terms, FP32 accumulation on the tcgen05 tensor cores, result
+ * added to C in FP64 when accumulate != 0).  It calls no cudaMalloc / cudaFree and no allocating library routine: the bf16
+ * operand planes, 6 (M + N) ceil8(K) bytes, live in ONE static device array of RISP_STATIC_SCRATCH_BYTES that every GPU which
+ * loads the library holds until exit.  Larger problems are rejected with RISP_EINVAL (text from risp_static_last_error()).
+ * Works on the CURRENT device, which cuda_stream must belong to; asynchronous on that stream.  All calls share the array: calls
+ * that overlap on the GPU (different streams, or host threads without ordering) race on it; calls on one stream do not.  Nothing
+ * in it has to be cleared between calls (every element a call reads it has written itself).  Needs no risp_ctx.
+ * Returns RISP_OK, RISP_EINVAL or RISP_ECUDA. */
+#define RISP_STATIC_SCRATCH_BYTES (16u << 20)
+int risp_tcgemm_static(int32_t M, int32_t N, int32_t K, const double *A_dev, const double *B_dev, double *C_dev, int32_t accumulate,
+                       void *cuda_stream);
+const char *risp_static_last_error(void); /* text of the calling thread's last risp_tcgemm_static failure ("" if none) */
+
 void risp_destroy(risp_ctx *ctx);
 const char *risp_last_error(const risp_ctx *ctx); /* static text if ctx == NULL */
 

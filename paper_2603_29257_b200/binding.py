@@ -106,6 +106,8 @@ def load_library():
                                      dbl, dbl, C.c_int, C.c_longlong, C.c_longlong, C.c_longlong, C.c_int, C.c_int, C.c_longlong, vp]
     lib.risp_debug_tcgemm.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp]
     lib.risp_debug_set_tc_segment.argtypes = [vp, C.c_int32]
+    lib.risp_tcgemm_static.argtypes = [C.c_int32, C.c_int32, C.c_int32, vp, vp, vp, C.c_int32, vp]
+    lib.risp_static_last_error.restype = C.c_char_p
     lib.risp_debug_sym_eig_lowest.argtypes = [C.c_int, C.c_int, vp, vp, vp]
     lib.risp_debug_force_plan.argtypes = [vp, C.c_int, C.c_int, C.c_int]
     lib.risp_debug_yardstick.argtypes = [vp, C.c_int, C.c_size_t, C.c_int, C.POINTER(dbl)]
@@ -318,3 +320,22 @@ class RispContext:
 def setup(sys: dict, **kw) -> RispContext:
     """risp_setup: build pair list, metrics, window and K tensors for `sys` (fields of `risp_system`)."""
     return RispContext(sys, **kw)
+
+
+STATIC_SCRATCH_BYTES = 16 << 20
+
+
+def tcgemm_static(A, B, C_out=None, accumulate=False, stream=None):
+    """`risp_tcgemm_static`: C[c][r] (+)= sum_k A[r][k] B[c][k] in the single-precision mode, allocating nothing inside the library
+    (A [M][K], B [N][K], C [N][M]: contiguous FP64 torch CUDA tensors; C_out is created here, by torch, when not given)."""
+    import torch
+    lib = load_library()
+    M, K = A.shape
+    N = B.shape[0]
+    if C_out is None:
+        C_out = torch.empty((N, M), dtype=torch.float64, device=A.device)
+    st = C.c_void_p(stream.cuda_stream) if stream is not None else C.c_void_p(torch.cuda.current_stream(A.device).cuda_stream)
+    rc = lib.risp_tcgemm_static(M, N, K, A.data_ptr(), B.data_ptr(), C_out.data_ptr(), 1 if accumulate else 0, st)
+    if rc != 0:
+        raise RispError(rc, lib.risp_static_last_error().decode())
+    return C_out

@@ -9,7 +9,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "librisp.so")
-SOURCES = ["gemm.cu", "gemm_tma.cu", "gemm_tc.cu", "eri_kernels.cu", "linalg.cu", "elementwise.cu", "setup.cu", "matvec.cu", "solve.cu", "solve_tddft.cu", "host_eig.cu", "yardstick.cu", "properties.cu", "api.cu"]
+SOURCES = ["gemm.cu", "gemm_tma.cu", "gemm_tc.cu", "gemm_tc_static.cu", "eri_kernels.cu", "linalg.cu", "elementwise.cu", "setup.cu", "matvec.cu", "solve.cu", "solve_tddft.cu", "host_eig.cu", "yardstick.cu", "properties.cu", "api.cu"]
 NVCC_FLAGS = ["-std=c++17", "--extended-lambda", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo",
               "-Xcompiler", "-fPIC"]
 
