@@ -159,9 +159,9 @@ def _fp32_mode(torch, ctx, X, sigma, flush, stream, steps, warmup, m, d, small):
         t1, t2 = phase["k_gemm1"] / steps, phase["k_gemm2"] / steps
         f1, f2 = 2.0 * m * no * nv * nv * npf, 2.0 * m * no * no * nv * npf
         # the tensor cores execute six bf16 MMAs per product: `achieved` is the executed bf16 rate, the peak is the measured bf16 one
-        out["roofline"] = dict(bound="tensor", kernel="tcgemm_bf16x3_kernel (Eq. 22, M^P = X' T_ab^P)", unit="TFLOP/s", achieved=6 * f1 / t1 / 1e12,
+        out["roofline"] = dict(bound="tensor", kernel="tcgemm2_bf16x3_kernel, CTA pair (Eq. 22, M^P = X' T_ab^P)", unit="TFLOP/s", achieved=6 * f1 / t1 / 1e12,
                                fp32_equivalent_tflops=f1 / t1 / 1e12, launch_ms=1e3 * t1, flops_per_launch_fp32=f1)
-        out["roofline_eq23"] = dict(bound="tensor", kernel="tcgemm_bf16x3_kernel (Eq. 23, K' += T_ij M)", unit="TFLOP/s", achieved=6 * f2 / t2 / 1e12,
+        out["roofline_eq23"] = dict(bound="tensor", kernel="tcgemm2_bf16x3_kernel, CTA pair (Eq. 23, K' += T_ij M)", unit="TFLOP/s", achieved=6 * f2 / t2 / 1e12,
                                     fp32_equivalent_tflops=f2 / t2 / 1e12, launch_ms=1e3 * t2, flops_per_launch_fp32=f2)
         out["k_phase_fp32_equivalent_tflops"] = 2.0 * m * nK * no * nv * (no + nv) / (phase["k_total"] / steps) / 1e12
         return out

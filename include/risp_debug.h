@@ -49,13 +49,14 @@ int risp_debug_oneel_ao(risp_ctx *ctx, const double *origin_bohr, double *out_ho
  * A [nbatch][M][K], B [nbatch][N][K], C [nbatch][N][M] contiguous.  via_planes != 0 routes the result through the three-bf16-plane
  * store that feeds Eq. 23; seg_kb = number of 32-k stages accumulated in tensor memory before the partial sum is added, rounded to
  * nearest, to the FP32 running sum in registers (0: the default of the library); shape 0: 128 x 256 tiles with 32 k per stage,
- * 1: 128 x 128 tiles with 64 k per stage.  Synchronous.  Returns RISP_OK, RISP_EINVAL,
+ * 1: 128 x 128 tiles with 64 k per stage, 2: CTA pair (cta_group::2) on a 256 x 256 tile with 32 k per stage.  Synchronous.  Returns RISP_OK, RISP_EINVAL,
  * RISP_ENOMEM or RISP_ECUDA. */
 int risp_debug_tcgemm(int32_t M, int32_t N, int32_t K, int32_t nbatch, const double *A_dev, const double *B_dev, double *C_dev,
                       int32_t accumulate, int32_t via_planes, int32_t seg_kb, int32_t shape, void *stream);
 
-/* The same segment length for the Eq. 22-23 GEMMs of the following risp_matvec calls in RISP_PRECISION_FP32_K (0: default). */
-int risp_debug_set_tc_segment(risp_ctx *ctx, int32_t seg_kb);
+/* Tile shape (see risp_debug_tcgemm; -1: the library's choice) and stages per accumulation segment (0: the library's choice) of the
+ * Eq. 22 and Eq. 23 launches of the following risp_matvec calls in RISP_PRECISION_FP32_K. */
+int risp_debug_set_tc_plan(risp_ctx *ctx, int32_t eq22_shape, int32_t eq22_seg, int32_t eq23_shape, int32_t eq23_seg);
 
 #ifdef __cplusplus
 }

@@ -105,7 +105,7 @@ def load_library():
     lib.risp_debug_dgemm.argtypes = [C.c_int, C.c_int, C.c_int, vp, C.c_longlong, C.c_int, vp, C.c_longlong, C.c_int, vp, C.c_longlong,
                                      dbl, dbl, C.c_int, C.c_longlong, C.c_longlong, C.c_longlong, C.c_int, C.c_int, C.c_longlong, vp]
     lib.risp_debug_tcgemm.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp]
-    lib.risp_debug_set_tc_segment.argtypes = [vp, C.c_int32]
+    lib.risp_debug_set_tc_plan.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32]
     lib.risp_tcgemm_static.argtypes = [C.c_int32, C.c_int32, C.c_int32, vp, vp, vp, C.c_int32, vp]
     lib.risp_static_last_error.restype = C.c_char_p
     lib.risp_debug_sym_eig_lowest.argtypes = [C.c_int, C.c_int, vp, vp, vp]

@@ -238,9 +238,9 @@ extern "C" int risp_set_precision(risp_ctx *ctx, int32_t mode)
     return RISP_OK;
 }
 
-extern "C" int risp_debug_set_tc_segment(risp_ctx *ctx, int32_t seg_kb)
+extern "C" int risp_debug_set_tc_plan(risp_ctx *ctx, int32_t eq22_shape, int32_t eq22_seg, int32_t eq23_shape, int32_t eq23_seg)
 {
-    if (!ctx || seg_kb < 0) return RISP_EINVAL;
-    ctx->tc_seg_kb = seg_kb;
+    if (!ctx || eq22_shape < -1 || eq22_shape > 2 || eq23_shape < -1 || eq23_shape > 2 || eq22_seg < 0 || eq23_seg < 0) return RISP_EINVAL;
+    ctx->tc_shape22 = eq22_shape; ctx->tc_shape23 = eq23_shape; ctx->tc_seg22 = eq22_seg; ctx->tc_seg23 = eq23_seg;
     return RISP_OK;
 }

@@ -74,7 +74,8 @@ struct TcGemmDesc {
     void *C; long long ldc, sC, planeC;
     int out_kind, rpg; long long gstride; int accumulate;
     int seg_kb = 0;          // stages per accumulation segment (0: the default, 1)
-    int shape = 0;           // 0: 128 x 256 tiles, 32 k per stage (64-byte swizzle rows); 1: 128 x 128 tiles, 64 k per stage (128-byte rows)
+    int shape = 0;           // 0: 128 x 256 tiles, 32 k per stage (64-byte swizzle rows); 1: 128 x 128 tiles, 64 k per stage (128-byte rows);
+                             // 2: CTA pair (cta_group::2), 256 x 256 tile per pair, 32 k per stage, four stages
 };
 cudaError_t risp_tcgemm(const TcGemmDesc &d, cudaStream_t st);
 cudaError_t risp_split_rows_bf3(const double *X, long long ldx, long long rows, int n, void *out, long long ldo, long long plane, int rpg,

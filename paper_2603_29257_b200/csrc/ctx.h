@@ -61,7 +61,8 @@ struct risp_ctx {
     int total_chunks = 0;
     size_t hbm_budget = 0, host_budget = 0;
     int max_batch = RISP_MS, flags = 0;
-    int precision = 0, tc_seg_kb = 0;                           // RISP_PRECISION_*; 32-k stages per accumulation segment of gemm_tc.cu (0: default)
+    int tc_shape22 = -1, tc_shape23 = -1, tc_seg22 = 0, tc_seg23 = 0;   // tile shape / stages per segment of the Eq. 22 / 23 launches of gemm_tc.cu (-1 / 0: default)
+    int precision = 0;                                          // RISP_PRECISION_*
     int shard_rank = 0, shard_count = 1, nauxK_global = 0;      // P-sharded sigma-build: this context holds 1 / shard_count of the pairs and K slices
     // ---- host copies needed after setup (getters, solver)
     std::vector<double> h_xyz, h_prim_exp, h_prim_d /* coef*radial norm, shell-normalised */, h_eps;

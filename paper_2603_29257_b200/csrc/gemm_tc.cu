@@ -11,10 +11,13 @@
 //   C^T-store GEMM:   acc(r, c) = sum_k A[r][k] B[c][k]        both operands K-contiguous, three planes each
 //   out(r, c) at      z * sC + (r / rpg) * gstride + (r % rpg) + c * ldc      (the accumulator row index is the CONTIGUOUS output index)
 //
-// One persistent CTA per SM, 320 threads: warp 0 = TMA producer (one lane), warp 1 = tensor-memory allocation + MMA issue (one
-// lane), warps 2-9 = epilogue (tcgen05.ld of the 128 x BN accumulator, one row and half the columns per thread, so that the 32 lanes
-// of a warp write 32 consecutive output elements per column).  Operand tiles are TMA boxes [3 planes][rows][32 k] in the 64-byte swizzle, three stages;
-// the accumulator is double-buffered in tensor memory (2 x 256 columns) so the epilogue of a tile runs under the MMAs of the next.
+// Single-CTA kernel (tcgemm_bf16x3_kernel): one persistent CTA per SM, 320 threads: warp 0 = TMA producer (one lane), warp 1 =
+// tensor-memory allocation + MMA issue (one lane), warps 2-9 = epilogue (tcgen05.ld of the 128 x BN accumulator, one row and half the
+// columns per thread, so that the 32 lanes of a warp write 32 consecutive output elements per column).  Operand tiles are TMA boxes
+// [3 planes][rows][32 k] in the 64-byte swizzle, three stages; the accumulator is double-buffered in tensor memory (2 x 256 columns)
+// so the register accumulation of one segment runs under the MMAs of the next.
+// CTA-pair kernel (tcgemm2_bf16x3_kernel, what risp_matvec launches): the same roles in each CTA of a 2-CTA cluster, one
+// tcgen05.mma.cta_group::2 stream issued by the leader for a 256 x BN tile; see the comment above it.
 #include "common.cuh"
 #include <cuda.h>
 #include <cuda_bf16.h>
@@ -287,6 +290,221 @@ __global__ void __launch_bounds__(NT, 1) tcgemm_bf16x3_kernel(const __grid_const
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------------
+// CTA-pair variant (cta_group::2): the two CTAs of a cluster, on the two SMs of a TPC, work on one 256 x BN tile.  Each CTA loads
+// its own 128 rows of A and HALF of the B rows (the tensor cores of the pair read both halves), so bytes and TMA requests per SM
+// drop by a third against the single-CTA kernel and a stage is 48 KB: four stages.  The MMAs are issued by the leader CTA (rank 0)
+// for the pair; each CTA's tensor memory holds the accumulator rows of its own A rows and is drained by its own epilogue warps.
+//   full[s]   (leader's copy): 1 arrival (the leader's producer, which also posts the bytes of BOTH CTAs' loads); the TMA loads of
+//             both CTAs complete on it
+//   empty[s]  (each CTA): tcgen05.commit of the leader, multicast to both CTAs
+//   tfull[a]  (each CTA): tcgen05.commit of the leader, multicast
+//   tempty[a] (leader's copy): 2 x 8 arrivals, the epilogue warps of both CTAs
+constexpr int STAGES2 = 4, BK2 = 32, A_PLANE2 = BM * BK2 * 2, BH_PLANE_MAX = (BN_MAX / 2) * BK2 * 2;
+constexpr int STAGE2_BYTES = 3 * A_PLANE2 + 3 * BH_PLANE_MAX;                 // 48 KiB
+constexpr size_t SMEM2_BYTES = (size_t)STAGES2 * STAGE2_BYTES + 1024 + 128;
+
+// shared::cluster address of the leader CTA's copy of a shared-memory object
+__device__ __forceinline__ unsigned leader_addr(unsigned addr)
+{
+    unsigned out;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(out) : "r"(addr), "r"(0));
+    return out;
+}
+__device__ __forceinline__ void tma_load_4d_2sm(unsigned dst, const CUtensorMap *tm, unsigned bar_leader, int c0, int c1, int c2, int c3)
+{
+    asm volatile("cp.async.bulk.tensor.4d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+                 ::"r"(dst), "l"(tm), "r"(bar_leader), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_cluster(unsigned bar) { asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar) : "memory"); }
+__device__ __forceinline__ void umma_bf16_2sm(unsigned tmem_d, unsigned long long adesc, unsigned long long bdesc, unsigned idesc, unsigned accumulate)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n"
+        "}\n" ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit_2sm(unsigned bar)
+{
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar), "h"((unsigned short)3) : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NT, 1)
+tcgemm2_bf16x3_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, TcArgs g)
+{
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char *smem = (unsigned char *)(((size_t)smem_raw + 1023) & ~(size_t)1023);
+    unsigned long long *bars = (unsigned long long *)(smem + STAGES2 * STAGE2_BYTES);
+    unsigned *tmem_slot = (unsigned *)(bars + 2 * STAGES2 + 4);
+    const unsigned smem_u = smem_u32(smem);
+    const unsigned full0 = smem_u32(bars), empty0 = smem_u32(bars + STAGES2), tfull0 = smem_u32(bars + 2 * STAGES2), tempty0 = smem_u32(bars + 2 * STAGES2 + 2);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    unsigned rank;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
+    const bool leader = rank == 0;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES2; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, 1); }
+        for (int s = 0; s < 2; ++s) { mbar_init(tfull0 + 8 * s, 1); mbar_init(tempty0 + 8 * s, 2 * NEPI); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(512) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    cluster_sync_all();
+    tc_fence_after();
+    const unsigned tmem_base = *tmem_slot;
+
+    const int nk = (g.K + BK2 - 1) / BK2;
+    const int nseg = (nk + g.seg_kb - 1) / g.seg_kb;
+    const int tiles_per_batch = g.tiles_m * g.tiles_n;          // tiles_m counts 256-row tiles here
+    const int total_tiles = tiles_per_batch * g.nb;
+    const int pair = blockIdx.x >> 1, npairs = gridDim.x >> 1;
+    const int bh = g.BN >> 1;                                   // B rows held by one CTA
+    const int bh_plane = bh * BK2 * 2;
+    const unsigned stage_tx = 2 * (3 * A_PLANE2 + 3 * bh_plane);
+
+    if (warp == 0) {
+        if (lane == 0) {
+            int slot = 0; unsigned par = 1;
+            for (int tile = pair; tile < total_tiles; tile += npairs) {
+                const int z = tile / tiles_per_batch, tt = tile % tiles_per_batch;
+                int tm, tn;
+                tile_coords(tt, g.tiles_m, g.tiles_n, g.gm, tm, tn);
+                for (int kb = 0; kb < nk; ++kb) {
+                    mbar_wait(empty0 + 8 * slot, par);
+                    const unsigned fb = leader_addr(full0 + 8 * slot), dst = smem_u + slot * STAGE2_BYTES;
+                    if (leader) mbar_expect_tx(full0 + 8 * slot, stage_tx);
+                    tma_load_4d_2sm(dst, &tmA, fb, kb * BK2, tm * 256 + (int)rank * BM, 0, g.za ? z : 0);
+                    tma_load_4d_2sm(dst + 3 * A_PLANE2, &tmB, fb, kb * BK2, tn * g.BN + (int)rank * bh, 0, g.zb ? z : 0);
+                    if (++slot == STAGES2) { slot = 0; par ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        if (lane == 0 && leader) {
+            // D = F32, A = B = BF16, both K-major, N >> 3 at bit 17, M = 256 >> 4 at bit 24
+            const unsigned idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((unsigned)(g.BN >> 3) << 17) | ((unsigned)(256 >> 4) << 24);
+            int slot = 0; unsigned par = 0;
+            int acc = 0; unsigned apar = 1;
+            for (int tile = pair; tile < total_tiles; tile += npairs) {
+                for (int kb0 = 0; kb0 < nk; kb0 += g.seg_kb) {
+                    mbar_wait(tempty0 + 8 * acc, apar);
+                    tc_fence_after();
+                    const unsigned tacc = tmem_base + acc * BN_MAX;
+                    const int kb1 = min(nk, kb0 + g.seg_kb);
+                    // A segment of up to STAGES2 / 2 stages is issued in two passes over its stages: the five small products of every
+                    // stage first, into the fresh accumulator where their truncation costs nothing, then the leading products a1 b1.
+                    // Only those (two per stage) truncate at the size of the result, however long the segment is; half of the ring
+                    // stays free for the loads of the next segment.
+                    const bool two_pass = 2 * g.seg_kb <= STAGES2;
+                    constexpr int PA[6] = {2, 0, 1, 1, 0, 0}, PB[6] = {0, 2, 1, 0, 1, 0};
+                    for (int pass = two_pass ? 0 : 2; pass < (two_pass ? 2 : 3); ++pass) {         // 0: small products, 1: leading products, 2: both
+                        int sl = slot; unsigned pr = par;
+                        for (int kb = kb0; kb < kb1; ++kb) {
+                            if (pass != 1) { mbar_wait(full0 + 8 * sl, pr); tc_fence_after(); }
+                            const unsigned a0 = smem_u + sl * STAGE2_BYTES, b0 = a0 + 3 * A_PLANE2;
+                            unsigned long long ad[3][BK2 / 16], bd[3][BK2 / 16];
+#pragma unroll
+                            for (int ks = 0; ks < BK2 / 16; ++ks)
+#pragma unroll
+                                for (int p = 0; p < 3; ++p) {
+                                    ad[p][ks] = smem_desc<BK2>(a0 + p * A_PLANE2 + ks * 32);
+                                    bd[p][ks] = smem_desc<BK2>(b0 + p * bh_plane + ks * 32);
+                                }
+#pragma unroll
+                            for (int t = 0; t < 6; ++t) {
+                                if ((pass == 0 && t == 5) || (pass == 1 && t != 5)) continue;
+#pragma unroll
+                                for (int ks = 0; ks < BK2 / 16; ++ks)
+                                    umma_bf16_2sm(tacc, ad[PA[t]][ks], bd[PB[t]][ks], idesc, (kb != kb0) || t != 0 || ks != 0);
+                            }
+                            if (pass != 0) umma_commit_2sm(empty0 + 8 * sl);
+                            if (++sl == STAGES2) { sl = 0; pr ^= 1; }
+                        }
+                        if (pass != 0) { slot = sl; par = pr; }
+                    }
+                    umma_commit_2sm(tfull0 + 8 * acc);
+                    if (++acc == 2) { acc = 0; apar ^= 1; }
+                }
+            }
+        }
+    } else {
+        const int lg = warp & 3;
+        const int half = (warp - 2) >> 2;
+        int acc = 0; unsigned apar = 0;
+        for (int tile = pair; tile < total_tiles; tile += npairs) {
+            const int z = tile / tiles_per_batch, tt = tile % tiles_per_batch;
+            int tm, tn;
+            tile_coords(tt, g.tiles_m, g.tiles_n, g.gm, tm, tn);
+            float run[128];
+#pragma unroll
+            for (int c = 0; c < 128; ++c) run[c] = 0.f;
+            const bool cols_used = half * 128 < g.BN;
+            for (int sg = 0; sg < nseg; ++sg) {
+                mbar_wait(tfull0 + 8 * acc, apar);
+                tc_fence_after();
+                if (cols_used) {
+                    const unsigned taddr = tmem_base + ((unsigned)(lg * 32) << 16) + acc * BN_MAX + half * 128;
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        unsigned v[32];
+                        tmem_ld32(taddr + q * 32, v);
+#pragma unroll
+                        for (int c = 0; c < 32; ++c) run[q * 32 + c] += __uint_as_float(v[c]);
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(leader_addr(tempty0 + 8 * acc));
+                if (++acc == 2) { acc = 0; apar ^= 1; }
+            }
+            const int row = tm * 256 + (int)rank * BM + lg * 32 + lane;
+            if (row < g.M && cols_used) {
+                long long roff = (long long)z * g.sC;
+                if (g.rpg > 0) roff += (long long)(row / g.rpg) * g.gstride + (row % g.rpg);
+                else roff += row;
+                const int colb = tn * g.BN + half * 128;
+                const int ncol = min(128, min(g.BN - half * 128, g.N - colb));
+                if (g.out_kind == 0) {
+                    double *C = (double *)g.C + roff + (long long)colb * g.ldc;
+#pragma unroll
+                    for (int c = 0; c < 128; ++c)
+                        if (c < ncol) {
+                            double *p = C + (long long)c * g.ldc;
+                            *p = g.accumulate ? *p + (double)run[c] : (double)run[c];
+                        }
+                } else {
+                    __nv_bfloat16 *C = (__nv_bfloat16 *)g.C + roff + (long long)colb * g.ldc;
+#pragma unroll
+                    for (int c = 0; c < 128; ++c)
+                        if (c < ncol) {
+                            __nv_bfloat16 b1, b2, b3;
+                            split3(run[c], b1, b2, b3);
+                            __nv_bfloat16 *p = C + (long long)c * g.ldc;
+                            p[0] = b1; p[g.planeC] = b2; p[2 * g.planeC] = b3;
+                        }
+                }
+            }
+        }
+    }
+    __syncwarp();
+    tc_fence_before();
+    cluster_sync_all();
+    if (warp == 1) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
+    }
+}
+
 typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
                              const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 EncodeFn get_encode()
@@ -426,14 +644,50 @@ cudaError_t launch_shape(const TcGemmDesc &d, cudaStream_t st)
 }
 }  // namespace
 
+namespace {
+cudaError_t launch_pair(const TcGemmDesc &d, cudaStream_t st)
+{
+    EncodeFn enc = get_encode();
+    if (!enc) return cudaErrorNotSupported;
+    static bool attr[64] = {};
+    static int sms[64] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (!attr[dev & 63]) {
+        cudaError_t e = cudaFuncSetAttribute(tcgemm2_bf16x3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM2_BYTES);
+        if (e != cudaSuccess) return e;
+        cudaDeviceGetAttribute(&sms[dev & 63], cudaDevAttrMultiProcessorCount, dev);
+        attr[dev & 63] = true;
+    }
+    TcArgs g;
+    const int nt = (d.N + BN_MAX - 1) / BN_MAX;
+    g.BN = std::min(BN_MAX, (((d.N + nt - 1) / nt) + 15) & ~15);
+    g.M = d.M; g.N = d.N; g.K = d.K; g.nb = d.nb; g.za = d.sA != 0; g.zb = d.sB != 0;
+    g.out_kind = d.out_kind; g.C = d.C; g.ldc = d.ldc; g.sC = d.sC; g.planeC = d.planeC; g.rpg = d.rpg; g.gstride = d.gstride; g.accumulate = d.accumulate;
+    g.seg_kb = d.seg_kb > 0 ? d.seg_kb : STAGES2 / 2;      // two stages (64 k), issued in two passes
+    g.tiles_m = (d.M + 255) / 256; g.tiles_n = (d.N + g.BN - 1) / g.BN;
+    const long long total = (long long)g.tiles_m * g.tiles_n * d.nb;
+    if (total >= (1ll << 31)) return cudaErrorNotSupported;
+    CUtensorMap ma, mb;
+    if (!make_map(enc, &ma, (const __nv_bfloat16 *)d.A, d.M, d.K, d.lda, d.planeA, d.sA, d.nb, BM, BK2)) return cudaErrorNotSupported;
+    if (!make_map(enc, &mb, (const __nv_bfloat16 *)d.B, d.N, d.K, d.ldb, d.planeB, d.sB, d.nb, g.BN / 2, BK2)) return cudaErrorNotSupported;
+    const int pairs = (int)std::min<long long>(total, sms[dev & 63] / 2);
+    g.gm = std::max(1, std::min(g.tiles_m, (sms[dev & 63] / 2 + g.tiles_n - 1) / g.tiles_n));
+    tcgemm2_bf16x3_kernel<<<2 * pairs, NT, SMEM2_BYTES, st>>>(ma, mb, g);
+    return cudaGetLastError();
+}
+}  // namespace
+
 cudaError_t risp_tcgemm(const TcGemmDesc &d, cudaStream_t st)
 {
     if (d.M <= 0 || d.N <= 0 || d.nb <= 0) return cudaSuccess;
     if (d.K <= 0) return cudaErrorNotSupported;
+    if (d.shape == 2) return launch_pair(d, st);
     // Measured on the 300-atom system with the MMAs switched off, the operand traffic alone costs 44 ms of the 50 ms of the Eq. 22
-    // launch: about half of it scales with the bytes (L2 -> SM), half with the number of TMA row requests.  128 x 256 tiles with
-    // 64-byte rows minimise the bytes; 128 x 128 tiles with 128-byte rows the requests -- the latter wins when the column count
-    // leaves a 256-wide tile half empty anyway (Eq. 23, N = N_occK').
+    // launch of the single-CTA kernel: about half of it scales with the bytes (L2 -> SM), half with the number of TMA row requests.
+    // The CTA pair (shape 2) moves a third fewer bytes per SM and is what risp_matvec uses: 44.9 / 14.7 ms for Eq. 22 / 23 against
+    // 50.7 / 16.9 ms.  Its accumulator hand-over crosses the SM pair and costs ~3000 cycles per segment, which is why its segments
+    // are two stages long and issued in two passes (at one stage per segment it is slower than the single-CTA kernel: 57 ms).
     if (d.shape == 1) return launch_shape<TcShape<64, 128, 2>>(d, st);
     return launch_shape<TcShape<32, 256, 3>>(d, st);
 }

@@ -363,7 +363,7 @@ after_pass1:
                 d.M = m * no; d.N = nv; d.K = nv; d.nb = c.np;
                 d.A = qX; d.lda = nv_q; d.planeA = plX; d.sA = 0;
                 d.B = qTab; d.ldb = nv_q; d.planeB = plTab; d.sB = (long long)nv * nv_q;
-                d.C = qM; d.ldc = ldK; d.sC = no_q; d.planeC = plM; d.out_kind = 1; d.rpg = no; d.gstride = (long long)nv * ldK; d.accumulate = 0; d.seg_kb = ctx->tc_seg_kb;
+                d.C = qM; d.ldc = ldK; d.sC = no_q; d.planeC = plM; d.out_kind = 1; d.rpg = no; d.gstride = (long long)nv * ldK; d.accumulate = 0; d.seg_kb = ctx->tc_seg22; d.shape = ctx->tc_shape22 >= 0 ? ctx->tc_shape22 : 2;
                 RISP_CUDA_TRY(risp_tcgemm(d, st)); ++launches;
                 if (ci == 0) RISP_CUDA_TRY(cudaEventRecord(ev[9], st));
                 // Eq. 23, stored transposed: K'[mi][i][a] (+)= sum_{(P, j)} Mt[mi][a][(P, j)] T_ij[i][(P, j)]
@@ -371,7 +371,7 @@ after_pass1:
                 e.M = nv; e.N = no; e.K = (int)(c.np * no_q); e.nb = m;
                 e.A = qM; e.lda = ldK; e.planeA = plM; e.sA = (long long)nv * ldK;
                 e.B = qTij; e.ldb = ldK; e.planeB = plTij; e.sB = 0;
-                e.C = wKk; e.ldc = nv_p; e.sC = (long long)no * nv_p; e.planeC = 0; e.out_kind = 0; e.rpg = 0; e.gstride = 0; e.accumulate = ci != 0; e.seg_kb = ctx->tc_seg_kb; e.shape = 1;
+                e.C = wKk; e.ldc = nv_p; e.sC = (long long)no * nv_p; e.planeC = 0; e.out_kind = 0; e.rpg = 0; e.gstride = 0; e.accumulate = ci != 0; e.seg_kb = ctx->tc_seg23; e.shape = ctx->tc_shape23 >= 0 ? ctx->tc_shape23 : 2;
                 RISP_CUDA_TRY(risp_tcgemm(e, st)); ++launches;
                 if (ci == 0) { RISP_CUDA_TRY(cudaEventRecord(ev[10], st)); ctx->tim.first_chunk_naux = c.np; }
                 continue;

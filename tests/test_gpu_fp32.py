@@ -34,7 +34,7 @@ def _tcgemm(torch, A, B, C0=None, via_planes=0, seg_kb=0, shape=0):
     return Cc
 
 
-@pytest.mark.parametrize("tile_shape", [0, 1])
+@pytest.mark.parametrize("tile_shape", [0, 1, 2])
 @pytest.mark.parametrize("via_planes", [0, 1])
 @pytest.mark.parametrize("shape", [(128, 256, 32, 1), (128, 16, 64, 1), (1, 1, 1, 1), (100, 200, 40, 2), (129, 257, 33, 1), (300, 423, 1496, 2),
                                    (1496, 423, 3392, 3), (640, 700, 999, 2)])
