@@ -499,6 +499,64 @@ def run_sharded(args, world, rank, local, dist):
                               note="sharded mode: device-resident replicated X; no roofline / e2e legs in this mode")))
 
 
+def run_extras(args):
+    """--extras: the follow-on rows of the path on the chosen workload, one JSON line of its own: the full-TDDFT
+    product ((A+B) X, (A-B) X) per second, the 15-root risp_tddft_solve, and risp_transition_properties of the TDA roots.  Reported
+    beside the headline, not part of it."""
+    import torch
+    from paper_2603_29257_b200 import setup
+    from workloads import make_system, trial_vectors
+    s = make_system(args.config)
+    m = args.batch if args.batch > 0 else s["m"]
+    dev = torch.device("cuda:0")
+    t0 = time.time()
+    ctx = setup(s, flags=8, max_batch=m)                      # RISP_FLAG_TDDFT: also builds T_ia^P over the window
+    t_setup = time.time() - t0
+    X = torch.from_numpy(trial_vectors(s, m)).to(dev)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream(dev)
+    for _ in range(max(args.warmup, 3)):
+        ctx.matvec_tddft(X)
+    torch.cuda.synchronize()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in evs:
+        flush.zero_()
+        a.record(stream)
+        sp, sm = ctx.matvec_tddft(X)
+        b.record(stream)
+        b.synchronize()
+    t_td = sum(a.elapsed_time(b) for a, b in evs) * 1e-3
+    launches = ctx.timings()["kernel_launches"]
+    sig = ctx.matvec(X)
+    # A = ((A+B) + (A-B)) / 2: the TDA product of the same context must be the mean of the two TDDFT products
+    mean_err = float(((0.5 * (sp + sm)) - sig).norm() / sig.norm())
+    del sp, sm, sig
+    n = s["nroots"]
+    om, Xr, info = ctx.tda_solve(n, tol=args.solve_tol, max_iter=args.solve_max_iter, want_vectors=True, allow_unconverged=True)
+    ctx.transition_properties(Xr, om)
+    t0 = time.perf_counter()
+    for _ in range(3):
+        mu, mm, f, R = ctx.transition_properties(Xr, om)
+    t_prop = (time.perf_counter() - t0) / 3
+    del Xr
+    Om, _, _, tinfo = ctx.tddft_solve(n, tol=args.solve_tol, max_iter=args.solve_max_iter, allow_unconverged=True)
+    d = ctx.dims()
+    ctx.close()
+    no, nv, nK = d["noccK"], d["nvirK"], d["nauxK"]
+    print(json.dumps(dict(
+        impl="extras", workload=s["name"], m=m, dtype="f64", data="synthetic", setup_s=round(t_setup, 3),
+        tddft_matvec=dict(value=m * args.steps / t_td, unit="(A+B, A-B) product pairs/s", ms_per_step=1e3 * t_td / args.steps, steps=args.steps,
+                          gpu_launches_per_step=launches, extra_flops_vs_tda=4.0 * m * nK * no * no * nv,
+                          tda_product_is_mean_of_both_rel_err=mean_err, l2="flushed between steps (512 MiB write)"),
+        tda_solve=dict(wall_s=info["sec_total"], iterations=info["iterations"], n_sigma=info["n_sigma"], converged=info["converged"]),
+        tddft_solve=dict(nroots=n, tol=args.solve_tol, wall_s=tinfo["sec_total"], matvec_s=tinfo["sec_matvec"], iterations=tinfo["iterations"],
+                         n_sigma=tinfo["n_sigma"], converged=tinfo["converged"], resid_max=float(max(tinfo["resid"])),
+                         omega_ev=[float(x) * HARTREE_EV for x in Om],
+                         max_tda_minus_tddft_ev=float(np.max(om - Om) * HARTREE_EV), min_tda_minus_tddft_ev=float(np.min(om - Om) * HARTREE_EV)),
+        transition_properties=dict(states=n, ms_per_call=1e3 * t_prop, oscillator_strengths=[float(x) for x in f],
+                                   rotatory_strengths=[float(x) for x in R]))))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -526,6 +584,7 @@ def main():
     ap.add_argument("--also-budget-s", type=float, default=420.0, help="an `also` config starts only if the run is younger than this")
     ap.add_argument("--parallel", default="vectors", choices=["vectors", "shard"],
                     help="N > 1: 'vectors' = every rank its own batch (weak scaling, no collective); 'shard' = one P-sharded problem (strong scaling)")
+    ap.add_argument("--extras", action="store_true", help="instead of the headline: full-TDDFT products and solve, transition properties (one JSON line)")
     ap.add_argument("--host-budget-gb", type=int, default=0, help="pinned-host budget of the Davidson subspace (0: half of the host memory)")
     args = ap.parse_args()
     # contract: >= 3 warm-up steps; the 1000/3000-atom configs (tens of seconds to minutes per step) are allowed 1 and say so
@@ -540,6 +599,10 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
+    if args.extras:
+        if rank == 0:
+            run_extras(args)
+        return
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
 
