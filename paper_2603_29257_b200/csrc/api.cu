@@ -11,7 +11,7 @@ extern "C" void risp_destroy(risp_ctx *ctx)
     risp_free_workspace(ctx);
     if (ctx->w_Xin) cudaFree(ctx->w_Xin);
     if (ctx->w_Sout) cudaFree(ctx->w_Sout);
-    double **bufs[] = {&ctx->d_Cocc, &ctx->d_Cvir, &ctx->d_eps, &ctx->d_boys, &ctx->d_MJ, &ctx->d_LinvJ, &ctx->d_MK, &ctx->d_MKinv, &ctx->d_TijP,
+    double **bufs[] = {&ctx->d_Cocc, &ctx->d_CoccT, &ctx->d_Cvir, &ctx->d_eps, &ctx->d_boys, &ctx->d_MJ, &ctx->d_LinvJ, &ctx->d_MK, &ctx->d_MKinv, &ctx->d_TijP,
                        &ctx->d_TabP, &ctx->d_Tov, &ctx->d_LinvK};
     for (auto b : bufs) if (*b) cudaFree(*b);
     if (ctx->h_TijP) cudaFreeHost(ctx->h_TijP);

@@ -73,6 +73,7 @@ struct risp_ctx {
     std::vector<int> h_even_shell_ao;      // AO offsets of shell starts that are even (candidate panel boundaries), ascending
     // ---- device data built by setup
     double *d_Cocc = nullptr;     // [nao][ldocc]
+    double *d_CoccT = nullptr;    // [nocc][ldao]: C_occ^T, so that the back-transform Z = C_occ^T U reads a K-contiguous operand (one TMA box per stage)
     double *d_Cvir = nullptr;     // [nao][ldvir]
     double *d_eps = nullptr;      // [nmo]
     double *d_boys = nullptr;     // Boys table

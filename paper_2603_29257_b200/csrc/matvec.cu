@@ -256,7 +256,7 @@ after_pass1:
             }
             if ((rc = join_classes(ctx, st))) return rc;
             // Z[i][nu] (+)= sum_{mu in panel} C_occ[mu][i] U[mu][nu]
-            GemmDesc d = gemm_desc(nocc, nao, pr, ctx->d_Cocc + (size_t)r0 * ldocc, ldocc, false, wD, ldao, false, wY, ldao, 1.0, p == 0 ? 0.0 : 1.0);
+            GemmDesc d = gemm_desc(nocc, nao, pr, ctx->d_CoccT + r0, ldao, true, wD, ldao, false, wY, ldao, 1.0, p == 0 ? 0.0 : 1.0);
             d.nb1 = mj; d.sB1 = mstride; d.sC1 = (long long)nocc * ldao;
             RISP_CUDA_TRY(risp_dgemm(d, st)); ++launches;
         }

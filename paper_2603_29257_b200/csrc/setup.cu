@@ -296,6 +296,12 @@ extern "C" int risp_setup(const risp_system *sys, const risp_options *opt_in, ri
             std::memcpy(&cv[(size_t)mu * ctx->ldvir], sys->C + (size_t)mu * ctx->nmo + ctx->nocc, (size_t)ctx->nvir * sizeof(double));
         }
         if ((rc = upload(ctx, ctx->d_Cocc, co.data(), co.size()))) return rc;
+        {
+            std::vector<double> cot((size_t)ctx->nocc * ctx->ldao, 0.0);
+            for (int mu = 0; mu < ctx->nao; ++mu)
+                for (int i = 0; i < ctx->nocc; ++i) cot[(size_t)i * ctx->ldao + mu] = sys->C[(size_t)mu * ctx->nmo + i];
+            if ((rc = upload(ctx, ctx->d_CoccT, cot.data(), cot.size()))) return rc;
+        }
         if ((rc = upload(ctx, ctx->d_Cvir, cv.data(), cv.size()))) return rc;
         if ((rc = upload(ctx, ctx->d_eps, sys->eps, (size_t)ctx->nmo))) return rc;
     }

@@ -181,3 +181,32 @@ def test_tcgemm_segment_length(torch_cuda):
     assert err[1] < err[4] < err[1000]
     assert err[1000] > 20 * err[1]
     assert err[1] <= 5e-7
+
+
+def test_fp32_mode_in_the_sharded_sigma_build(torch_cuda, sys_small_rsh, oracle_small_rsh):
+    """RISP_PRECISION_FP32_K with the P-sharded sigma-build (risp_matvec_shard_begin / _end on two shards emulated on one GPU): the sum
+    of the shards' partial sigma lies as close to the FP64 oracle as the unsharded single-precision product, and the J part, which
+    stays FP64, is unchanged."""
+    torch = torch_cuda
+    from paper_2603_29257_b200 import setup
+    from workloads import trial_vectors
+    s, o = sys_small_rsh, oracle_small_rsh
+    m = 4
+    X = trial_vectors(s, m)
+    Xd = torch.from_numpy(X).cuda()
+    sig_ref, dg, J_ref, K_ref = o.sigma(X, parts=True)
+    ctxs = [setup(s, shard_rank=r, shard_count=2) for r in range(2)]
+    try:
+        for c in ctxs:
+            c.set_precision(1)
+        R = torch.stack([c.matvec_shard_begin(Xd) for c in ctxs]).sum(0)
+        sig = torch.stack([c.matvec_shard_end(Xd, R) for c in ctxs]).sum(0).cpu().numpy()
+        K = sum(c.stage("K", m) for c in ctxs)
+        relK = np.linalg.norm(K - K_ref) / np.linalg.norm(K_ref)
+        assert 1e-12 < relK <= 1e-6
+        J = (sig - dg + K) / 2.0
+        assert np.linalg.norm(J - J_ref) / np.linalg.norm(J_ref) <= 1e-9
+        assert np.linalg.norm(sig - sig_ref) / np.linalg.norm(sig_ref) <= 1e-6
+    finally:
+        for c in ctxs:
+            c.close()
