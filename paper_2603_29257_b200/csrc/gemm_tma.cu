@@ -25,6 +25,7 @@ constexpr int TILE_BYTES = BM_MAX * BK * 8;                   // 16 KiB per oper
 constexpr size_t SMEM_BYTES = (size_t)STAGES * 2 * TILE_BYTES + 1024 /*alignment slack*/ + 2 * STAGES * 8;
 
 int sm_count();
+long long l2_bytes();
 
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 
@@ -76,11 +77,39 @@ __device__ __forceinline__ int frag_off(int mn, int k)
 struct TmaArgs {
     int coff_a, coff_b;          // offset of the contiguous coordinate (always 0: TMA needs 16-byte aligned box starts)
     int za1, za2, zb1, zb2;      // 1: the operand moves with batch index z1 / z2; 0: shared by the batch
+    int grp;                     // GRP kernels: row tiles per group (tile_coords)
 };
+
+// Tile number -> (batch z, row tile tm, column tile tn).  Plain order: tm fastest, then tn, then z -- the CTAs of a wave share
+// one or two B panels in L2.  Grouped order (GRP; Eq. 22, where A = X' is shared by the whole batch and larger than L2): the
+// row tiles are cut into groups of `grp`, and inside a group tm runs fastest, then tn, then z, so that the group's rows of A
+// (sized by the host to a quarter of L2) stay resident while every B panel of the batch streams past them once per group.
+// In the plain order each wave of 148 tiles touches all of A, and A is re-read from DRAM per column tile and batch entry
+// (300 atoms: 202 GB read per launch against 3 GB of operands).
+template <bool GRP>
+__device__ __forceinline__ void tile_coords(int tile, int tiles_m, int tiles_n, int nbz, int grp, int &z, int &tm, int &tn)
+{
+    if (!GRP) {
+        const int tiles_per_batch = tiles_m * tiles_n;
+        z = tile / tiles_per_batch;
+        const int tt = tile - z * tiles_per_batch;
+        tn = tt / tiles_m;
+        tm = tt - tn * tiles_m;
+    } else {
+        const int per_group = grp * tiles_n * nbz;               // tiles of a full group; only the last group can be shorter
+        const int g = tile / per_group;
+        const int rem = tile - g * per_group;
+        const int gsz = min(grp, tiles_m - g * grp);
+        const int r2 = rem / gsz;
+        tm = g * grp + (rem - r2 * gsz);
+        z = r2 / tiles_n;
+        tn = r2 - z * tiles_n;
+    }
+}
 
 // MI = 8x8 DMMA tiles per warp along m: CTA tile BM = 16 MI rows (128 ... 16), chosen per call (pick_mi).  The small values
 // serve the skinny products of the Davidson loop (15 x dim Gram and Ritz updates), which are HBM-bound anyway.
-template <bool AKC, bool BKC, int MI>
+template <bool AKC, bool BKC, int MI, bool GRP>
 __global__ void __launch_bounds__(NT, 1) dgemm_tma_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                                                           GemmDesc d, TmaArgs ta, int tiles_m, int tiles_n)
 {
@@ -103,8 +132,8 @@ __global__ void __launch_bounds__(NT, 1) dgemm_tma_kernel(const __grid_constant_
     __syncthreads();
 
     const int nk = (d.K + BK - 1) / BK;
-    const int tiles_per_batch = tiles_m * tiles_n;
-    const int total_tiles = tiles_per_batch * d.nb1 * d.nb2;
+    const int nbz = d.nb1 * d.nb2;
+    const int total_tiles = tiles_m * tiles_n * nbz;
     const int my_tiles = ((int)blockIdx.x < total_tiles) ? (total_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     const long long total_steps = (long long)my_tiles * nk;
 
@@ -114,12 +143,15 @@ __global__ void __launch_bounds__(NT, 1) dgemm_tma_kernel(const __grid_constant_
     unsigned h_par = 1;                                        // parity to wait on the empty barrier (fresh barrier passes 1)
     // executed by all lanes of warp 0: lane 0 waits for the slot and arms the barrier, then the boxes of the stage are issued by
     // one lane each (an MN-contiguous operand is BM/16 or 8 boxes: issuing them from one thread costs that warp ~10 % of a k tile)
+    int h_m0 = 0, h_n0 = 0, h_z1 = 0, h_z2 = 0;                // coordinates of the producer's tile, recomputed once per tile
     auto issue = [&]() {
-        const int tile = (int)blockIdx.x + h_ti * (int)gridDim.x;
-        const int z = tile / tiles_per_batch, tt = tile % tiles_per_batch;
-        const int tm = tt % tiles_m, tn = tt / tiles_m;      // m fastest: concurrently running CTAs share the B panel in L2
-        const int z1 = z / d.nb2, z2 = z % d.nb2;
-        const int m0 = tm * BM, n0 = tn * BN, k0 = h_kt * BK;
+        if (h_kt == 0) {
+            int z, tm, tn;
+            tile_coords<GRP>((int)blockIdx.x + h_ti * (int)gridDim.x, tiles_m, tiles_n, nbz, ta.grp, z, tm, tn);
+            h_z1 = z / d.nb2; h_z2 = z - h_z1 * d.nb2;
+            h_m0 = tm * BM; h_n0 = tn * BN;
+        }
+        const int z1 = h_z1, z2 = h_z2, m0 = h_m0, n0 = h_n0, k0 = h_kt * BK;
         const unsigned fb = full0 + 8 * h_slot;
         if (lane == 0) {
             mbar_wait(empty0 + 8 * h_slot, h_par);
@@ -197,9 +229,8 @@ __global__ void __launch_bounds__(NT, 1) dgemm_tma_kernel(const __grid_constant_
             if (++slot == STAGES) { slot = 0; par ^= 1; }
         }
         // epilogue: thread holds C(row = q, col = 2r, 2r+1) of each 8x8 tile
-        const int tile = (int)blockIdx.x + ti * (int)gridDim.x;
-        const int z = tile / tiles_per_batch, tt = tile % tiles_per_batch;
-        const int tm = tt % tiles_m, tn = tt / tiles_m;
+        int z, tm, tn;
+        tile_coords<GRP>((int)blockIdx.x + ti * (int)gridDim.x, tiles_m, tiles_n, nbz, ta.grp, z, tm, tn);
         const int z1 = z / d.nb2, z2 = z % d.nb2;
         const int m0 = tm * BM, n0 = tn * BN;
         double *Cp = d.C + z1 * d.sC1 + z2 * d.sC2;
@@ -263,14 +294,14 @@ bool make_map(EncodeFn enc, CUtensorMap *tm, const double *p, bool kc, int MN, i
     return rc == CUDA_SUCCESS;
 }
 
-template <bool AKC, bool BKC, int MI>
-cudaError_t launch_mi(const CUtensorMap &ma, const CUtensorMap &mb, const GemmDesc &d, const TmaArgs &ta, cudaStream_t st)
+template <bool AKC, bool BKC, int MI, bool GRP>
+cudaError_t launch_mi(const CUtensorMap &ma, const CUtensorMap &mb, const GemmDesc &d, TmaArgs ta, cudaStream_t st)
 {
     static bool attr[64] = {};              // per device
     int dev = 0;
     cudaGetDevice(&dev);
     if (!attr[dev & 63]) {
-        cudaError_t e = cudaFuncSetAttribute(dgemm_tma_kernel<AKC, BKC, MI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
+        cudaError_t e = cudaFuncSetAttribute(dgemm_tma_kernel<AKC, BKC, MI, GRP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
         if (e != cudaSuccess) return e;
         attr[dev & 63] = true;
     }
@@ -279,7 +310,14 @@ cudaError_t launch_mi(const CUtensorMap &ma, const CUtensorMap &mb, const GemmDe
     const int tiles_m = (d.M + BM - 1) / BM, tiles_n = (d.N + BN - 1) / BN;
     const long long total = (long long)tiles_m * tiles_n * d.nb1 * d.nb2;
     const int grid = (int)std::min<long long>(total, sms);
-    dgemm_tma_kernel<AKC, BKC, MI><<<grid, NT, SMEM_BYTES, st>>>(ma, mb, d, ta, tiles_m, tiles_n);
+    if (GRP) {
+        // rows of A kept resident per group: a quarter of L2 (the two halves of the L2 mirror each other's lines, B and C stream through)
+        const long long row_tile_bytes = (long long)BM * d.K * 8;
+        const int gmax = (int)std::max<long long>(8, l2_bytes() / 4 / row_tile_bytes);
+        const int ngroups = (tiles_m + gmax - 1) / gmax;
+        ta.grp = (tiles_m + ngroups - 1) / ngroups;
+    }
+    dgemm_tma_kernel<AKC, BKC, MI, GRP><<<grid, NT, SMEM_BYTES, st>>>(ma, mb, d, ta, tiles_m, tiles_n);
     return cudaGetLastError();
 }
 
@@ -300,6 +338,15 @@ int pick_mi(int M, long long col_tiles_x_batch, int sms)
     return best;
 }
 
+long long l2_bytes()
+{
+    static int l2[64] = {};                 // per device
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (!l2[dev & 63]) cudaDeviceGetAttribute(&l2[dev & 63], cudaDevAttrL2CacheSize, dev);
+    return l2[dev & 63];
+}
+
 int sm_count()
 {
     static int sms[64] = {};                // per device
@@ -309,18 +356,18 @@ int sm_count()
     return sms[dev & 63];
 }
 
-template <bool AKC, bool BKC>
+template <bool AKC, bool BKC, bool GRP = false>
 cudaError_t launch(const CUtensorMap &ma, const CUtensorMap &mb, const GemmDesc &d, const TmaArgs &ta, int mi, cudaStream_t st)
 {
     switch (mi) {
-    case 7: return launch_mi<AKC, BKC, 7>(ma, mb, d, ta, st);
-    case 6: return launch_mi<AKC, BKC, 6>(ma, mb, d, ta, st);
-    case 5: return launch_mi<AKC, BKC, 5>(ma, mb, d, ta, st);
-    case 4: return launch_mi<AKC, BKC, 4>(ma, mb, d, ta, st);
-    case 3: return launch_mi<AKC, BKC, 3>(ma, mb, d, ta, st);
-    case 2: return launch_mi<AKC, BKC, 2>(ma, mb, d, ta, st);
-    case 1: return launch_mi<AKC, BKC, 1>(ma, mb, d, ta, st);
-    default: return launch_mi<AKC, BKC, 8>(ma, mb, d, ta, st);
+    case 7: return launch_mi<AKC, BKC, 7, GRP>(ma, mb, d, ta, st);
+    case 6: return launch_mi<AKC, BKC, 6, GRP>(ma, mb, d, ta, st);
+    case 5: return launch_mi<AKC, BKC, 5, GRP>(ma, mb, d, ta, st);
+    case 4: return launch_mi<AKC, BKC, 4, GRP>(ma, mb, d, ta, st);
+    case 3: return launch_mi<AKC, BKC, 3, GRP>(ma, mb, d, ta, st);
+    case 2: return launch_mi<AKC, BKC, 2, GRP>(ma, mb, d, ta, st);
+    case 1: return launch_mi<AKC, BKC, 1, GRP>(ma, mb, d, ta, st);
+    default: return launch_mi<AKC, BKC, 8, GRP>(ma, mb, d, ta, st);
     }
 }
 
@@ -339,6 +386,12 @@ cudaError_t risp_dgemm_tma(const GemmDesc &d, cudaStream_t st)
     TmaArgs ta;
     if (!make_map(enc, &ma, d.A, d.a_kc, d.M, d.K, d.lda, d.sA1, d.nb1, d.sA2, d.nb2, 16 * mi, &ta.coff_a, &ta.za1, &ta.za2)) return cudaErrorNotSupported;
     if (!make_map(enc, &mb, d.B, d.b_kc, d.N, d.K, d.ldb, d.sB1, d.nb1, d.sB2, d.nb2, BN, &ta.coff_b, &ta.zb1, &ta.zb2)) return cudaErrorNotSupported;
+    ta.grp = 0;
+    // Eq. 22 shape: both operands K-contiguous, A shared by a batch of B's and too large to survive a sweep in L2
+    const bool a_shared = ta.za1 == 0 && ta.za2 == 0 && (long long)d.nb1 * d.nb2 > 1;
+    if (d.a_kc && d.b_kc && a_shared && mi >= 6 && (long long)d.M * d.K * 8 > l2_bytes() / 4)
+        return mi == 6 ? launch_mi<true, true, 6, true>(ma, mb, d, ta, st) : mi == 7 ? launch_mi<true, true, 7, true>(ma, mb, d, ta, st)
+                                                                                      : launch_mi<true, true, 8, true>(ma, mb, d, ta, st);
     if (d.a_kc) return d.b_kc ? launch<true, true>(ma, mb, d, ta, mi, st) : launch<true, false>(ma, mb, d, ta, mi, st);
     return d.b_kc ? launch<false, true>(ma, mb, d, ta, mi, st) : launch<false, false>(ma, mb, d, ta, mi, st);
 }

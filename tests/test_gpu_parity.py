@@ -97,6 +97,39 @@ def test_dgemm_row_split_epilogue(torch_cuda, no, nv, variant):
     assert bool((untouched == -7.0).all())                       # padding rows / columns / unused P slots are never written
 
 
+@pytest.mark.parametrize("rows,no", [(3100, 775), (2960, 370)])
+def test_dgemm_grouped_tile_order(torch_cuda, rows, no):
+    """Eq. 22 with X' shared by the batch and larger than a quarter of L2: the TMA kernel walks its tiles in row groups
+    (gemm_tma.cu, tile_coords<true>).  Several groups with a short last one, ragged M, N, K, the row-split epilogue; against
+    torch and against the cp.async kernel (variant 0), which has no grouped order."""
+    torch = torch_cuda
+    from paper_2603_29257_b200 import load_library
+    lib = load_library()
+    l2 = torch.cuda.get_device_properties(0).L2_cache_size
+    npc, pc, N = 5, 6, 290
+    K = max(1402, (l2 // 4) // (rows * 8) + 2) & ~1
+    assert rows * K * 8 > l2 // 4 and rows % no == 0
+    m = rows // no
+    no_p, ldn = no + (no & 1), N + 2
+    g = torch.Generator(device="cuda").manual_seed(rows)
+    X = torch.randn((rows, K), dtype=torch.float64, device="cuda", generator=g)
+    T = torch.randn((npc, N, K), dtype=torch.float64, device="cuda", generator=g)
+    outs = []
+    for variant in (1, 0):
+        Mout = torch.full((m, pc, no_p, ldn), -7.0, dtype=torch.float64, device="cuda")
+        rc = lib.risp_debug_dgemm(rows, N, K, X.data_ptr(), K, 1, T.data_ptr(), K, 1, Mout.data_ptr(), ldn, 1.0, 0.0,
+                                  npc, 0, N * K, no_p * ldn, variant, no, pc * no_p * ldn, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        assert rc == 0
+        outs.append(Mout)
+    ref = torch.einsum('mjb,pab->mpja', X.reshape(m, no, K), T)
+    got = outs[0][:, :npc, :no, :N]
+    assert float((got - ref).abs().max()) <= 1e-12 * K ** 0.5 * float(ref.abs().max() + 1)
+    assert float((outs[0] - outs[1]).abs().max()) <= 1e-12 * K ** 0.5 * float(ref.abs().max() + 1)
+    untouched = outs[0].clone(); untouched[:, :npc, :no, :N] = -7.0
+    assert bool((untouched == -7.0).all())
+
+
 def test_dgemm_batched(torch_cuda):
     torch = torch_cuda
     from paper_2603_29257_b200 import load_library
