@@ -170,6 +170,36 @@ def _fp32_mode(torch, ctx, X, sigma, flush, stream, steps, warmup, m, d, small):
         del K64, sig64
 
 
+def _fp32_jk_mode(torch, ctx, X, sigma, flush, stream, steps, warmup, m, sig64):
+    """risp_matvec with RISP_PRECISION_FP32_JK: the four AO<->MO transform GEMMs of the J term on the tcgen05 path as well
+    (the paper keeps everything after the integrals in single precision)."""
+    ctx.set_precision(2)
+    try:
+        for _ in range(warmup):
+            ctx.matvec(X, sigma)
+        torch.cuda.synchronize()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        phase = {}
+        for a, b in evs:
+            flush.zero_()
+            a.record(stream)
+            ctx.matvec(X, sigma)
+            b.record(stream)
+            b.synchronize()
+            for k, v in ctx.timings().items():
+                phase[k] = phase.get(k, 0.0) + (v if isinstance(v, float) else 0.0)
+        tim = ctx.timings()
+        t_dev = sum(a.elapsed_time(b) for a, b in evs) * 1e-3
+        return dict(value=m * steps / t_dev, unit=UNIT, ms_per_step=1e3 * t_dev / steps,
+                    dtype="as fp32_mode, and the AO<->MO transforms of the J term (Eq. 12, 17) as bf16x3 operands on tcgen05; integrals, ERI passes, "
+                          "metric solve, diagonal and Davidson algebra FP64",
+                    phases_ms={k: round(1e3 * v / steps, 4) for k, v in phase.items() if k not in ("kernel_launches", "first_chunk_naux")},
+                    gpu_launches=tim["kernel_launches"] * steps,
+                    sigma_rel_diff_vs_fp64=float((sigma - sig64).norm() / sig64.norm()))
+    finally:
+        ctx.set_precision(0)
+
+
 def run_reference(args):
     """The CPU oracle as the reference arm: sigma-builds/s of the oracle on a bounded sample of the same workload."""
     rank = int(os.environ.get("RANK", "0"))
@@ -258,9 +288,13 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
     launches = tim["kernel_launches"] * steps
 
     # ---- the single-precision mode of the K contractions, same batch, same timing rules
-    fp32 = None
+    fp32 = fp32_jk = None
     if rank == 0 and world == 1 and not args.no_fp32 and d["nauxK"] > 0 and (cfg <= 3 or args.fp32_large):
+        sig64_keep = sigma.clone() if cfg <= 3 else None
         fp32 = _fp32_mode(torch, ctx, X, sigma, flush, stream, steps, warmup, m, d, small=cfg <= 3)
+        if cfg <= 3:
+            fp32_jk = _fp32_jk_mode(torch, ctx, X, sigma, flush, stream, steps, warmup, m, sig64_keep)
+        del sig64_keep
 
     # ---- end to end: pinned host buffers through risp_matvec_host
     fp = None
@@ -385,6 +419,8 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
                 r["peak"] = pk16; r["frac"] = r["achieved"] / pk16
                 r["peak_source"] = f"{pk['src']} bf16 cuBLAS throughput ({'sustained' if fp32['ms_per_step'] >= 1000.0 else 'burst'})"
             line["fp32_mode"] = fp32
+            if fp32_jk is not None:
+                line["fp32_jk_mode"] = fp32_jk
         smp = None
         if want_cpu and world == 1 and cfg <= 4:
             ms_ = min(m, 30 if cfg <= 2 else args.ref_vectors)
@@ -444,6 +480,15 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
                                          max_abs_diff_vs_fp64_solve_ev=float(np.abs(np.asarray(om32) - np.asarray(omega)).max() * HARTREE_EV))
                 finally:
                     ctx.set_precision(0)
+                if fp32_jk is not None:
+                    ctx.set_precision(2)
+                    try:
+                        omjk, _, ijk = ctx.tda_solve(s["nroots"], want_vectors=False, flags=flags & ~32, **kw)
+                        fp32_jk["solve"] = dict(wall_s=ijk["sec_total"], matvec_s=ijk["sec_matvec"], iterations=ijk["iterations"], n_sigma=ijk["n_sigma"],
+                                                converged=ijk["converged"], resid_max=float(max(ijk["resid"])), tol=args.solve_tol,
+                                                max_abs_diff_vs_fp64_solve_ev=float(np.abs(np.asarray(omjk) - np.asarray(omega)).max() * HARTREE_EV))
+                    finally:
+                        ctx.set_precision(0)
         res = line
     ctx.close()
     del ctx

@@ -181,9 +181,17 @@ int risp_matvec(risp_ctx *ctx, int32_t m, const double *X_dev, double *sigma_dev
  *                          relative error of order 1e-7 (DESIGN.md "FP32 mode" derives the bound; oracle/risp_fp32.py is the
  *                          plain binary32 contraction it is compared with).  Diagonal, J term and the Davidson algebra stay FP64;
  *                          the K tensors stay stored in FP64.  risp_matvec_tddft returns RISP_EINVAL in this mode.
- * Returns RISP_OK or RISP_EINVAL (unknown mode, or RISP_PRECISION_FP32_K on a device without tcgen05). */
+ *   RISP_PRECISION_FP32_JK RISP_PRECISION_FP32_K, and the four dense AO<->MO transforms of the Coulomb term (Eq. 12, 17;
+ *                          PAPER.md:109, 123) through the same tensor-core GEMM (X, C_occ, C_vir, U and the half-transformed
+ *                          intermediates as three bf16 terms); integrals, both ERI passes, the metric solve, the diagonal and the
+ *                          Davidson algebra stay FP64.  The rounding of the density enters R~ = (P|Q)^-1 R, so J carries a relative
+ *                          error of up to cond(P|Q) x 1e-7.  Used for unsharded TDA sigma-builds whose J
+ *                          work space holds all rows at once (no row panels, one sub-batch); otherwise the transforms silently
+ *                          stay FP64 (slower, more accurate).
+ * Returns RISP_OK or RISP_EINVAL (unknown mode, or a single-precision mode on a device without tcgen05). */
 #define RISP_PRECISION_FP64 0
 #define RISP_PRECISION_FP32_K 1
+#define RISP_PRECISION_FP32_JK 2
 int risp_set_precision(risp_ctx *ctx, int32_t mode);
 
 /* Full TDDFT-risp (Eq. 1-2; XC kernel dropped): for m trial vectors

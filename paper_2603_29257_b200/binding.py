@@ -274,7 +274,8 @@ class RispContext:
         return out
 
     def set_precision(self, mode: int):
-        """0: FP64 (default); 1: the K contractions in the paper's single precision on the tcgen05 tensor cores."""
+        """0: FP64 (default); 1: the K contractions in the paper's single precision on the tcgen05 tensor cores; 2: as 1, and the
+        AO<->MO transforms of the J term as well (RISP_PRECISION_FP32_JK)."""
         self._check(self.lib.risp_set_precision(self.handle, int(mode)))
 
     def force_plan(self, mj: int = 0, prow: int = 0, pc: int = 0):

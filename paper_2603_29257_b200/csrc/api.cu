@@ -10,6 +10,7 @@ extern "C" void risp_destroy(risp_ctx *ctx)
     cudaDeviceSynchronize();
     risp_free_workspace(ctx);
     if (ctx->w_Xin) cudaFree(ctx->w_Xin);
+    if (ctx->q_C) cudaFree(ctx->q_C);
     if (ctx->w_Sout) cudaFree(ctx->w_Sout);
     double **bufs[] = {&ctx->d_Cocc, &ctx->d_CoccT, &ctx->d_Cvir, &ctx->d_eps, &ctx->d_boys, &ctx->d_MJ, &ctx->d_LinvJ, &ctx->d_MK, &ctx->d_MKinv, &ctx->d_TijP,
                        &ctx->d_TabP, &ctx->d_Tov, &ctx->d_LinvK};
@@ -156,7 +157,7 @@ extern "C" int risp_get_stage(risp_ctx *ctx, int32_t which, const int64_t *sel, 
         double *tmp = nullptr;
         RISP_CUDA_TRY(scr.alloc(tmp, n));
         // K' of the last matvec (matvec.cu arena layout: behind X' in FP64 mode, first in the single-precision mode)
-        const double *wKk = ctx->w_arena + (ctx->precision == RISP_PRECISION_FP32_K ? 0 : (size_t)m * ctx->noccK * ctx->nv_p);
+        const double *wKk = ctx->w_arena + (ctx->precision != RISP_PRECISION_FP64 ? 0 : (size_t)m * ctx->noccK * ctx->nv_p);
         RISP_CUDA_TRY(risp_scatter_window(wKk, tmp, m, ctx->nocc, ctx->nvir, ctx->occK0, ctx->noccK, ctx->virK0, ctx->nvirK, ctx->nv_p, 0));
         RISP_CUDA_TRY(cudaMemcpy(out, tmp, n * 8, cudaMemcpyDeviceToHost));
         return RISP_OK;
@@ -228,11 +229,17 @@ extern "C" int risp_debug_dgemm(int M, int N, int K, const double *A, long long 
 extern "C" int risp_set_precision(risp_ctx *ctx, int32_t mode)
 {
     if (!ctx) return RISP_EINVAL;
-    if (mode != RISP_PRECISION_FP64 && mode != RISP_PRECISION_FP32_K) { risp_set_error(ctx, "risp_set_precision: unknown mode"); return RISP_EINVAL; }
-    if (mode == RISP_PRECISION_FP32_K) {
+    if (mode != RISP_PRECISION_FP64 && mode != RISP_PRECISION_FP32_K && mode != RISP_PRECISION_FP32_JK) { risp_set_error(ctx, "risp_set_precision: unknown mode"); return RISP_EINVAL; }
+    if (mode != RISP_PRECISION_FP64) {
         cudaDeviceProp prop;
         RISP_CUDA_TRY(cudaGetDeviceProperties(&prop, ctx->device));
         if (prop.major != 10) { risp_set_error(ctx, "risp_set_precision: the single-precision mode needs the tcgen05 tensor cores (sm_100)"); return RISP_EINVAL; }
+    }
+    if (mode == RISP_PRECISION_FP32_JK && ctx->precision != mode) {
+        // the work space of this mode holds the bf16 planes of the J transforms too: plan it again at the next sigma-build
+        RISP_CUDA_TRY(cudaSetDevice(ctx->device));
+        RISP_CUDA_TRY(cudaDeviceSynchronize());
+        risp_free_workspace(ctx);
     }
     ctx->precision = mode;
     return RISP_OK;

@@ -80,6 +80,7 @@ struct TcGemmDesc {
 cudaError_t risp_tcgemm(const TcGemmDesc &d, cudaStream_t st);
 cudaError_t risp_split_rows_bf3(const double *X, long long ldx, long long rows, int n, void *out, long long ldo, long long plane, int rpg,
                                 long long gstride, cudaStream_t st);
+cudaError_t risp_split_transpose_bf3(const double *X, long long ldx, int rows, int n, void *out, long long ldo, long long plane, cudaStream_t st);
 cudaError_t risp_expand_sym_bf3(const double *packed, long long tri, int n, int np, void *full, long long row_stride, long long p_stride, long long plane,
                                 cudaStream_t st);
 inline GemmDesc gemm_desc(int M, int N, int K, const double *A, long long lda, bool a_kc, const double *B, long long ldb, bool b_kc,

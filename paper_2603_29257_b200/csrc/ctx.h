@@ -102,6 +102,10 @@ struct risp_ctx {
     double *w_J = nullptr;        // [m][nocc][nvir], only with RISP_FLAG_KEEP_STAGES
     double *w_stage[2] = {nullptr, nullptr};      // packed host-resident T chunks in flight
     double *w_Xin = nullptr, *w_Sout = nullptr;   // staging for risp_matvec_host
+    // RISP_PRECISION_FP32_JK: bf16 x 3 planes of the MO coefficients (matvec.cu, built at the first sigma-build in that mode):
+    // C_vir [nao][nvir_q], C_occ [nao][nocc_q], C_occ^T [nocc][nao_q], C_vir^T [nvir][nao_q]; rows padded to 8 elements
+    unsigned short *q_C = nullptr;
+    int q_C_failed = 0;
     int xin_cap = 0;
     size_t w_bytes = 0, setup_bytes = 0;
     int last_m = 0;

@@ -552,6 +552,32 @@ __global__ void __launch_bounds__(256) split_rows_kernel(const double *__restric
     }
 }
 
+// X^T (FP64 [rows][ldx], n columns) -> three bf16 planes out[p*plane + c*ldo + r], 32 x 32 tiles through shared memory; the padding
+// columns r in [rows, ldo) of every output row are zeroed
+__global__ void __launch_bounds__(256) split_transpose_kernel(const double *__restrict__ X, long long ldx, int rows, int n, __nv_bfloat16 *__restrict__ out,
+                                                              long long ldo, long long plane)
+{
+    __shared__ double s[32][33];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int r0 = blockIdx.x * 32, c0 = blockIdx.y * 32;
+    for (int rr = ty; rr < 32; rr += 8) {
+        const int r = r0 + rr, c = c0 + tx;
+        s[rr][tx] = (r < rows && c < n) ? X[(long long)r * ldx + c] : 0.0;
+    }
+    __syncthreads();
+    for (int cc = ty; cc < 32; cc += 8) {
+        const int c = c0 + cc, r = r0 + tx;
+        if (c < n && r < ldo) {
+            const double v = s[tx][cc];
+            const __nv_bfloat16 b1 = __double2bfloat16(v);
+            const double r1 = v - (double)__bfloat162float(b1);
+            const __nv_bfloat16 b2 = __double2bfloat16(r1);
+            __nv_bfloat16 *o = out + (long long)c * ldo + r;
+            o[0] = b1; o[plane] = b2; o[2 * plane] = __double2bfloat16(r1 - (double)__bfloat162float(b2));
+        }
+    }
+}
+
 // full[p*p_stride + r*row_stride + c] = packed[p][max(r,c), min(r,c)] as three bf16 planes (the tiling of expand_sym_kernel)
 __global__ void __launch_bounds__(256) expand_sym_bf3_kernel(const double *__restrict__ packed, long long tri, int n, __nv_bfloat16 *__restrict__ full,
                                                              long long row_stride, long long p_stride, long long plane)
@@ -593,6 +619,14 @@ cudaError_t risp_split_rows_bf3(const double *X, long long ldx, long long rows, 
 {
     if (rows <= 0 || ldo <= 0) return cudaSuccess;
     split_rows_kernel<<<(unsigned)std::min<long long>(rows, 148 * 32), 256, 0, st>>>(X, ldx, rows, n, (__nv_bfloat16 *)out, ldo, plane, rpg, gstride);
+    return cudaGetLastError();
+}
+
+cudaError_t risp_split_transpose_bf3(const double *X, long long ldx, int rows, int n, void *out, long long ldo, long long plane, cudaStream_t st)
+{
+    if (rows <= 0 || n <= 0) return cudaSuccess;
+    dim3 grid((unsigned)((ldo + 31) / 32), (unsigned)((n + 31) / 32));
+    split_transpose_kernel<<<grid, 256, 0, st>>>(X, ldx, rows, n, (__nv_bfloat16 *)out, ldo, plane);
     return cudaGetLastError();
 }
 

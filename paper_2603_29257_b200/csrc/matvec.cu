@@ -90,6 +90,12 @@ size_t risp_plan_workspace(const risp_ctx *ctx, int m, size_t avail, MatvecPlan 
     }
     pl.mj = mj; pl.prow = (int)prow_max;
     pl.arena_bytes = std::max(karena, jneed(mj, prow_max));
+    if (ctx->precision == RISP_PRECISION_FP32_JK && mj == m && prow_max >= nao) {
+        // bf16 x 3 planes of X, Y^T / Z and U behind the FP64 D / U block (risp_matvec_impl); without room for them the J transforms stay FP64
+        const size_t nvir_q = ((size_t)ctx->nvir + 7) & ~(size_t)7, nocc_q = (nocc + 7) & ~(size_t)7, nao_q = (nao + 7) & ~(size_t)7;
+        const size_t j32 = jneed(m, nao) + 6 * (size_t)m * (nocc * nvir_q + std::max(nao * nocc_q, nocc * nao_q) + nao * nao_q) + 64;
+        if (j32 <= std::max(jlimit, karena)) pl.arena_bytes = std::max(pl.arena_bytes, j32);
+    }
     return pl.arena_bytes + (ctx->has_K ? pl.pc * stage_per_fn : 0);
 }
 
@@ -170,6 +176,28 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
     cudaEvent_t *ev = ctx->ev;
     double *wY = ctx->w_arena;                                   // [mj][nocc][ldao]   (J-phase views of the arena)
     double *wD = wY + (size_t)pl.mj * nocc * ldao;               // [mj][prow][ldao]
+    // RISP_PRECISION_FP32_JK: the four AO<->MO GEMMs on the tcgen05 path (gemm_tc.cu).  bf16 x 3 planes behind wD:
+    //   qX [m nocc][nvir_q]   qH [m][nao][nocc_q] (Y^T), later [m][nocc][nao_q] (Z)   qU [m][nao][nao_q]
+    const long long nvir_q = (nvir + 7) & ~7, nocc_q = (nocc + 7) & ~7, nao_q = (nao + 7) & ~7;
+    const long long plX = (long long)m * nocc * nvir_q, plH = (long long)m * std::max((long long)nao * nocc_q, (long long)nocc * nao_q),
+                    plU = (long long)m * nao * nao_q;
+    const long long plCv = (long long)nao * nvir_q, plCo = (long long)nao * nocc_q, plCoT = (long long)nocc * nao_q, plCvT = (long long)nvir * nao_q;
+    unsigned short *qX = (unsigned short *)(((size_t)(wD + (size_t)pl.mj * nao * ldao) + 15) & ~(size_t)15), *qH = qX + 3 * plX, *qU = qH + 3 * plH;
+    bool f32j = ctx->precision == RISP_PRECISION_FP32_JK && phase == 0 && !tddft && dense && pl.mj >= m && !ctx->q_C_failed &&
+                (size_t)((char *)(qU + 3 * plU) - (char *)ctx->w_arena) <= ctx->plan.arena_bytes;
+    if (f32j && !ctx->q_C) {
+        // the MO coefficients as bf16 x 3 planes, once per context; if they do not fit the transforms stay FP64
+        const size_t bytes = (size_t)6 * (plCv + plCo + plCoT + plCvT) + 64;
+        if (cudaMalloc((void **)&ctx->q_C, bytes) != cudaSuccess) { (void)cudaGetLastError(); ctx->q_C = nullptr; ctx->q_C_failed = 1; f32j = false; }
+        else {
+            unsigned short *c = ctx->q_C;
+            RISP_CUDA_TRY(risp_split_rows_bf3(ctx->d_Cvir, ldvir, nao, nvir, c, nvir_q, plCv, 0, 0, st)); c += 3 * plCv;
+            RISP_CUDA_TRY(risp_split_rows_bf3(ctx->d_Cocc, ldocc, nao, nocc, c, nocc_q, plCo, 0, 0, st)); c += 3 * plCo;
+            RISP_CUDA_TRY(risp_split_rows_bf3(ctx->d_CoccT, ldao, nocc, nao, c, nao_q, plCoT, 0, 0, st)); c += 3 * plCoT;
+            RISP_CUDA_TRY(risp_split_transpose_bf3(ctx->d_Cvir, ldvir, nao, nvir, c, nao_q, plCvT, st));
+        }
+    }
+    const unsigned short *qCv = ctx->q_C, *qCo = qCv + 3 * plCv, *qCoT = qCo + 3 * plCo, *qCvT = qCoT + 3 * plCoT;
     if (phase == 2) goto after_pass1;
     RISP_CUDA_TRY(cudaEventRecord(ev[0], st));
     if (phase == 1) goto density;
@@ -183,15 +211,34 @@ density:
     for (int l0 = 0; l0 < m; l0 += pl.mj) {
         const int mj = std::min(pl.mj, m - l0);
         const double *Xb = X + (size_t)l0 * nocc * nvir;
-        GemmDesc d = gemm_desc(mj * nocc, nao, nvir, Xb, nvir, true, ctx->d_Cvir, ldvir, true, wY, ldao);
-        RISP_CUDA_TRY(risp_dgemm(d, st)); ++launches;
+        if (f32j) {
+            // Y^T[mi][nu][i] = sum_a X[(mi, i)][a] C_vir[nu][a] (rows split by trial vector), then D[mi][mu][nu] = sum_i Y^T[mi][nu][i] C_occ[mu][i]
+            RISP_CUDA_TRY(risp_split_rows_bf3(Xb, nvir, (long long)m * nocc, nvir, qX, nvir_q, plX, 0, 0, st)); ++launches;
+            TcGemmDesc d;
+            d.M = m * nocc; d.N = nao; d.K = nvir; d.nb = 1;
+            d.A = qX; d.lda = nvir_q; d.planeA = plX; d.sA = 0;
+            d.B = qCv; d.ldb = nvir_q; d.planeB = plCv; d.sB = 0;
+            d.C = qH; d.ldc = nocc_q; d.sC = 0; d.planeC = plH; d.out_kind = 1; d.rpg = nocc; d.gstride = (long long)nao * nocc_q; d.accumulate = 0; d.shape = 2;
+            RISP_CUDA_TRY(risp_tcgemm(d, st)); ++launches;
+            TcGemmDesc e;
+            e.M = nao; e.N = nao; e.K = nocc; e.nb = m;
+            e.A = qH; e.lda = nocc_q; e.planeA = plH; e.sA = (long long)nao * nocc_q;
+            e.B = qCo; e.ldb = nocc_q; e.planeB = plCo; e.sB = 0;
+            e.C = wD; e.ldc = ldao; e.sC = (long long)nao * ldao; e.planeC = 0; e.out_kind = 0; e.rpg = 0; e.gstride = 0; e.accumulate = 0; e.shape = 2;
+            RISP_CUDA_TRY(risp_tcgemm(e, st)); ++launches;
+        } else {
+            GemmDesc d = gemm_desc(mj * nocc, nao, nvir, Xb, nvir, true, ctx->d_Cvir, ldvir, true, wY, ldao);
+            RISP_CUDA_TRY(risp_dgemm(d, st)); ++launches;
+        }
         for (int p = 0; p < npanel; ++p) {
             const int r0 = pl.panel_r0[p], r1 = pl.panel_r0[p + 1], pr = r1 - r0;
             const long long mstride = (long long)pr * ldao;
-            // D[mu in panel][nu] = sum_i C_occ[mu][i] Y[i][nu]
-            GemmDesc e = gemm_desc(pr, nao, nocc, ctx->d_Cocc + (size_t)r0 * ldocc, ldocc, true, wY, ldao, false, wD, ldao);
-            e.nb1 = mj; e.sB1 = (long long)nocc * ldao; e.sC1 = mstride;
-            RISP_CUDA_TRY(risp_dgemm(e, st)); ++launches;
+            if (!f32j) {
+                // D[mu in panel][nu] = sum_i C_occ[mu][i] Y[i][nu]
+                GemmDesc e = gemm_desc(pr, nao, nocc, ctx->d_Cocc + (size_t)r0 * ldocc, ldocc, true, wY, ldao, false, wD, ldao);
+                e.nb1 = mj; e.sB1 = (long long)nocc * ldao; e.sC1 = mstride;
+                RISP_CUDA_TRY(risp_dgemm(e, st)); ++launches;
+            }
             if ((rc = fork_classes(ctx, st))) return rc;
             for (int c = 0; c < 6; ++c) {
                 const PairClass &pc = ctx->cls[c];
@@ -255,12 +302,33 @@ after_pass1:
                 }
             }
             if ((rc = join_classes(ctx, st))) return rc;
+            if (f32j) continue;
             // Z[i][nu] (+)= sum_{mu in panel} C_occ[mu][i] U[mu][nu]
             GemmDesc d = gemm_desc(nocc, nao, pr, ctx->d_CoccT + r0, ldao, true, wD, ldao, false, wY, ldao, 1.0, p == 0 ? 0.0 : 1.0);
             d.nb1 = mj; d.sB1 = mstride; d.sC1 = (long long)nocc * ldao;
             RISP_CUDA_TRY(risp_dgemm(d, st)); ++launches;
         }
         double *Sb = sigma + (size_t)l0 * nocc * nvir;
+        if (f32j) {
+            // U is symmetric: Z[mi][i][nu] = sum_mu U[mi][nu][mu] C_occ^T[i][mu], then J[(mi, i)][a] = sum_nu C_vir^T[a][nu] Z[(mi, i)][nu];
+            // J lands in the (free) Y region or in the stage buffer, sigma += 2 J
+            RISP_CUDA_TRY(risp_split_rows_bf3(wD, ldao, (long long)m * nao, nao, qU, nao_q, plU, 0, 0, st)); ++launches;
+            TcGemmDesc d;
+            d.M = nao; d.N = nocc; d.K = nao; d.nb = m;
+            d.A = qU; d.lda = nao_q; d.planeA = plU; d.sA = (long long)nao * nao_q;
+            d.B = qCoT; d.ldb = nao_q; d.planeB = plCoT; d.sB = 0;
+            d.C = qH; d.ldc = nao_q; d.sC = (long long)nocc * nao_q; d.planeC = plH; d.out_kind = 1; d.rpg = 0; d.gstride = 0; d.accumulate = 0; d.shape = 2;
+            RISP_CUDA_TRY(risp_tcgemm(d, st)); ++launches;
+            double *Jb = ctx->w_J ? ctx->w_J + (size_t)l0 * nocc * nvir : wY;
+            TcGemmDesc e;
+            e.M = nvir; e.N = m * nocc; e.K = nao; e.nb = 1;
+            e.A = qCvT; e.lda = nao_q; e.planeA = plCvT; e.sA = 0;
+            e.B = qH; e.ldb = nao_q; e.planeB = plH; e.sB = 0;
+            e.C = Jb; e.ldc = nvir; e.sC = 0; e.planeC = 0; e.out_kind = 0; e.rpg = 0; e.gstride = 0; e.accumulate = 0; e.shape = 2;
+            RISP_CUDA_TRY(risp_tcgemm(e, st)); ++launches;
+            RISP_CUDA_TRY(risp_axpy_window(Jb, 2.0, Sb, m, nocc, nvir, 0, nocc, 0, nvir, nvir, st)); ++launches;
+            continue;
+        }
         if (ctx->w_J) {
             GemmDesc e = gemm_desc(mj * nocc, nvir, nao, wY, ldao, true, ctx->d_Cvir, ldvir, false, ctx->w_J + (size_t)l0 * nocc * nvir, nvir);
             RISP_CUDA_TRY(risp_dgemm(e, st)); ++launches;
@@ -272,7 +340,7 @@ after_pass1:
     RISP_CUDA_TRY(cudaEventRecord(ev[5], st));
     // ---------------- K (Eq. 22-23)
     if (ctx->has_K) {
-        const bool f32 = ctx->precision == RISP_PRECISION_FP32_K;
+        const bool f32 = ctx->precision != RISP_PRECISION_FP64;
         if (f32 && tddft) { risp_set_error(ctx, "risp_matvec_tddft: the single-precision mode covers the TDA sigma-build only"); return RISP_EINVAL; }
         int pc = pl.pc;
         double *wXk = ctx->w_arena;                                  // [m][no][nv_p]

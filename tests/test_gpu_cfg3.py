@@ -96,3 +96,30 @@ def test_cfg3_roots(cfg3):
           f"max |d omega| over the lowest 15 = {np.abs(omega2[:n] - omega).max() * HARTREE_EV:.2e} eV", flush=True)
     assert info2["converged"] == 1
     assert np.abs(omega2[:n] - omega).max() * HARTREE_EV <= 1e-6
+
+
+def test_cfg3_single_precision_modes(cfg3):
+    """RISP_PRECISION_FP32_K and RISP_PRECISION_FP32_JK at 300 atoms against the FULL FP64 oracle: K inside the binary32 bound of
+    tests/test_gpu_fp32.py (1e-6 normwise), J bit-for-bit FP64 accuracy in the K-only mode and within (2 cond (P|Q)_J + 2) x 1e-6 with
+    the transforms on the tcgen05 path."""
+    import torch
+    from workloads import trial_vectors
+    s, o, c = cfg3
+    m = 6
+    X = trial_vectors(s, m)
+    sig_ref, dg, J_ref, K_ref = o.sigma(X, parts=True)
+    Xd = torch.from_numpy(X).cuda()
+    cond = np.linalg.cond(o.MJ)
+    try:
+        c.set_precision(1)
+        sig1 = c.matvec(Xd).cpu().numpy()
+        eJ1, eK1, eS1 = _rel(c.stage("J", m), J_ref), _rel(c.stage("K", m), K_ref), _rel(sig1, sig_ref)
+        c.set_precision(2)
+        sig2 = c.matvec(Xd).cpu().numpy()
+        eJ2, eK2, eS2 = _rel(c.stage("J", m), J_ref), _rel(c.stage("K", m), K_ref), _rel(sig2, sig_ref)
+    finally:
+        c.set_precision(0)
+    print(f"[cfg3-full] FP32_K : |dJ|/|J| = {eJ1:.2e}, |dK|/|K| = {eK1:.2e}, |dsigma|/|sigma| = {eS1:.2e}", flush=True)
+    print(f"[cfg3-full] FP32_JK: |dJ|/|J| = {eJ2:.2e}, |dK|/|K| = {eK2:.2e}, |dsigma|/|sigma| = {eS2:.2e}; cond (P|Q)_J = {cond:.2e}", flush=True)
+    assert eJ1 <= 1e-10 and 1e-12 < eK1 <= 1e-6 and eS1 <= 1e-6
+    assert 1e-12 < eJ2 <= (2 * cond + 2) * 1e-6 and 1e-12 < eK2 <= 1e-6 and eS2 <= (2 * cond + 3) * 1e-6

@@ -140,6 +140,82 @@ def test_fp32_mode_cfg2_roots(cfg2):
     assert d <= 1e-4
 
 
+# ------------------------------------------------------------------------------------------------ RISP_PRECISION_FP32_JK
+# Tolerance of the J term in this mode (J transforms): each of the four transform GEMMs carries the
+# normwise error of a binary32 product, eps = 1e-6 (the bound used for the K term above); the two of the forward transform
+# reach R~ = (P|Q)_J^-1 R, whose relative error is at most cond((P|Q)_J) times that of R, the two of the back-transform add theirs:
+#     ||dJ|| / ||J|| <= (2 cond + 2) eps
+_EPS32 = 1e-6
+
+
+def _check_mode_jk(torch, s, o, c, m):
+    from workloads import trial_vectors
+    from oracle.risp_fp32 import exchange_error_bound
+    X = trial_vectors(s)[:m]
+    Xd = torch.from_numpy(X).cuda()
+    sig_ref, dg, J_ref, K_ref = o.sigma(X, parts=True)
+    c.set_precision(1)
+    try:
+        sig_k = c.matvec(Xd).cpu().numpy()
+        K_k = c.stage("K", m)
+        c.set_precision(2)
+        sig32 = c.matvec(Xd).cpu().numpy()
+        K32 = c.stage("K", m)
+        J32 = c.stage("J", m)
+    finally:
+        c.set_precision(0)
+    assert np.linalg.norm(K32 - K_k) <= 1e-12 * np.linalg.norm(K_k)    # the K term is that of RISP_PRECISION_FP32_K (up to the aux chunking)
+    assert np.all(np.abs(K32 - K_ref) <= exchange_error_bound(o, X) + 1e-300)
+    cond = np.linalg.cond(o.MJ)
+    relJ = np.linalg.norm(J32 - J_ref) / np.linalg.norm(J_ref)
+    assert relJ > 1e-12                                   # the mode is on (no silent FP64 fallback at these sizes)
+    assert relJ <= (2 * cond + 2) * _EPS32
+    rel_sig = np.linalg.norm(sig32 - sig_ref) / np.linalg.norm(sig_ref)
+    assert rel_sig <= (2 * cond + 3) * _EPS32
+    # sigma is assembled from the same terms as in the K-only mode: diagonal and K identical, J as checked
+    assert np.linalg.norm((sig32 - sig_k) - 2 * (J32 - J_ref)) <= 1e-9 * np.linalg.norm(sig_ref)
+    return relJ, rel_sig, cond
+
+
+def test_fp32_jk_mode_small(torch_cuda, sys_small_rsh, oracle_small_rsh):
+    from paper_2603_29257_b200 import setup
+    c = setup(sys_small_rsh, flags=1)
+    try:
+        relJ, rel_sig, cond = _check_mode_jk(torch_cuda, sys_small_rsh, oracle_small_rsh, c, 5)
+        print(f"12-atom system, single-precision J transforms: J rel error {relJ:.3e}, sigma {rel_sig:.3e}, cond(P|Q)_J {cond:.2e}")
+        # row panels: the transforms stay FP64 (documented fallback), the K term stays single precision
+        from workloads import trial_vectors
+        X = trial_vectors(sys_small_rsh)[:3]
+        _, _, J_ref, _ = oracle_small_rsh.sigma(X, parts=True)
+        c.force_plan(0, 16, 0)
+        c.set_precision(2)
+        c.matvec(torch_cuda.from_numpy(X).cuda())
+        assert np.linalg.norm(c.stage("J", 3) - J_ref) / np.linalg.norm(J_ref) <= 1e-10
+    finally:
+        c.set_precision(0)
+        c.close()
+
+
+def test_fp32_jk_mode_cfg2_sigma(torch_cuda, cfg2):
+    s, o, c = cfg2
+    relJ, rel_sig, cond = _check_mode_jk(torch_cuda, s, o, c, 30)
+    print(f"cfg2 single-precision J transforms: J rel error {relJ:.3e}, sigma {rel_sig:.3e}, cond(P|Q)_J {cond:.2e}")
+
+
+def test_fp32_jk_mode_cfg2_roots(cfg2):
+    s, o, c = cfg2
+    th_ref, _, info_ref = o.davidson(15, tol=1e-8)
+    c.set_precision(2)
+    try:
+        omega, _, info = c.tda_solve(15, tol=1e-5)
+    finally:
+        c.set_precision(0)
+    assert info["converged"] == 1
+    d = np.abs(omega - th_ref).max() * HARTREE_EV
+    print(f"cfg2 single-precision J and K roots: max deviation {d:.3e} eV")
+    assert d <= 1e-4
+
+
 def test_fp32_mode_host_spilled_slices(torch_cuda, sys_small_rsh, oracle_small_rsh):
     from paper_2603_29257_b200 import setup
     c = setup(sys_small_rsh, flags=1 | 2)          # RISP_FLAG_SPILL_HALF: half of the K slices stream from pinned host memory
