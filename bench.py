@@ -290,10 +290,11 @@ def run_config(cfg, args, world, rank, local, dist, want_solve, want_cpu, steps,
     # ---- the single-precision mode of the K contractions, same batch, same timing rules
     fp32 = fp32_jk = None
     if rank == 0 and world == 1 and not args.no_fp32 and d["nauxK"] > 0 and (cfg <= 3 or args.fp32_large):
-        sig64_keep = sigma.clone() if cfg <= 3 else None
+        sig64_keep = sigma.clone() if cfg <= 4 else None
         fp32 = _fp32_mode(torch, ctx, X, sigma, flush, stream, steps, warmup, m, d, small=cfg <= 3)
-        if cfg <= 3:
+        if cfg <= 4:
             fp32_jk = _fp32_jk_mode(torch, ctx, X, sigma, flush, stream, steps, warmup, m, sig64_keep)
+            fp32_jk["j_sub_batch"] = ctx.dims()["j_sub_batch"]
         del sig64_keep
 
     # ---- end to end: pinned host buffers through risp_matvec_host

@@ -185,9 +185,10 @@ int risp_matvec(risp_ctx *ctx, int32_t m, const double *X_dev, double *sigma_dev
  *                          PAPER.md:109, 123) through the same tensor-core GEMM (X, C_occ, C_vir, U and the half-transformed
  *                          intermediates as three bf16 terms); integrals, both ERI passes, the metric solve, the diagonal and the
  *                          Davidson algebra stay FP64.  The rounding of the density enters R~ = (P|Q)^-1 R, so J carries a relative
- *                          error of up to cond(P|Q) x 1e-7.  Used for unsharded TDA sigma-builds whose J
- *                          work space holds all rows at once (no row panels, one sub-batch); otherwise the transforms silently
- *                          stay FP64 (slower, more accurate).
+ *                          error of up to (2 cond(P|Q) + 2) x 1e-6 (measured 1e-5 at cond 9e4).  Used for
+ *                          unsharded TDA sigma-builds whose J work space holds all AO rows of a sub-batch at once; with row
+ *                          panels (3000 atoms on one GPU) and in the sharded sigma-build the transforms stay FP64 (slower,
+ *                          more accurate).
  * Returns RISP_OK or RISP_EINVAL (unknown mode, or a single-precision mode on a device without tcgen05). */
 #define RISP_PRECISION_FP64 0
 #define RISP_PRECISION_FP32_K 1

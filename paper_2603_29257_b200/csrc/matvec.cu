@@ -69,6 +69,20 @@ size_t risp_plan_workspace(const risp_ctx *ctx, int m, size_t avail, MatvecPlan 
     }
     if (ctx->force_mj > 0) mj = std::min(ctx->force_mj, m);
     if (ctx->force_prow > 0) prow = std::min<size_t>(ctx->force_prow, nao);
+    // RISP_PRECISION_FP32_JK: bf16 x 3 planes of X, Y^T / Z and U behind the FP64 D / U block (risp_matvec_impl), all AO rows at once;
+    // the largest sub-batch whose planes fit is taken, and without room for a single vector the J transforms stay FP64
+    auto j32need = [&](size_t mj_) {
+        const size_t nvir_q = ((size_t)ctx->nvir + 7) & ~(size_t)7, nocc_q = (nocc + 7) & ~(size_t)7, nao_q = (nao + 7) & ~(size_t)7;
+        return jneed(mj_, nao) + 6 * mj_ * (nocc * nvir_q + std::max(nao * nocc_q, nocc * nao_q) + nao * nao_q) + 64;
+    };
+    bool jk = false;
+    if (ctx->precision == RISP_PRECISION_FP32_JK && ctx->force_prow <= 0) {
+        const int mtop = ctx->force_mj > 0 ? std::min(ctx->force_mj, m) : m;
+        for (int div = 1; div <= mtop && !jk; ++div) {
+            const int mj2 = (mtop + div - 1) / div;
+            if (j32need(mj2) <= std::max(jlimit, karena)) { mj = mj2; prow = nao; jk = true; }
+        }
+    }
     // panel boundaries: even, shell-aligned AO offsets (TMA coordinates of the MN-contiguous operand must be 16-byte aligned)
     pl.panel_r0.clear();
     pl.panel_r0.push_back(0);
@@ -90,12 +104,7 @@ size_t risp_plan_workspace(const risp_ctx *ctx, int m, size_t avail, MatvecPlan 
     }
     pl.mj = mj; pl.prow = (int)prow_max;
     pl.arena_bytes = std::max(karena, jneed(mj, prow_max));
-    if (ctx->precision == RISP_PRECISION_FP32_JK && mj == m && prow_max >= nao) {
-        // bf16 x 3 planes of X, Y^T / Z and U behind the FP64 D / U block (risp_matvec_impl); without room for them the J transforms stay FP64
-        const size_t nvir_q = ((size_t)ctx->nvir + 7) & ~(size_t)7, nocc_q = (nocc + 7) & ~(size_t)7, nao_q = (nao + 7) & ~(size_t)7;
-        const size_t j32 = jneed(m, nao) + 6 * (size_t)m * (nocc * nvir_q + std::max(nao * nocc_q, nocc * nao_q) + nao * nao_q) + 64;
-        if (j32 <= std::max(jlimit, karena)) pl.arena_bytes = std::max(pl.arena_bytes, j32);
-    }
+    if (jk) pl.arena_bytes = std::max(pl.arena_bytes, j32need(mj));
     return pl.arena_bytes + (ctx->has_K ? pl.pc * stage_per_fn : 0);
 }
 
@@ -177,13 +186,12 @@ int risp_matvec_impl(risp_ctx *ctx, int m, const double *X, double *sigma, cudaS
     double *wY = ctx->w_arena;                                   // [mj][nocc][ldao]   (J-phase views of the arena)
     double *wD = wY + (size_t)pl.mj * nocc * ldao;               // [mj][prow][ldao]
     // RISP_PRECISION_FP32_JK: the four AO<->MO GEMMs on the tcgen05 path (gemm_tc.cu).  bf16 x 3 planes behind wD:
-    //   qX [m nocc][nvir_q]   qH [m][nao][nocc_q] (Y^T), later [m][nocc][nao_q] (Z)   qU [m][nao][nao_q]
-    const long long nvir_q = (nvir + 7) & ~7, nocc_q = (nocc + 7) & ~7, nao_q = (nao + 7) & ~7;
-    const long long plX = (long long)m * nocc * nvir_q, plH = (long long)m * std::max((long long)nao * nocc_q, (long long)nocc * nao_q),
-                    plU = (long long)m * nao * nao_q;
+    //   qX [mq nocc][nvir_q]   qH [mq][nao][nocc_q] (Y^T), later [mq][nocc][nao_q] (Z)   qU [mq][nao][nao_q],   mq = vectors per sub-batch
+    const long long nvir_q = (nvir + 7) & ~7, nocc_q = (nocc + 7) & ~7, nao_q = (nao + 7) & ~7, mq = std::min(pl.mj, m);
+    const long long plX = mq * nocc * nvir_q, plH = mq * std::max((long long)nao * nocc_q, (long long)nocc * nao_q), plU = mq * nao * nao_q;
     const long long plCv = (long long)nao * nvir_q, plCo = (long long)nao * nocc_q, plCoT = (long long)nocc * nao_q, plCvT = (long long)nvir * nao_q;
     unsigned short *qX = (unsigned short *)(((size_t)(wD + (size_t)pl.mj * nao * ldao) + 15) & ~(size_t)15), *qH = qX + 3 * plX, *qU = qH + 3 * plH;
-    bool f32j = ctx->precision == RISP_PRECISION_FP32_JK && phase == 0 && !tddft && dense && pl.mj >= m && !ctx->q_C_failed &&
+    bool f32j = ctx->precision == RISP_PRECISION_FP32_JK && phase == 0 && !tddft && dense && !ctx->q_C_failed &&
                 (size_t)((char *)(qU + 3 * plU) - (char *)ctx->w_arena) <= ctx->plan.arena_bytes;
     if (f32j && !ctx->q_C) {
         // the MO coefficients as bf16 x 3 planes, once per context; if they do not fit the transforms stay FP64
@@ -213,15 +221,15 @@ density:
         const double *Xb = X + (size_t)l0 * nocc * nvir;
         if (f32j) {
             // Y^T[mi][nu][i] = sum_a X[(mi, i)][a] C_vir[nu][a] (rows split by trial vector), then D[mi][mu][nu] = sum_i Y^T[mi][nu][i] C_occ[mu][i]
-            RISP_CUDA_TRY(risp_split_rows_bf3(Xb, nvir, (long long)m * nocc, nvir, qX, nvir_q, plX, 0, 0, st)); ++launches;
+            RISP_CUDA_TRY(risp_split_rows_bf3(Xb, nvir, (long long)mj * nocc, nvir, qX, nvir_q, plX, 0, 0, st)); ++launches;
             TcGemmDesc d;
-            d.M = m * nocc; d.N = nao; d.K = nvir; d.nb = 1;
+            d.M = mj * nocc; d.N = nao; d.K = nvir; d.nb = 1;
             d.A = qX; d.lda = nvir_q; d.planeA = plX; d.sA = 0;
             d.B = qCv; d.ldb = nvir_q; d.planeB = plCv; d.sB = 0;
             d.C = qH; d.ldc = nocc_q; d.sC = 0; d.planeC = plH; d.out_kind = 1; d.rpg = nocc; d.gstride = (long long)nao * nocc_q; d.accumulate = 0; d.shape = 2;
             RISP_CUDA_TRY(risp_tcgemm(d, st)); ++launches;
             TcGemmDesc e;
-            e.M = nao; e.N = nao; e.K = nocc; e.nb = m;
+            e.M = nao; e.N = nao; e.K = nocc; e.nb = mj;
             e.A = qH; e.lda = nocc_q; e.planeA = plH; e.sA = (long long)nao * nocc_q;
             e.B = qCo; e.ldb = nocc_q; e.planeB = plCo; e.sB = 0;
             e.C = wD; e.ldc = ldao; e.sC = (long long)nao * ldao; e.planeC = 0; e.out_kind = 0; e.rpg = 0; e.gstride = 0; e.accumulate = 0; e.shape = 2;
@@ -312,21 +320,21 @@ after_pass1:
         if (f32j) {
             // U is symmetric: Z[mi][i][nu] = sum_mu U[mi][nu][mu] C_occ^T[i][mu], then J[(mi, i)][a] = sum_nu C_vir^T[a][nu] Z[(mi, i)][nu];
             // J lands in the (free) Y region or in the stage buffer, sigma += 2 J
-            RISP_CUDA_TRY(risp_split_rows_bf3(wD, ldao, (long long)m * nao, nao, qU, nao_q, plU, 0, 0, st)); ++launches;
+            RISP_CUDA_TRY(risp_split_rows_bf3(wD, ldao, (long long)mj * nao, nao, qU, nao_q, plU, 0, 0, st)); ++launches;
             TcGemmDesc d;
-            d.M = nao; d.N = nocc; d.K = nao; d.nb = m;
+            d.M = nao; d.N = nocc; d.K = nao; d.nb = mj;
             d.A = qU; d.lda = nao_q; d.planeA = plU; d.sA = (long long)nao * nao_q;
             d.B = qCoT; d.ldb = nao_q; d.planeB = plCoT; d.sB = 0;
             d.C = qH; d.ldc = nao_q; d.sC = (long long)nocc * nao_q; d.planeC = plH; d.out_kind = 1; d.rpg = 0; d.gstride = 0; d.accumulate = 0; d.shape = 2;
             RISP_CUDA_TRY(risp_tcgemm(d, st)); ++launches;
             double *Jb = ctx->w_J ? ctx->w_J + (size_t)l0 * nocc * nvir : wY;
             TcGemmDesc e;
-            e.M = nvir; e.N = m * nocc; e.K = nao; e.nb = 1;
+            e.M = nvir; e.N = mj * nocc; e.K = nao; e.nb = 1;
             e.A = qCvT; e.lda = nao_q; e.planeA = plCvT; e.sA = 0;
             e.B = qH; e.ldb = nao_q; e.planeB = plH; e.sB = 0;
             e.C = Jb; e.ldc = nvir; e.sC = 0; e.planeC = 0; e.out_kind = 0; e.rpg = 0; e.gstride = 0; e.accumulate = 0; e.shape = 2;
             RISP_CUDA_TRY(risp_tcgemm(e, st)); ++launches;
-            RISP_CUDA_TRY(risp_axpy_window(Jb, 2.0, Sb, m, nocc, nvir, 0, nocc, 0, nvir, nvir, st)); ++launches;
+            RISP_CUDA_TRY(risp_axpy_window(Jb, 2.0, Sb, mj, nocc, nvir, 0, nocc, 0, nvir, nvir, st)); ++launches;
             continue;
         }
         if (ctx->w_J) {

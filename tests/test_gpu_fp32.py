@@ -183,6 +183,11 @@ def test_fp32_jk_mode_small(torch_cuda, sys_small_rsh, oracle_small_rsh):
     try:
         relJ, rel_sig, cond = _check_mode_jk(torch_cuda, sys_small_rsh, oracle_small_rsh, c, 5)
         print(f"12-atom system, single-precision J transforms: J rel error {relJ:.3e}, sigma {rel_sig:.3e}, cond(P|Q)_J {cond:.2e}")
+        # sub-batches of two vectors (2, 2, 1): the planes of one sub-batch at a time
+        c.force_plan(2, 0, 0)
+        relJ2, _, _ = _check_mode_jk(torch_cuda, sys_small_rsh, oracle_small_rsh, c, 5)
+        assert c.dims()["j_sub_batch"] == 2 and relJ2 <= 4 * relJ
+        c.force_plan(0, 0, 0)
         # row panels: the transforms stay FP64 (documented fallback), the K term stays single precision
         from workloads import trial_vectors
         X = trial_vectors(sys_small_rsh)[:3]
